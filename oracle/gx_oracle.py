@@ -1,0 +1,408 @@
+"""fp64 CPU oracle for the nonlinear E×B term of the Fourier-Laguerre-Hermite gyrokinetic
+system (arxiv 2209.06731, "GX").  TEST INFRASTRUCTURE ONLY.
+
+Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s cpu_baseline / ``--impl
+reference`` legs may import this file.  It shares no code with the CUDA path
+(``paper_2209_06731_b200/csrc``) and imports nothing from the package: every function takes
+plain numpy arrays.  Everything is float64 / complex128, written in the paper's order and
+notation so that it can be checked against PAPER.md by eye.  "P:nnn" = PAPER.md line nnn.
+
+What is computed (App. D Eq. D1 first line; Eq. 4.19), for every
+species s, Hermite index m, grid point z and dealiased mode k:
+
+    out[s,m,l,z,k] = - sum_j  w_j psi_l(x_j) * C_k[ chi_{s,z,j}, gt_{s,m,z,j} ]
+    gt_{s,m,z,j}(q) = sum_{l'} psi_l'(x_j) G[s,m,l',z,q]            psi_l(x) = (-1)^l L_l(x)
+    chi_{s,z,j}(p)  = J0( sqrt(2 x_j b_s(p,z)) ) Phi[z,p]            (Eq. 4.5)
+    b_s             = kperp2 * tau_s m_s / (Z_s^2 bmag^2)            (rho_s = m_s v_ts/(Z_s B))
+    kperp2          = ky^2 gds2 + 2 kx ky gds21/shat + kx^2 gds22/shat^2
+    C_k[chi,g]      = Fourier coefficient of  d_y chi d_x g - d_x chi d_y g
+                    = sum_{p+q=k} (p_x q_y - p_y q_x) chi_p g_q      (dealiased, exact)
+
+(x_j, w_j): J-point Gauss-Laguerre rule, J = floor((3 Nl - 1)/2)  (reading R2 in DESIGN.md).
+
+Two independent evaluations of C_k are provided:
+  * ``bracket_convolution``   -- the definition: direct sum over mode pairs;
+  * ``bracket_pseudospectral`` -- P:647 literally: zero-pad, inverse DFT, pointwise product,
+    forward DFT, 2/3-rule mask, with explicit naive-DFT matrices exp(+-2 pi i (ab mod N)/N).
+The 2/3 rule makes the two agree to rounding (3*kmax < N), which tests/ checks.
+
+Readings of silent / garbled passages: R1 psi^{l'} = psi_l(x_j);
+R3 the second factor of D1 line 1 carries G_{l',m} (not m+1); R5 Fourier-series amplitude
+convention (inverse = plain sum, forward carries 1/(Nx Ny)); R6 out = -N.
+
+Pins (tests/test_oracle_pins.py): Gauss-Laguerre J=2 closed form and moment exactness;
+Tinv*T = I; Eq. 4.7 closed form of the Laguerre-projected J0; sum_l J_l^2 -> I0(b)e^-b;
+single-mode bracket closed form; convolution == pseudo-spectral; free-energy invariant;
+b=0 reduction; Hermitian ky=0 output; the paper's printed dealiased counts.
+Nothing here is "parity unpinned".
+"""
+from __future__ import annotations
+
+import ctypes
+import math
+import os
+
+import numpy as np
+from scipy import special as _sp          # library primitives: J0, I0e (each pinned in tests)
+
+
+# ============================================================================ index sets
+def dealiased_counts(Nx, Ny):
+    """2/3 rule: keep |p| <= (Nx-1)//3 and 0 <= q <= (Ny-1)//3.
+    Printed values P:806: 192->127, 64->22, 64->43, 192->64."""
+    return 1 + 2 * ((Nx - 1) // 3), 1 + (Ny - 1) // 3
+
+
+def kx_index(Nx):
+    """Compact storage order of the kept kx integers: 0,1,..,K,-K,..,-1 (reading R8)."""
+    K = (Nx - 1) // 3
+    return np.array(list(range(0, K + 1)) + list(range(-K, 0)), dtype=np.int64)
+
+
+def ky_index(Ny):
+    return np.arange(1 + (Ny - 1) // 3, dtype=np.int64)
+
+
+def pad_row(Nx):
+    """Row of the zero-padded length-Nx transform that compact row i lands on: p mod Nx."""
+    return np.mod(kx_index(Nx), Nx)
+
+
+def dealias_mask(Nx, Ny):
+    """mask[r][q] over the padded half-spectrum Nx x (Ny/2+1): 1 where the mode is kept."""
+    Nyc = Ny // 2 + 1
+    K = (Nx - 1) // 3
+    Q = (Ny - 1) // 3
+    mask = np.zeros((Nx, Nyc), dtype=np.uint8)
+    for r in range(Nx):
+        p = r if r <= Nx // 2 else r - Nx
+        for q in range(Nyc):
+            if abs(p) <= K and q <= Q:
+                mask[r, q] = 1
+    return mask
+
+
+# ============================================================================ Laguerre
+def num_mu_nodes(Nl):
+    """Smallest J with 2J-1 >= 3(Nl-1): triple products of degree-<Nl polynomials exact."""
+    return (3 * Nl - 1) // 2
+
+
+def gauss_laguerre(J):
+    """Nodes/weights for weight e^-x on [0,inf) by Golub-Welsch: eigen-decomposition of the
+    Jacobi matrix of the Laguerre recurrence (diag 2i+1, off-diag i+1); w = (first
+    eigenvector component)^2 since mu_0 = int e^-x = 1."""
+    i = np.arange(J, dtype=np.float64)
+    A = np.diag(2.0 * i + 1.0) + np.diag(i[1:], 1) + np.diag(i[1:], -1)
+    x, V = np.linalg.eigh(A)
+    w = V[0, :] ** 2
+    return x, w
+
+
+def laguerre_L(l, x):
+    """L_l(x) by the three-term recurrence (k+1)L_{k+1} = (2k+1-x)L_k - k L_{k-1} (Eq. 4.3)."""
+    x = np.asarray(x, dtype=np.float64)
+    Lm, L = np.zeros_like(x), np.ones_like(x)
+    for k in range(l):
+        Lm, L = L, ((2 * k + 1 - x) * L - k * Lm) / (k + 1)
+    return L
+
+
+def psi(l, x):
+    """psi_l = (-1)^l L_l."""
+    return (-1.0) ** l * laguerre_L(l, x)
+
+
+def laguerre_matrices(Nl, J=None):
+    """T[j][l] = psi_l(x_j) (l -> mu nodes) and Tinv[l][j] = w_j psi_l(x_j) (mu nodes -> l).
+    The e^{-muB} weight is carried by the quadrature weights (reading R1)."""
+    J = J or num_mu_nodes(Nl)
+    x, w = gauss_laguerre(J)
+    T = np.stack([psi(l, x) for l in range(Nl)], axis=1)          # [J][Nl]
+    Tinv = (T * w[:, None]).T.copy()                               # [Nl][J]
+    return x, w, T, Tinv
+
+
+def jflr(l, b):
+    """Closed form of the Laguerre-projected gyroaverage, Eq. 4.7:
+    J_l(b) = (1/l!) (-b/2)^l e^{-b/2};  zero for l < 0."""
+    if l < 0:
+        return np.zeros_like(np.asarray(b, dtype=np.float64))
+    b = np.asarray(b, dtype=np.float64)
+    return (-0.5 * b) ** l / math.factorial(l) * np.exp(-0.5 * b)
+
+
+# ============================================================================ geometry / species
+def kperp2(kx, ky, gds2, gds21, gds22, shat):
+    """[z][kx][ky]: ky^2 gds2 + 2 kx ky gds21/shat + kx^2 gds22/shat^2 (P:182 with E6-E8)."""
+    kx = np.asarray(kx, np.float64)[None, :, None]
+    ky = np.asarray(ky, np.float64)[None, None, :]
+    g2 = np.asarray(gds2, np.float64)[:, None, None]
+    g21 = np.asarray(gds21, np.float64)[:, None, None]
+    g22 = np.asarray(gds22, np.float64)[:, None, None]
+    return ky * ky * g2 + 2.0 * kx * ky * g21 / shat + kx * kx * g22 / (shat * shat)
+
+
+def b_species(kp2, bmag, Z, mass, temp):
+    """b_s = kperp2 rho_s^2, rho_s^2 = tau_s m_s / (Z_s^2 bmag^2)  (P:85 with v_ts = sqrt(tau/m))."""
+    return kp2 * (temp * mass / (Z * Z)) / (np.asarray(bmag, np.float64)[:, None, None] ** 2)
+
+
+def gyro_table(b, x_nodes):
+    """M[z][j][kx][ky] = J0( sqrt(2 x_j b) )   (P:85 alpha_s = sqrt(2 muB b_s))."""
+    return np.stack([_sp.j0(np.sqrt(2.0 * xj * b)) for xj in x_nodes], axis=1)
+
+
+# ============================================================================ brackets
+def extend_reality(F):
+    """Compact [nakx][naky] (kx order 0..K,-K..-1; ky 0..Q) -> centred full array
+    E[a+K][b+Q], a in -K..K, b in -Q..Q, using f(-p) = conj f(p)."""
+    nakx, naky = F.shape
+    K, Q = (nakx - 1) // 2, naky - 1
+    E = np.zeros((2 * K + 1, 2 * Q + 1), dtype=np.complex128)
+    for i in range(nakx):
+        a = i if i <= K else i - nakx
+        for b in range(naky):
+            E[a + K, b + Q] = F[i, b]
+            if b > 0:
+                E[-a + K, -b + Q] = np.conj(F[i, b])
+    return E
+
+
+def bracket_convolution(chi, g, dkx, dky):
+    """C_k[chi,g] = sum_{p+q=k} (p_x q_y - p_y q_x) chi_p g_q over the reality-extended
+    dealiased sets, for k in the compact set.  Pure-python double loop over (k, p): the
+    definition itself.  O(nk * nk) -- small grids only (see conv_c for a C transcription)."""
+    nakx, naky = g.shape
+    K, Q = (nakx - 1) // 2, naky - 1
+    X, Gx = extend_reality(np.asarray(chi, np.complex128)), extend_reality(np.asarray(g, np.complex128))
+    out = np.zeros((nakx, naky), dtype=np.complex128)
+    for i in range(nakx):
+        ka = i if i <= K else i - nakx
+        for kb in range(naky):
+            acc = 0.0 + 0.0j
+            for pa in range(-K, K + 1):
+                qa = ka - pa
+                if abs(qa) > K:
+                    continue
+                for pb in range(-Q, Q + 1):
+                    qb = kb - pb
+                    if abs(qb) > Q:
+                        continue
+                    px, py, qx, qy = dkx * pa, dky * pb, dkx * qa, dky * qb
+                    acc += (px * qy - py * qx) * X[pa + K, pb + Q] * Gx[qa + K, qb + Q]
+            out[i, kb] = acc
+    return out
+
+
+def bracket_convolution_np(chi, g, dkx, dky):
+    """Same sum as bracket_convolution with the inner (q) loops vectorised: for each p the
+    shifted window of g is accumulated.  Identical arithmetic up to summation order."""
+    nakx, naky = g.shape
+    K, Q = (nakx - 1) // 2, naky - 1
+    X, Gx = extend_reality(np.asarray(chi, np.complex128)), extend_reality(np.asarray(g, np.complex128))
+    a = np.arange(-K, K + 1, dtype=np.float64)[:, None] * dkx       # q_x on the full grid
+    b = np.arange(-Q, Q + 1, dtype=np.float64)[None, :] * dky       # q_y
+    # full output over k in [-2K,2K] x [-2Q,2Q], then cut to the compact set
+    full = np.zeros((4 * K + 1, 4 * Q + 1), dtype=np.complex128)
+    for pa in range(-K, K + 1):
+        for pb in range(-Q, Q + 1):
+            xp = X[pa + K, pb + Q]
+            if xp == 0:
+                continue
+            px, py = dkx * pa, dky * pb
+            full[pa + K:pa + 3 * K + 1, pb + Q:pb + 3 * Q + 1] += xp * (px * b - py * a) * Gx
+    out = np.zeros((nakx, naky), dtype=np.complex128)
+    for i in range(nakx):
+        ka = i if i <= K else i - nakx
+        out[i, :] = full[ka + 2 * K, 2 * Q:2 * Q + naky]
+    return out
+
+
+_CONV_LIB = None
+
+
+def _conv_lib():
+    """The C transcription of bracket_convolution (oracle/conv_bracket.c), if built."""
+    global _CONV_LIB
+    if _CONV_LIB is None:
+        path = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libgxconv.so")
+        if not os.path.exists(path):
+            raise FileNotFoundError(path + " (run __graft_entry__.build())")
+        lib = ctypes.CDLL(path)
+        lib.gxo_bracket_convolution.restype = None
+        lib.gxo_bracket_convolution.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_double,
+                                                ctypes.c_double, ctypes.c_void_p, ctypes.c_void_p,
+                                                ctypes.c_void_p]
+        _CONV_LIB = lib
+    return _CONV_LIB
+
+
+def bracket_convolution_c(chi, g, dkx, dky):
+    """bracket_convolution evaluated by the plain-C loop nest in conv_bracket.c."""
+    nakx, naky = g.shape
+    X = np.ascontiguousarray(chi, dtype=np.complex128)
+    Gc = np.ascontiguousarray(g, dtype=np.complex128)
+    out = np.zeros((nakx, naky), dtype=np.complex128)
+    _conv_lib().gxo_bracket_convolution(nakx, naky, float(dkx), float(dky),
+                                        X.ctypes.data, Gc.ctypes.data, out.ctypes.data)
+    return out
+
+
+def dft_matrix(N, idx, sign):
+    """E[a][n] = exp(sign * 2 pi i (idx[a]*n mod N) / N): explicit naive-DFT table."""
+    a = np.asarray(idx, dtype=np.int64)[:, None]
+    n = np.arange(N, dtype=np.int64)[None, :]
+    return np.exp(sign * 2j * math.pi * np.mod(a * n, N).astype(np.float64) / N)
+
+
+class PseudoSpectral:
+    """P:647 written out: derivatives in k space, zero-padded inverse transform to the
+    Nx x Ny grid, pointwise bracket, forward transform, 2/3-rule truncation.  The transforms
+    are separable naive DFTs applied as matrix products (a library matmul is a step)."""
+
+    def __init__(self, Nx, Ny, dkx, dky):
+        self.Nx, self.Ny = Nx, Ny
+        self.kxi, self.kyi = kx_index(Nx), ky_index(Ny)
+        self.kx, self.ky = dkx * self.kxi, dky * self.kyi
+        Q = len(self.kyi) - 1
+        self.Q = Q
+        # inverse: f(x_i,y_j) = sum_{a,b} F[a,b] e^{+2 pi i (a i/Nx + b j/Ny)}, b over -Q..Q
+        self.Ex = dft_matrix(Nx, self.kxi, +1).T                    # [Nx][nakx]
+        self.Ey_pos = dft_matrix(Ny, self.kyi, +1)                  # [naky][Ny]
+        # forward: F[a,b] = 1/(Nx Ny) sum f e^{-...}
+        self.Fx = dft_matrix(Nx, self.kxi, -1)                      # [nakx][Nx]
+        self.Fy = dft_matrix(Ny, self.kyi, -1).T                    # [Ny][naky]
+
+    def to_real(self, F):
+        """Real field from a compact half-spectrum (ky>=0) via the reality condition:
+        f = Re( X0 + 2 sum_{b>0} X_b ), X_b(x,y) = [Ex F][:,b] e^{2 pi i b y/Ny}."""
+        H = self.Ex @ F                                             # [Nx][naky]
+        wgt = np.full(H.shape[1], 2.0)
+        wgt[0] = 1.0
+        return np.real((H * wgt[None, :]) @ self.Ey_pos)            # [Nx][Ny]
+
+    def to_spectral(self, f):
+        return (self.Fx @ f.astype(np.complex128) @ self.Fy) / (self.Nx * self.Ny)
+
+    def bracket(self, chi, g):
+        ikx = 1j * self.kx[:, None]
+        iky = 1j * self.ky[None, :]
+        dx_chi, dy_chi = self.to_real(ikx * chi), self.to_real(iky * chi)
+        dx_g, dy_g = self.to_real(ikx * g), self.to_real(iky * g)
+        return self.to_spectral(dy_chi * dx_g - dx_chi * dy_g)
+
+
+def bracket_pseudospectral(chi, g, Nx, Ny, dkx, dky):
+    return PseudoSpectral(Nx, Ny, dkx, dky).bracket(np.asarray(chi, np.complex128),
+                                                    np.asarray(g, np.complex128))
+
+
+# ============================================================================ the nonlinear term
+def nonlinear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, method="dft", planes=None,
+                  gyro="exact", J=None):
+    """out = -N  (same shape/layout as G: [s][m][l][z][kx][ky]), fp64.
+
+    G, Phi : complex arrays (any precision; up-cast to complex128 -- reading R15)
+    geo    : dict with bmag, gds2, gds21, gds22 (length Nz)
+    species: list of dicts/objects with Z, mass, temp
+    method : "dft" (pseudo-spectral, naive DFT), "conv" (pure python definition),
+             "conv_np" (vectorised definition), "conv_c" (C transcription)
+    planes : optional iterable of (s, m, z) to evaluate (others left zero)
+    gyro   : "exact" J0(sqrt(2 x_j b)) (default) or "series" sum_l psi_l(x_j) J_l(b)
+    """
+    G = np.asarray(G).astype(np.complex128)
+    Phi = np.asarray(Phi).astype(np.complex128)
+    Ns, Nm, Nl, Nz, nakx, naky = G.shape
+    x, w, T, Tinv = laguerre_matrices(Nl, J)
+    nJ = len(x)
+    kx, ky = dkx * kx_index(Nx), dky * ky_index(Ny)
+    kp2 = kperp2(kx, ky, geo["gds2"], geo["gds21"], geo["gds22"], shat)
+    ps = PseudoSpectral(Nx, Ny, dkx, dky) if method == "dft" else None
+    fn = {"dft": None, "conv": bracket_convolution, "conv_np": bracket_convolution_np,
+          "conv_c": bracket_convolution_c}[method]
+    out = np.zeros_like(G)
+    todo = planes if planes is not None else [(s, m, z) for s in range(Ns) for m in range(Nm)
+                                              for z in range(Nz)]
+    Mcache = {}
+    for (s, m, z) in todo:
+        sp = species[s]
+        Z, mass, temp = (sp["Z"], sp["mass"], sp["temp"]) if isinstance(sp, dict) else (sp.Z, sp.mass, sp.temp)
+        if (s, z) not in Mcache:
+            b = b_species(kp2[z:z + 1], np.asarray(geo["bmag"])[z:z + 1], Z, mass, temp)[0]
+            if gyro == "exact":
+                Mcache[(s, z)] = np.stack([_sp.j0(np.sqrt(2.0 * xj * b)) for xj in x])
+            else:
+                Mcache[(s, z)] = np.stack([sum(psi(l, xj) * jflr(l, b) for l in range(Nl)) for xj in x])
+        M = Mcache[(s, z)]
+        for j in range(nJ):
+            chi = M[j] * Phi[z]                                              # a1
+            gt = sum(T[j, l] * G[s, m, l, z] for l in range(Nl))             # a2
+            C = ps.bracket(chi, gt) if ps is not None else fn(chi, gt, dkx, dky)   # a3-a7
+            for l in range(Nl):                                              # a8
+                out[s, m, l, z] -= Tinv[l, j] * C
+    return out
+
+
+# ============================================================================ field solve
+def field_solve(G, Nx, Ny, dkx, dky, shat, geo, species, tau_fac=1.0, adiabatic=True):
+    """Quasineutrality for Phi[z][kx][ky], sums truncated at Nl.
+
+    adiabatic=True : Boltzmann electrons, Eq. 6.1 with one kinetic ion species:
+        nbar = sum_l J_l G_{l,0};  (1 + tau_fac - sum_l J_l^2) Phi = nbar + tau_fac <<Phi>> d_{ky,0}
+        (Eq. 6.1 in G via Eq. 4.8; tau_fac = T_i/T_e -- the paper prints T_e/T_i, =1 everywhere here),
+        <<.>> = jacobian-weighted z average; solving the ky=0 rows for <<Phi>>:
+        <<Phi>> = <<nbar/D>> / (1 - tau_fac <<1/D>>),  D = 1 + tau_fac - sum J_l^2.
+    adiabatic=False: Eq. 4.23 with dB_par = 0:
+        sum_s Z^2 n/tau (1 - sum_l J_l^2) Phi = sum_s Z n sum_l J_l G_{l,0}.
+    Phi(kx=0,ky=0) = 0.
+    """
+    G = np.asarray(G).astype(np.complex128)
+    Ns, Nm, Nl, Nz, nakx, naky = G.shape
+    kx, ky = dkx * kx_index(Nx), dky * ky_index(Ny)
+    kp2 = kperp2(kx, ky, geo["gds2"], geo["gds21"], geo["gds22"], shat)
+    get = lambda sp, k: sp[k] if isinstance(sp, dict) else getattr(sp, k)
+    num = np.zeros((Nz, nakx, naky), dtype=np.complex128)
+    den = np.zeros((Nz, nakx, naky), dtype=np.float64)
+    for s, sp in enumerate(species):
+        Z, mass, temp, dens = get(sp, "Z"), get(sp, "mass"), get(sp, "temp"), get(sp, "dens")
+        b = b_species(kp2, geo["bmag"], Z, mass, temp)
+        Jl = [jflr(l, b) for l in range(Nl)]
+        nbar = sum(Jl[l] * G[s, 0, l] for l in range(Nl))
+        g0 = sum(Jl[l] ** 2 for l in range(Nl))
+        num += Z * dens * nbar
+        den += Z * Z * dens / temp * (1.0 - g0)
+    if adiabatic:
+        sp = species[0]
+        qn = get(sp, "Z") * get(sp, "dens")          # ion charge density factor
+        pref = get(sp, "Z") ** 2 * get(sp, "dens") / get(sp, "temp")
+        # (pref*(1-g0) + qn*tau_fac... ) general form; with Z=n=tau=1 this is Eq. 6.1
+        D = den + pref * tau_fac
+        Phi = num / D
+        jac = np.asarray(geo["jacobian"], np.float64)
+        wz = jac / jac.sum()
+        avg = lambda f: np.tensordot(wz, f, axes=(0, 0))           # [kx]
+        fden = 1.0 - pref * tau_fac * avg(1.0 / D[:, :, 0])
+        fden[0] = 1.0                                  # kx=ky=0: b=0, D=tau_fac; Phi(0,0) := 0 below
+        fs = avg(num[:, :, 0] / D[:, :, 0]) / fden
+        Phi[:, :, 0] = (num[:, :, 0] + pref * tau_fac * fs[None, :]) / D[:, :, 0]
+    else:
+        with np.errstate(divide="ignore", invalid="ignore"):
+            Phi = np.where(den != 0.0, num / np.where(den != 0.0, den, 1.0), 0.0)
+    Phi[:, 0, 0] = 0.0
+    return Phi
+
+
+# ============================================================================ invariants
+def free_energy_moment(G, out):
+    """sum_l [ sum_{ky=0} + 2 Re sum_{ky>0} ] conj(G_l(k)) out_l(k) per (s,m,z): the
+    contribution of the E×B term to d/dt of sum |g|^2; vanishes identically."""
+    w = np.full(G.shape[-1], 2.0)
+    w[0] = 1.0
+    return np.real(np.einsum("smlzxy,smlzxy,y->smz", np.conj(G), out, w))
+
+
+def relative_max_error(a, ref):
+    """max|a-ref| / max|ref| over the whole array (BASELINE.json north_star metric)."""
+    den = float(np.max(np.abs(ref)))
+    return float(np.max(np.abs(np.asarray(a) - ref))) / (den if den > 0 else 1.0)
