@@ -1,0 +1,133 @@
+/* gx.h -- C-ABI of the B200-native nonlinear E×B term of the Fourier-Laguerre-Hermite
+ * gyrokinetic system of GX (arxiv 2209.06731).  "P:nnn" = line nnn of PAPER.md.
+ *
+ * The library evaluates, for every species s, Hermite index m, field-line point z and
+ * dealiased perpendicular mode k = (kx, ky),
+ *
+ *   out[s,m,l,z,k] = - N^s_{l,m}(k,z)                                   (Eq. 4.9: N sits on the LHS)
+ *   N^s_{l,m} = L_l F_k ( F^-1[i ky J0s Phi] F^-1[i kx sum_l' psi_l' G_{l',m}]
+ *                       - F^-1[i kx J0s Phi] F^-1[i ky sum_l' psi_l' G_{l',m}] )
+ *                                                                       (App. D Eq. D1 line 1; Eq. 4.19)
+ * pseudo-spectrally: Laguerre l -> mu-nodes, spectral derivatives, zero-padded inverse 2D FFT,
+ * pointwise bracket, forward FFT, 2/3-rule dealiasing, Laguerre mu-nodes -> l.
+ * All device arithmetic is fp32; tables are computed in fp64 on the host and rounded once.
+ *
+ * LAYOUT (slowest -> fastest), interleaved complex64 (re,im):
+ *   g, out : [s][m][l][z][kx][ky]   compact dealiased: nakx = 1+2*((Nx-1)/3), naky = 1+(Ny-1)/3
+ *            kx integers in FFT order 0,1,..,K,-K,..,-1 (K=(nakx-1)/2); ky integers 0..naky-1
+ *            (ky<0 implied by the reality condition)
+ *   phi    : [z][kx][ky]
+ * PRECONDITION: the ky=0 column is Hermitian, f(-kx,0) = conj f(kx,0), f(0,0) real; otherwise the
+ *   result is unspecified.
+ * OWNERSHIP: g, phi, out are caller-owned DEVICE pointers (16-byte aligned; out must not alias g);
+ *   the library keeps no reference after the call returns.  The handle owns all tables and the
+ *   workspace.  Geometry / species arrays are HOST pointers, copied during the call.
+ * ASYNC: compute calls enqueue on the given cudaStream_t (passed as void*) and do not synchronise.
+ * ERRORS: every call returns 0 (GX_OK) or a negative code; no exception crosses the ABI;
+ *   gx_last_error() returns a message for the last failure on that handle.
+ * There is NO CPU fallback: without a CUDA device gx_grid_create fails with GX_ERR_CUDA.
+ */
+#ifndef GX_H_
+#define GX_H_
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct gx_grid gx_grid;
+
+enum {
+    GX_OK = 0,
+    GX_ERR_ARG = -1,         /* bad size / null pointer / index out of range                    */
+    GX_ERR_STATE = -2,       /* box, species or geometry not set before a compute call           */
+    GX_ERR_UNSUPPORTED = -3, /* (Nx,Ny) has no kernel instantiation, or the plane does not fit   */
+    GX_ERR_CUDA = -4,        /* CUDA runtime error (message via gx_last_error)                   */
+    GX_ERR_ALLOC = -5
+};
+
+/* what-codes for gx_query */
+enum {
+    GX_Q_NAKX = 0, GX_Q_NAKY = 1, GX_Q_NJ = 2,        /* dealiased counts, number of mu-nodes J   */
+    GX_Q_G_ELEMS = 3, GX_Q_PHI_ELEMS = 4,             /* complex elements of g/out and of phi      */
+    GX_Q_WORKSPACE_BYTES = 5,                         /* device bytes owned by the handle          */
+    GX_Q_LAUNCHES_PER_NL = 6,                         /* kernels launched by one gx_nonlinear_rhs  */
+    GX_Q_LAUNCHES_PER_RHS = 7,
+    GX_Q_NL_FLOPS = 8, GX_Q_NL_BYTES = 9              /* algorithmic flops / HBM bytes per call */
+};
+
+/* Create a handle for real-space grid Nx x Ny, Nz field-line points, Nl Laguerre and Nm Hermite
+ * moments, Ns species.  Nx, Ny must be even, >= 4, and factor as R1*R2 with R1,R2 in
+ * {2,3,4,6,8,12,16} (all sizes of BASELINE.json configs do); Nl <= 16.  The number of mu-nodes
+ * is J = (3*Nl-1)/2 (smallest Gauss-Laguerre rule exact for triple products; R2).
+ * Builds index maps, Gauss-Laguerre nodes/weights, T[j][l] = psi_l(x_j), Tinv[l][j] = w_j psi_l(x_j),
+ * psi_l = (-1)^l L_l, and FFT twiddles.  Uses the current CUDA device. */
+int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out);
+int gx_grid_destroy(gx_grid* g);
+
+/* Perpendicular box: ky = dky*q, kx = dkx*p (units 1/rho_ref, Table 4); shat enters
+ * kperp2 through gds21/shat, gds22/shat^2 (P:681-686 Eq. E6-E7). */
+int gx_box_set(gx_grid* g, double dky, double dkx, double shat);
+
+/* Species s: charge Z_s, mass m_s, temperature tau_s, density n_s, gradients
+ * tprim = 1/L_Ts, fprim = 1/L_ns, like-species collision frequency nu_ss. */
+int gx_species_set(gx_grid* g, int s, double Z, double mass, double temp, double dens,
+                   double tprim, double fprim, double nu_ss);
+
+/* Adiabatic (Boltzmann) electron response for the field solve, Eq. 6.1:
+ * enabled != 0 selects it (requires Ns == 1); tau_fac = T_i/T_e. Default: enabled iff Ns == 1, tau_fac 1. */
+int gx_adiabatic_set(gx_grid* g, int enabled, double tau_fac);
+
+/* Dissipation parameters of gx_rhs: hyper-viscosity D (k_perp^2/k_perp,max^2)^n (Eq. 4.26) and
+ * hyper-collisions nu_hyp m^p, p = Nm/2, strength f_hyp (Eq. 4.27-4.28). Defaults 0.05, 4, 1. */
+int gx_dissipation_set(gx_grid* g, double D_hyper, int n_hyper, double f_hyp);
+
+/* Per-z geometry coefficients (HOST arrays of length Nz, P:677-694 Eq. E4-E11) and the constant
+ * gradpar = b.grad z.  bmag, gds2, gds21, gds22 define k_perp^2 and b_s and hence the
+ * gyroaverage table M[s][z][j][kx][ky] = J0(sqrt(2 x_j b_s)) built here in fp64; the drift,
+ * bgrad (= grad_par ln B) and jacobian arrays are used by gx_rhs / gx_field_solve only and may be
+ * NULL if those are never called.  Requires gx_box_set and every gx_species_set first. */
+int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const double* gds21,
+                    const double* gds22, const double* gbdrift, const double* gbdrift0,
+                    const double* cvdrift, const double* cvdrift0, const double* bgrad,
+                    const double* jacobian, double gradpar);
+
+/* out = -N[g, phi]  (the hot path).  Device pointers; enqueued on `cuda_stream`. */
+int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev,
+                     void* cuda_stream);
+
+/* Same call with HOST buffers (pinned for full speed): copies g and phi to internal device buffers,
+ * runs gx_nonlinear_rhs, copies out back, and synchronises the stream before returning. */
+int gx_nonlinear_rhs_host(gx_grid* g, const void* g_host, const void* phi_host, void* out_host,
+                          void* cuda_stream);
+
+/* Quasineutrality field solve phi = phi[g] on the device: Eq. 6.1 for adiabatic electrons
+ * (with the jacobian-weighted flux-surface average at ky=0), else Eq. 4.23 with dB_par = 0;
+ * sums over l truncated at Nl; phi(kx=0,ky=0) = 0. */
+int gx_field_solve(gx_grid* g, const void* g_dev, void* phi_dev, void* cuda_stream);
+
+/* out = dG/dt = -N + linear terms of Eq. 4.9: streaming, mirror, curvature and grad-B
+ * drifts, drive (Eq. 4.12), Dougherty collisions (Eq. 4.13-4.18), hyper-viscosity, hyper-collisions;
+ * phi is computed internally with gx_field_solve.  Electrostatic (beta_ref = 0). */
+int gx_rhs(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream);
+
+/* Linear part only (gx_rhs without -N), given phi; used to test the linear terms on their own. */
+int gx_linear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream);
+
+int gx_query(gx_grid* g, int what, long long* value);
+
+/* Parity exports (HOST outputs; any pointer may be NULL): compact kx integers [nakx], ky integers
+ * [naky], padded row of each compact kx row [nakx] (= p mod Nx), 2/3-rule mask over the padded
+ * half-spectrum [Nx*(Ny/2+1)], Gauss-Laguerre nodes and weights [nj]. */
+int gx_export_maps(gx_grid* g, int* kx_index, int* ky_index, int* pad_row, unsigned char* mask,
+                   double* lag_nodes, double* lag_weights);
+
+/* Table exports for parity tests (HOST outputs, fp32 as used on the device):
+ * T [nj*Nl], Tinv [Nl*nj], M [Ns*Nz*nj*nakx*naky] (needs geometry set; may be NULL). */
+int gx_export_tables(gx_grid* g, float* T, float* Tinv, float* M);
+
+const char* gx_last_error(gx_grid* g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GX_H_ */

@@ -1,0 +1,135 @@
+// dft_regs.cuh -- small complex DFTs held entirely in registers (sm_100a, fp32).
+//
+// Building block of the shared-memory FFT passes in nl_kernels.cuh.  dft<N,S>(v) overwrites the
+// N complex values v[0..N-1] (natural order) with their DFT, X[k] = sum_n v[n] e^{S 2 pi i n k / N},
+// S = +1 (inverse, unnormalised) or -1 (forward).  N in {2,3,4,6,8,12,16}; composite sizes are one
+// Cooley-Tukey split A x B done with compile-time indices, so after full unrolling everything is
+// register renaming plus FADD/FMUL/FFMA with immediate twiddles (no local memory, no tables).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace gx {
+
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+    return make_float2(fmaf(-a.y, b.y, a.x * b.x), fmaf(a.y, b.x, a.x * b.y));
+}
+__device__ __forceinline__ float2 cmul_conj(float2 a, float2 b) {   // a * conj(b)
+    return make_float2(fmaf(a.y, b.y, a.x * b.x), fmaf(a.y, b.x, -a.x * b.y));
+}
+// multiply by S*i
+template <int S> __device__ __forceinline__ float2 mul_i(float2 a) {
+    return S > 0 ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
+}
+
+// cos(2 pi t / 48), t = 0..47, fp64 values rounded to fp32 at compile time.
+__host__ __device__ constexpr double cos48(int t) {
+    constexpr double C[13] = {1.0,
+                              0.99144486137381041114, 0.96592582628906828675, 0.92387953251128675613,
+                              0.86602540378443864676, 0.79335334029123516458, 0.70710678118654752440,
+                              0.60876142900872063942, 0.5,
+                              0.38268343236508977173, 0.25881904510252076235, 0.13052619222005159155,
+                              0.0};
+    t = ((t % 48) + 48) % 48;
+    if (t > 24) t = 48 - t;          // cos(-a) = cos(a)
+    return t <= 12 ? C[t] : -C[24 - t];
+}
+__host__ __device__ constexpr double sin48(int t) { return cos48(t - 12); }
+
+// v *= e^{S 2 pi i t / N} with t, N compile-time after unrolling; trivial cases cost no multiply.
+template <int N, int S> __device__ __forceinline__ float2 twiddle(float2 v, int t) {
+    static_assert(48 % N == 0, "N must divide 48");
+    const int a = ((t * (48 / N)) % 48 + 48) % 48;
+    if (a == 0) return v;
+    if (a == 12) return mul_i<S>(v);
+    if (a == 24) return make_float2(-v.x, -v.y);
+    if (a == 36) return mul_i<-S>(v);
+    if (a % 12 == 6) {               // (+-1 +- i)/sqrt(2): two adds, two multiplies
+        const float h = 0.70710678118654752440f;
+        const float cr = (a == 6 || a == 42) ? h : -h;
+        const float ci = ((a == 6 || a == 18) ? h : -h) * (S > 0 ? 1.f : -1.f);
+        // (x+iy)(cr+ici): |cr| = |ci| = h
+        const float p = v.x * h, q = v.y * h;
+        const float sr = cr > 0 ? 1.f : -1.f, si = ci > 0 ? 1.f : -1.f;
+        return make_float2(sr * p - si * q, si * p + sr * q);
+    }
+    const float c = (float)cos48(a);
+    const float s = (float)sin48(a) * (S > 0 ? 1.f : -1.f);
+    return make_float2(fmaf(-v.y, s, v.x * c), fmaf(v.x, s, v.y * c));
+}
+
+template <int N, int S> struct Dft;
+
+template <int S> struct Dft<2, S> {
+    __device__ __forceinline__ static void run(float2 (&v)[2]) {
+        const float2 a = v[0], b = v[1];
+        v[0] = cadd(a, b);
+        v[1] = csub(a, b);
+    }
+};
+
+template <int S> struct Dft<3, S> {
+    __device__ __forceinline__ static void run(float2 (&v)[3]) {
+        const float2 t = cadd(v[1], v[2]);
+        const float2 d = csub(v[1], v[2]);
+        const float2 m = make_float2(fmaf(-0.5f, t.x, v[0].x), fmaf(-0.5f, t.y, v[0].y));
+        const float h = 0.86602540378443864676f;
+        const float2 r = mul_i<S>(make_float2(h * d.x, h * d.y));
+        v[0] = cadd(v[0], t);
+        v[1] = cadd(m, r);
+        v[2] = csub(m, r);
+    }
+};
+
+template <int S> struct Dft<4, S> {
+    __device__ __forceinline__ static void run(float2 (&v)[4]) {
+        const float2 a = cadd(v[0], v[2]), b = csub(v[0], v[2]);
+        const float2 c = cadd(v[1], v[3]), d = mul_i<S>(csub(v[1], v[3]));
+        v[0] = cadd(a, c);
+        v[1] = cadd(b, d);
+        v[2] = csub(a, c);
+        v[3] = csub(b, d);
+    }
+};
+
+// One Cooley-Tukey split N = A*B:  n = n1*B + n2,  k = k1 + A*k2.
+template <int N, int A, int B, int S> __device__ __forceinline__ void dft_split(float2 (&v)[N]) {
+    static_assert(A * B == N, "bad split");
+    float2 y[N];
+#pragma unroll
+    for (int n2 = 0; n2 < B; ++n2) {
+        float2 t[A];
+#pragma unroll
+        for (int n1 = 0; n1 < A; ++n1) t[n1] = v[n1 * B + n2];
+        Dft<A, S>::run(t);
+#pragma unroll
+        for (int k1 = 0; k1 < A; ++k1) y[k1 * B + n2] = twiddle<N, S>(t[k1], n2 * k1);
+    }
+#pragma unroll
+    for (int k1 = 0; k1 < A; ++k1) {
+        float2 u[B];
+#pragma unroll
+        for (int n2 = 0; n2 < B; ++n2) u[n2] = y[k1 * B + n2];
+        Dft<B, S>::run(u);
+#pragma unroll
+        for (int k2 = 0; k2 < B; ++k2) v[k1 + A * k2] = u[k2];
+    }
+}
+
+template <int S> struct Dft<6, S> {
+    __device__ __forceinline__ static void run(float2 (&v)[6]) { dft_split<6, 2, 3, S>(v); }
+};
+template <int S> struct Dft<8, S> {
+    __device__ __forceinline__ static void run(float2 (&v)[8]) { dft_split<8, 2, 4, S>(v); }
+};
+template <int S> struct Dft<12, S> {
+    __device__ __forceinline__ static void run(float2 (&v)[12]) { dft_split<12, 3, 4, S>(v); }
+};
+template <int S> struct Dft<16, S> {
+    __device__ __forceinline__ static void run(float2 (&v)[16]) { dft_split<16, 4, 4, S>(v); }
+};
+
+template <int N, int S> __device__ __forceinline__ void dft(float2 (&v)[N]) { Dft<N, S>::run(v); }
+
+}  // namespace gx

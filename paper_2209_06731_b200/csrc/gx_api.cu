@@ -1,0 +1,532 @@
+// gx_api.cu -- host side of the C-ABI declared in include/gx.h: handle, tables (fp64 -> fp32 once),
+// kernel dispatch.  No CPU compute path exists: every step of the hot path runs in nl_kernels.cuh.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/gx.h"
+#include "linear_kernels.cuh"
+#include "nl_kernels.cuh"
+
+namespace {
+
+using gx::NlParams;
+
+struct Species {
+    double Z = 1, mass = 1, temp = 1, dens = 1, tprim = 0, fprim = 0, nu = 0;
+    bool set = false;
+};
+
+// per-(Nx,Ny) kernel launchers
+struct KernelSet {
+    int Nx, Ny;
+    int smem_bytes;
+    cudaError_t (*launch_chi)(const NlParams&, int units, cudaStream_t);
+    cudaError_t (*launch_bracket)(const NlParams&, int units, cudaStream_t);
+};
+
+template <class C> cudaError_t launch_chi_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    gx::chi_planes_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
+    return cudaGetLastError();
+}
+template <class C> cudaError_t launch_bracket_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::bracket_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    gx::bracket_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
+    return cudaGetLastError();
+}
+template <class C> constexpr KernelSet make_set() {
+    return KernelSet{C::NX, C::NY, C::SMEM_BYTES, &launch_chi_t<C>, &launch_bracket_t<C>};
+}
+
+//                         NX   NY  RX1 RX2 RY1 RY2  RB   NT MINB STAGE
+using Cfg16x16   = gx::PlaneCfg<16, 16, 4, 4, 4, 4, 16, 64, 1, true>;
+using Cfg64x64   = gx::PlaneCfg<64, 64, 8, 8, 8, 8, 64, 256, 2, true>;
+using Cfg128x64  = gx::PlaneCfg<128, 64, 16, 8, 8, 8, 64, 256, 2, true>;
+using Cfg192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, 64, 256, 2, true>;
+using Cfg256x64  = gx::PlaneCfg<256, 64, 16, 16, 8, 8, 64, 256, 1, true>;
+using Cfg256x96  = gx::PlaneCfg<256, 96, 16, 16, 8, 12, 64, 256, 1, true>;
+using Cfg192x192 = gx::PlaneCfg<192, 192, 16, 12, 12, 16, 16, 256, 1, false>;
+using Cfg64x192  = gx::PlaneCfg<64, 192, 8, 8, 12, 16, 32, 256, 1, true>;
+
+const KernelSet kKernelSets[] = {
+    make_set<Cfg16x16>(),  make_set<Cfg64x64>(),  make_set<Cfg128x64>(),  make_set<Cfg192x64>(),
+    make_set<Cfg256x64>(), make_set<Cfg256x96>(), make_set<Cfg192x192>(), make_set<Cfg64x192>(),
+};
+
+const KernelSet* find_set(int Nx, int Ny) {
+    for (const auto& k : kKernelSets)
+        if (k.Nx == Nx && k.Ny == Ny) return &k;
+    return nullptr;
+}
+
+// ---------------------------------------------------------------------------- Gauss-Laguerre
+// L_n(x) by the three-term recurrence (Eq. 4.3).
+double laguerre(int n, double x) {
+    double lm = 0.0, l = 1.0;
+    for (int k = 0; k < n; ++k) {
+        const double ln = ((2 * k + 1 - x) * l - k * lm) / (k + 1);
+        lm = l;
+        l = ln;
+    }
+    return l;
+}
+
+// Roots of L_n by interlacing: the roots of L_n separate those of L_{n+1}; each bracket is
+// refined by bisection and polished by Newton.  Weights w_i = x_i / ((n+1) L_{n+1}(x_i))^2.
+void gauss_laguerre(int n, std::vector<double>& x, std::vector<double>& w) {
+    std::vector<double> prev{1.0};                        // root of L_1
+    for (int deg = 2; deg <= n; ++deg) {
+        std::vector<double> cur(deg);
+        for (int i = 0; i < deg; ++i) {
+            double lo = (i == 0) ? 0.0 : prev[i - 1];
+            double hi = (i == deg - 1) ? 4.0 * deg + 3.0 : prev[i];
+            double flo = laguerre(deg, lo);
+            for (int it = 0; it < 200; ++it) {
+                const double mid = 0.5 * (lo + hi);
+                const double fm = laguerre(deg, mid);
+                if ((fm < 0) == (flo < 0)) { lo = mid; flo = fm; } else { hi = mid; }
+                if (hi - lo < 1e-15 * (1.0 + hi)) break;
+            }
+            double r = 0.5 * (lo + hi);
+            for (int it = 0; it < 4; ++it) {               // Newton: L_n' = n (L_n - L_{n-1}) / x
+                const double f = laguerre(deg, r), fp = deg * (f - laguerre(deg - 1, r)) / r;
+                const double rn = r - f / fp;
+                if (rn > lo && rn < hi) r = rn;
+            }
+            cur[i] = r;
+        }
+        prev.swap(cur);
+    }
+    x = prev;
+    x.resize(n);
+    w.resize(n);
+    for (int i = 0; i < n; ++i) {
+        const double l1 = laguerre(n + 1, x[i]);
+        w[i] = x[i] / ((n + 1.0) * (n + 1.0) * l1 * l1);
+    }
+}
+
+}  // namespace
+
+// ================================================================================================
+struct gx_grid {
+    int Nx, Ny, Nz, Nl, Nm, Ns, J, nakx, naky, K, Q;
+    long long nk;
+    double dkx = 0, dky = 0, shat = 1;
+    bool box_set = false, geo_set = false;
+    bool adiabatic = false;
+    double tau_fac = 1.0;
+    double D_hyper = 0.05, f_hyp = 1.0;
+    int n_hyper = 4;
+    std::vector<Species> sp;
+    std::vector<double> bmag, gds2, gds21, gds22, gbdrift, gbdrift0, cvdrift, cvdrift0, bgrad, jacobian;
+    bool have_lin_geo = false;
+    double gradpar = 1;
+    std::vector<double> xj, wj;
+    std::vector<float> hT, hTinv;
+    const KernelSet* ks = nullptr;
+    // device
+    float *dT = nullptr, *dTinv = nullptr, *dM = nullptr;
+    float2 *dtwx = nullptr, *dtwy = nullptr, *ddchi = nullptr, *dbhat = nullptr;
+    float2 *dgbuf = nullptr, *dphibuf = nullptr, *doutbuf = nullptr;   // for the *_host entry point
+    gx::LinTables lin;                                                  // linear-term tables
+    float2* dphi_rhs = nullptr;                                         // phi of gx_rhs
+    size_t bytes = 0;
+    std::string err;
+};
+
+namespace {
+
+int fail(gx_grid* g, int code, const std::string& msg) {
+    if (g) g->err = msg;
+    return code;
+}
+int cuda_fail(gx_grid* g, cudaError_t e, const char* where) {
+    return fail(g, GX_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+}
+#define GX_CUDA(g, call)                                            \
+    do {                                                            \
+        cudaError_t e_ = (call);                                    \
+        if (e_ != cudaSuccess) return cuda_fail(g, e_, #call);      \
+    } while (0)
+
+template <class T> int dev_alloc(gx_grid* g, T** p, size_t n) {
+    cudaError_t e = cudaMalloc((void**)p, n * sizeof(T));
+    if (e != cudaSuccess) return fail(g, GX_ERR_ALLOC, std::string("cudaMalloc: ") + cudaGetErrorString(e));
+    g->bytes += n * sizeof(T);
+    return GX_OK;
+}
+
+bool splits(int N) {   // N = R1*R2 with R in {2,3,4,6,8,12,16}
+    const int R[] = {2, 3, 4, 6, 8, 12, 16};
+    for (int a : R)
+        for (int b : R)
+            if (a * b == N) return true;
+    return false;
+}
+
+NlParams make_params(gx_grid* g, const void* gd, const void* phid, void* outd) {
+    NlParams p{};
+    p.g = (const float2*)gd;
+    p.phi = (const float2*)phid;
+    p.dchi = g->ddchi;
+    p.bhat = g->dbhat;
+    p.out = (float2*)outd;
+    p.M = g->dM;
+    p.T = g->dT;
+    p.Tinv = g->dTinv;
+    p.twx = g->dtwx;
+    p.twy = g->dtwy;
+    p.dkx = (float)g->dkx;
+    p.dky = (float)g->dky;
+    p.scale = (float)(1.0 / ((double)g->Nx * (double)g->Ny));
+    p.Nz = g->Nz; p.Nl = g->Nl; p.Nm = g->Nm; p.Ns = g->Ns; p.J = g->J;
+    return p;
+}
+
+long long nl_flops(const gx_grid* g) {
+    // nominal FFT convention, zero columns not transformed.
+    const double Nx = g->Nx, Ny = g->Ny, naky = g->naky, nk = (double)g->nk, J = g->J, Nl = g->Nl;
+    const double P = (double)g->Ns * g->Nm * g->Nz * J, SZJ = (double)g->Ns * g->Nz * J;
+    const double nT = 3 * P + 2 * SZJ;
+    const double fft = 5 * Nx * std::log2(Nx) * naky + 2.5 * Ny * std::log2(Ny) * Nx;
+    const double F = nT * fft + 3 * Nx * Ny * P + 2 * (4 * J * Nl) * nk * g->Ns * g->Nm * g->Nz +
+                     (4 * nk * P + 6 * nk * SZJ);
+    return (long long)F;
+}
+
+}  // namespace
+
+// ================================================================================================
+extern "C" {
+
+int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out) {
+    if (!out) return GX_ERR_ARG;
+    *out = nullptr;
+    if (Nx < 4 || Ny < 4 || (Nx & 1) || (Ny & 1) || Nz < 1 || Nl < 1 || Nl > 16 || Nm < 1 || Ns < 1)
+        return GX_ERR_ARG;
+    if (!splits(Nx) || !splits(Ny)) return GX_ERR_ARG;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return GX_ERR_CUDA;
+    gx_grid* g = new (std::nothrow) gx_grid();
+    if (!g) return GX_ERR_ALLOC;
+    g->Nx = Nx; g->Ny = Ny; g->Nz = Nz; g->Nl = Nl; g->Nm = Nm; g->Ns = Ns;
+    g->K = (Nx - 1) / 3; g->Q = (Ny - 1) / 3;
+    g->nakx = 2 * g->K + 1; g->naky = g->Q + 1;
+    g->nk = (long long)g->nakx * g->naky;
+    g->J = (3 * Nl - 1) / 2;
+    g->sp.resize(Ns);
+    g->adiabatic = (Ns == 1);
+    g->ks = find_set(Nx, Ny);
+    *out = g;                       // returned even on failure below so that gx_last_error works
+    if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
+
+    gauss_laguerre(g->J, g->xj, g->wj);
+    g->hT.resize((size_t)g->J * Nl);
+    g->hTinv.resize((size_t)Nl * g->J);
+    for (int j = 0; j < g->J; ++j)
+        for (int l = 0; l < Nl; ++l) {
+            const double psi = ((l & 1) ? -1.0 : 1.0) * laguerre(l, g->xj[j]);   // psi_l = (-1)^l L_l
+            g->hT[(size_t)j * Nl + l] = (float)psi;
+            g->hTinv[(size_t)l * g->J + j] = (float)(g->wj[j] * psi);
+        }
+    int rc;
+    if ((rc = dev_alloc(g, &g->dT, g->hT.size()))) return rc;
+    if ((rc = dev_alloc(g, &g->dTinv, g->hTinv.size()))) return rc;
+    GX_CUDA(g, cudaMemcpy(g->dT, g->hT.data(), g->hT.size() * sizeof(float), cudaMemcpyHostToDevice));
+    GX_CUDA(g, cudaMemcpy(g->dTinv, g->hTinv.data(), g->hTinv.size() * sizeof(float), cudaMemcpyHostToDevice));
+
+    std::vector<float2> tw(Nx);
+    for (int t = 0; t < Nx; ++t) {
+        const double a = 2.0 * M_PI * t / Nx;
+        tw[t] = make_float2((float)std::cos(a), (float)std::sin(a));
+    }
+    if ((rc = dev_alloc(g, &g->dtwx, (size_t)Nx))) return rc;
+    GX_CUDA(g, cudaMemcpy(g->dtwx, tw.data(), Nx * sizeof(float2), cudaMemcpyHostToDevice));
+    tw.resize(Ny);
+    for (int t = 0; t < Ny; ++t) {
+        const double a = 2.0 * M_PI * t / Ny;
+        tw[t] = make_float2((float)std::cos(a), (float)std::sin(a));
+    }
+    if ((rc = dev_alloc(g, &g->dtwy, (size_t)Ny))) return rc;
+    GX_CUDA(g, cudaMemcpy(g->dtwy, tw.data(), Ny * sizeof(float2), cudaMemcpyHostToDevice));
+
+    const size_t szj = (size_t)Ns * Nz * g->J;
+    if ((rc = dev_alloc(g, &g->dM, szj * g->nk))) return rc;
+    if ((rc = dev_alloc(g, &g->ddchi, szj * Nx * Ny))) return rc;
+    if ((rc = dev_alloc(g, &g->dbhat, szj * Nm * g->nk))) return rc;
+    return GX_OK;
+}
+
+int gx_grid_destroy(gx_grid* g) {
+    if (!g) return GX_ERR_ARG;
+    cudaFree(g->dT); cudaFree(g->dTinv); cudaFree(g->dM); cudaFree(g->dtwx); cudaFree(g->dtwy);
+    cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
+    cudaFree(g->dphi_rhs);
+    gx::lin_tables_free(g->lin);
+    delete g;
+    return GX_OK;
+}
+
+int gx_box_set(gx_grid* g, double dky, double dkx, double shat) {
+    if (!g) return GX_ERR_ARG;
+    if (!(dky > 0) || !(dkx > 0) || shat == 0.0) return fail(g, GX_ERR_ARG, "gx_box_set: dky, dkx > 0, shat != 0");
+    g->dky = dky; g->dkx = dkx; g->shat = shat;
+    g->box_set = true;
+    g->geo_set = false;
+    return GX_OK;
+}
+
+int gx_species_set(gx_grid* g, int s, double Z, double mass, double temp, double dens, double tprim,
+                   double fprim, double nu_ss) {
+    if (!g) return GX_ERR_ARG;
+    if (s < 0 || s >= g->Ns || Z == 0.0 || mass < 0 || !(temp > 0) || !(dens > 0))
+        return fail(g, GX_ERR_ARG, "gx_species_set: bad argument");
+    Species& sp = g->sp[s];
+    sp.Z = Z; sp.mass = mass; sp.temp = temp; sp.dens = dens; sp.tprim = tprim; sp.fprim = fprim; sp.nu = nu_ss;
+    sp.set = true;
+    g->geo_set = false;
+    return GX_OK;
+}
+
+int gx_adiabatic_set(gx_grid* g, int enabled, double tau_fac) {
+    if (!g) return GX_ERR_ARG;
+    if (enabled && g->Ns != 1) return fail(g, GX_ERR_ARG, "adiabatic electrons need Ns == 1");
+    g->adiabatic = enabled != 0;
+    g->tau_fac = tau_fac;
+    g->geo_set = false;
+    return GX_OK;
+}
+
+int gx_dissipation_set(gx_grid* g, double D_hyper, int n_hyper, double f_hyp) {
+    if (!g) return GX_ERR_ARG;
+    if (D_hyper < 0 || n_hyper < 0 || f_hyp < 0) return fail(g, GX_ERR_ARG, "negative dissipation parameter");
+    g->D_hyper = D_hyper; g->n_hyper = n_hyper; g->f_hyp = f_hyp;
+    g->geo_set = false;
+    return GX_OK;
+}
+
+int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const double* gds21,
+                    const double* gds22, const double* gbdrift, const double* gbdrift0,
+                    const double* cvdrift, const double* cvdrift0, const double* bgrad,
+                    const double* jacobian, double gradpar) {
+    if (!g) return GX_ERR_ARG;
+    if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
+    if (!bmag || !gds2 || !gds21 || !gds22) return fail(g, GX_ERR_ARG, "gx_geometry_set: null metric array");
+    if (!g->box_set) return fail(g, GX_ERR_STATE, "gx_geometry_set: call gx_box_set first");
+    for (const auto& s : g->sp)
+        if (!s.set) return fail(g, GX_ERR_STATE, "gx_geometry_set: call gx_species_set for every species first");
+    const int Nz = g->Nz;
+    g->bmag.assign(bmag, bmag + Nz); g->gds2.assign(gds2, gds2 + Nz);
+    g->gds21.assign(gds21, gds21 + Nz); g->gds22.assign(gds22, gds22 + Nz);
+    g->have_lin_geo = gbdrift && gbdrift0 && cvdrift && cvdrift0 && bgrad && jacobian;
+    if (g->have_lin_geo) {
+        g->gbdrift.assign(gbdrift, gbdrift + Nz); g->gbdrift0.assign(gbdrift0, gbdrift0 + Nz);
+        g->cvdrift.assign(cvdrift, cvdrift + Nz); g->cvdrift0.assign(cvdrift0, cvdrift0 + Nz);
+        g->bgrad.assign(bgrad, bgrad + Nz); g->jacobian.assign(jacobian, jacobian + Nz);
+    }
+    g->gradpar = gradpar;
+    for (int z = 0; z < Nz; ++z)
+        if (!(bmag[z] > 0)) return fail(g, GX_ERR_ARG, "gx_geometry_set: bmag must be positive");
+
+    // gyroaverage table M[s][z][j][kx][ky] = J0( sqrt(2 x_j b_s) ), b_s = kperp2 tau m / (Z^2 bmag^2)
+    // (PAPER.md line 85), kperp2 = ky^2 gds2 + 2 kx ky gds21/shat + kx^2 gds22/shat^2 (lines 681-686).
+    const int nakx = g->nakx, naky = g->naky, J = g->J, K = g->K;
+    std::vector<float> M((size_t)g->Ns * Nz * J * g->nk);
+    std::vector<double> kp2((size_t)Nz * g->nk);
+    for (int z = 0; z < Nz; ++z)
+        for (int i = 0; i < nakx; ++i) {
+            const double kx = g->dkx * (i <= K ? i : i - nakx);
+            for (int q = 0; q < naky; ++q) {
+                const double ky = g->dky * q;
+                kp2[((size_t)z * nakx + i) * naky + q] = ky * ky * gds2[z] + 2.0 * kx * ky * gds21[z] / g->shat +
+                                                          kx * kx * gds22[z] / (g->shat * g->shat);
+            }
+        }
+    for (int s = 0; s < g->Ns; ++s) {
+        const Species& sp = g->sp[s];
+        const double rho2 = sp.temp * sp.mass / (sp.Z * sp.Z);
+        for (int z = 0; z < Nz; ++z) {
+            const double fac = rho2 / (bmag[z] * bmag[z]);
+            for (int j = 0; j < J; ++j) {
+                float* Mp = M.data() + (((size_t)s * Nz + z) * J + j) * g->nk;
+                const double* kp = kp2.data() + (size_t)z * g->nk;
+                for (long long k = 0; k < g->nk; ++k) {
+                    const double b = kp[k] * fac;
+                    Mp[k] = (float)::j0(std::sqrt(2.0 * g->xj[j] * (b > 0 ? b : 0.0)));
+                }
+            }
+        }
+    }
+    GX_CUDA(g, cudaMemcpy(g->dM, M.data(), M.size() * sizeof(float), cudaMemcpyHostToDevice));
+
+    if (g->have_lin_geo) {
+        gx::LinHostInput in;
+        in.Nz = Nz; in.Nl = g->Nl; in.Nm = g->Nm; in.Ns = g->Ns; in.nakx = nakx; in.naky = naky;
+        in.dkx = g->dkx; in.dky = g->dky; in.shat = g->shat; in.gradpar = gradpar;
+        in.kp2 = kp2.data(); in.bmag = g->bmag.data(); in.gbdrift = g->gbdrift.data();
+        in.gbdrift0 = g->gbdrift0.data(); in.cvdrift = g->cvdrift.data(); in.cvdrift0 = g->cvdrift0.data();
+        in.bgrad = g->bgrad.data(); in.jacobian = g->jacobian.data();
+        in.adiabatic = g->adiabatic; in.tau_fac = g->tau_fac;
+        in.D_hyper = g->D_hyper; in.n_hyper = g->n_hyper; in.f_hyp = g->f_hyp;
+        for (const auto& sp : g->sp)
+            in.species.push_back({sp.Z, sp.mass, sp.temp, sp.dens, sp.tprim, sp.fprim, sp.nu});
+        std::string msg;
+        size_t bytes = 0;
+        if (!gx::lin_tables_build(in, g->lin, bytes, msg)) return fail(g, GX_ERR_CUDA, msg);
+        g->bytes += bytes;
+        if (!g->dphi_rhs) {
+            int rc = dev_alloc(g, &g->dphi_rhs, (size_t)Nz * g->nk);
+            if (rc) return rc;
+        }
+    }
+    g->geo_set = true;
+    return GX_OK;
+}
+
+int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_dev || !phi_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: null pointer");
+    if (g_dev == out_dev) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: out must not alias g");
+    if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
+    if (!g->geo_set) return fail(g, GX_ERR_STATE, "gx_nonlinear_rhs: geometry not set");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const NlParams p = make_params(g, g_dev, phi_dev, out_dev);
+    const int szj = g->Ns * g->Nz * g->J;
+    GX_CUDA(g, g->ks->launch_chi(p, szj, st));
+    GX_CUDA(g, g->ks->launch_bracket(p, szj * g->Nm, st));
+    dim3 grid((unsigned)((g->nk + 255) / 256), (unsigned)(g->Ns * g->Nm * g->Nz));
+    if (g->Nl <= 4) gx::laguerre_inverse_kernel<4, 5><<<grid, 256, 0, st>>>(p, (int)g->nk);
+    else if (g->Nl <= 8) gx::laguerre_inverse_kernel<8, 11><<<grid, 256, 0, st>>>(p, (int)g->nk);
+    else gx::laguerre_inverse_kernel<16, 23><<<grid, 256, 0, st>>>(p, (int)g->nk);
+    GX_CUDA(g, cudaGetLastError());
+    return GX_OK;
+}
+
+int gx_nonlinear_rhs_host(gx_grid* g, const void* g_host, const void* phi_host, void* out_host, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_host || !phi_host || !out_host) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs_host: null pointer");
+    const size_t ng = (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk, np = (size_t)g->Nz * g->nk;
+    int rc;
+    if (!g->dgbuf) {
+        if ((rc = dev_alloc(g, &g->dgbuf, ng))) return rc;
+        if ((rc = dev_alloc(g, &g->doutbuf, ng))) return rc;
+        if ((rc = dev_alloc(g, &g->dphibuf, np))) return rc;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    GX_CUDA(g, cudaMemcpyAsync(g->dgbuf, g_host, ng * sizeof(float2), cudaMemcpyHostToDevice, st));
+    GX_CUDA(g, cudaMemcpyAsync(g->dphibuf, phi_host, np * sizeof(float2), cudaMemcpyHostToDevice, st));
+    if ((rc = gx_nonlinear_rhs(g, g->dgbuf, g->dphibuf, g->doutbuf, cuda_stream))) return rc;
+    GX_CUDA(g, cudaMemcpyAsync(out_host, g->doutbuf, ng * sizeof(float2), cudaMemcpyDeviceToHost, st));
+    GX_CUDA(g, cudaStreamSynchronize(st));
+    return GX_OK;
+}
+
+int gx_field_solve(gx_grid* g, const void* g_dev, void* phi_dev, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_dev || !phi_dev) return fail(g, GX_ERR_ARG, "gx_field_solve: null pointer");
+    if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_field_solve: full geometry not set");
+    cudaError_t e = gx::lin_field_solve(g->lin, (const float2*)g_dev, (float2*)phi_dev, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(g, e, "gx_field_solve");
+    return GX_OK;
+}
+
+int gx_linear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_dev || !phi_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_linear_rhs: null pointer");
+    if (g_dev == out_dev) return fail(g, GX_ERR_ARG, "gx_linear_rhs: out must not alias g");
+    if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_linear_rhs: full geometry not set");
+    cudaError_t e = gx::lin_rhs(g->lin, (const float2*)g_dev, (const float2*)phi_dev, (float2*)out_dev,
+                                /*accumulate=*/false, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(g, e, "gx_linear_rhs");
+    return GX_OK;
+}
+
+int gx_rhs(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_rhs: null pointer");
+    if (g_dev == out_dev) return fail(g, GX_ERR_ARG, "gx_rhs: out must not alias g");
+    if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_rhs: full geometry not set");
+    int rc;
+    if ((rc = gx_field_solve(g, g_dev, g->dphi_rhs, cuda_stream))) return rc;
+    if ((rc = gx_nonlinear_rhs(g, g_dev, g->dphi_rhs, out_dev, cuda_stream))) return rc;
+    cudaError_t e = gx::lin_rhs(g->lin, (const float2*)g_dev, g->dphi_rhs, (float2*)out_dev,
+                                /*accumulate=*/true, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(g, e, "gx_rhs");
+    return GX_OK;
+}
+
+int gx_query(gx_grid* g, int what, long long* value) {
+    if (!g || !value) return GX_ERR_ARG;
+    switch (what) {
+        case GX_Q_NAKX: *value = g->nakx; break;
+        case GX_Q_NAKY: *value = g->naky; break;
+        case GX_Q_NJ: *value = g->J; break;
+        case GX_Q_G_ELEMS: *value = (long long)g->Ns * g->Nm * g->Nl * g->Nz * g->nk; break;
+        case GX_Q_PHI_ELEMS: *value = (long long)g->Nz * g->nk; break;
+        case GX_Q_WORKSPACE_BYTES: *value = (long long)g->bytes; break;
+        case GX_Q_LAUNCHES_PER_NL: *value = 3; break;
+        case GX_Q_LAUNCHES_PER_RHS: *value = 3 + gx::kLinLaunchesFieldSolve + gx::kLinLaunchesRhs; break;
+        case GX_Q_NL_FLOPS: *value = nl_flops(g); break;
+        case GX_Q_NL_BYTES:
+            *value = 8LL * (2LL * g->Ns * g->Nm * g->Nl * g->Nz * g->nk + (long long)g->Nz * g->nk);
+            break;
+        default: return fail(g, GX_ERR_ARG, "gx_query: unknown code");
+    }
+    return GX_OK;
+}
+
+int gx_export_maps(gx_grid* g, int* kx_index, int* ky_index, int* pad_row, unsigned char* mask,
+                   double* lag_nodes, double* lag_weights) {
+    if (!g) return GX_ERR_ARG;
+    for (int i = 0; i < g->nakx; ++i) {
+        const int a = i <= g->K ? i : i - g->nakx;
+        if (kx_index) kx_index[i] = a;
+        if (pad_row) pad_row[i] = a >= 0 ? a : a + g->Nx;
+    }
+    if (ky_index)
+        for (int q = 0; q < g->naky; ++q) ky_index[q] = q;
+    if (mask) {
+        const int Nyc = g->Ny / 2 + 1;
+        for (int r = 0; r < g->Nx; ++r)
+            for (int q = 0; q < Nyc; ++q)
+                mask[(size_t)r * Nyc + q] = ((r <= g->K || r >= g->Nx - g->K) && q <= g->Q) ? 1 : 0;
+    }
+    for (int j = 0; j < g->J; ++j) {
+        if (lag_nodes) lag_nodes[j] = g->xj[j];
+        if (lag_weights) lag_weights[j] = g->wj[j];
+    }
+    return GX_OK;
+}
+
+int gx_export_tables(gx_grid* g, float* T, float* Tinv, float* M) {
+    if (!g) return GX_ERR_ARG;
+    if (T) std::memcpy(T, g->hT.data(), g->hT.size() * sizeof(float));
+    if (Tinv) std::memcpy(Tinv, g->hTinv.data(), g->hTinv.size() * sizeof(float));
+    if (M) {
+        if (!g->geo_set) return fail(g, GX_ERR_STATE, "gx_export_tables: geometry not set");
+        GX_CUDA(g, cudaMemcpy(M, g->dM, (size_t)g->Ns * g->Nz * g->J * g->nk * sizeof(float), cudaMemcpyDeviceToHost));
+    }
+    return GX_OK;
+}
+
+const char* gx_last_error(gx_grid* g) { return g ? g->err.c_str() : "null handle"; }
+
+}  // extern "C"

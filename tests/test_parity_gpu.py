@@ -1,0 +1,233 @@
+"""Parity of the CUDA path (through the C-ABI) against the fp64 oracle on the same seeded inputs.
+
+Bar (BASELINE.json north_star): max|gpu - oracle| / max|oracle| <= 2e-5 per output array; index
+maps, mask and (to fp64 rounding) the Gauss-Laguerre rule must match exactly."""
+import numpy as np
+import pytest
+
+import gx_oracle as O
+from paper_2209_06731_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+TOL = 2e-5
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def _grid(cfg, geo):
+    from paper_2209_06731_b200 import binding
+    return binding.Grid(cfg, geo)
+
+
+def _oracle_phi(cfg, geo, G):
+    return O.field_solve(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species,
+                         tau_fac=cfg.tau_fac, adiabatic=(cfg.Ns == 1)).astype(np.complex64)
+
+
+def _gpu_nl(torch, grid, G, Phi):
+    g = torch.from_numpy(G).cuda()
+    phi = torch.from_numpy(Phi).cuda()
+    out = torch.full_like(g, float("nan"))
+    grid.nonlinear_rhs(g, phi, out)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def _oracle_nl(cfg, geo, G, Phi, **kw):
+    return O.nonlinear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, **kw)
+
+
+def test_maps_mask_and_quadrature_match_oracle(torch_cuda):
+    for name in ["tiny", "cyclone", "hires", "w7x-shape"]:
+        cfg = I.named_config(name)
+        small = I.Config(name, cfg.Nx, cfg.Ny, 2, cfg.Nl, 1, cfg.species, geometry=cfg.geometry, seed=1)
+        grid = _grid(small, I.geometry_arrays(small))
+        m = grid.export_maps()
+        assert np.array_equal(m["kx_index"], O.kx_index(cfg.Nx))
+        assert np.array_equal(m["ky_index"], O.ky_index(cfg.Ny))
+        assert np.array_equal(m["pad_row"], O.pad_row(cfg.Nx))
+        assert np.array_equal(m["mask"], O.dealias_mask(cfg.Nx, cfg.Ny))
+        x, w = O.gauss_laguerre(small.nj)
+        assert np.allclose(m["lag_nodes"], x, rtol=1e-12, atol=0)
+        assert np.allclose(m["lag_weights"], w, rtol=1e-10, atol=0)
+        from paper_2209_06731_b200 import binding
+        T, Tinv, M = binding.gx_export_tables(grid.h, small.Nl, small.Ns * 2 * small.nj * small.nakx * small.naky)
+        _, _, To, Tinvo = O.laguerre_matrices(small.Nl)
+        assert np.array_equal(T, To.astype(np.float32)) or np.max(np.abs(T - To)) <= 2e-7 * np.max(np.abs(To))
+        assert np.max(np.abs(Tinv - Tinvo)) <= 2e-7 * np.max(np.abs(Tinvo))
+        geo = grid.geo
+        kx, ky = small.dkx * O.kx_index(cfg.Nx), small.dky * O.ky_index(cfg.Ny)
+        sp = small.species[0]
+        b = O.b_species(O.kperp2(kx, ky, geo["gds2"], geo["gds21"], geo["gds22"], small.shat), geo["bmag"],
+                        sp.Z, sp.mass, sp.temp)
+        Mo = O.gyro_table(b, x)                       # [z][j][kx][ky]
+        Mg = M.reshape(small.Ns, 2, small.nj, small.nakx, small.naky)[0]
+        assert np.max(np.abs(Mg - Mo)) < 1.5e-7
+        grid.close()
+
+
+def test_tiny_full_parity_against_definition(torch_cuda):
+    cfg = I.named_config("tiny")
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = _grid(cfg, geo)
+    out = _gpu_nl(torch_cuda, grid, G, Phi)
+    ref = _oracle_nl(cfg, geo, G, Phi, method="conv_c")        # the definition, every plane
+    assert np.all(np.isfinite(out))
+    assert O.relative_max_error(out, ref) <= TOL
+    for l in range(cfg.Nl):                                   # per-l slabs too (stricter)
+        assert O.relative_max_error(out[:, :, l], ref[:, :, l]) <= TOL
+    # output properties that hold at any size
+    K = (cfg.nakx - 1) // 2
+    s = np.max(np.abs(ref))
+    assert np.max(np.abs(out[..., cfg.nakx - 1:K:-1, 0] - np.conj(out[..., 1:K + 1, 0]))) < 1e-5 * s
+    assert np.max(np.abs(out[..., 0, 0])) < 1e-5 * s
+    grid.close()
+
+
+def test_single_mode_closed_form_on_gpu(torch_cuda):
+    # b = 0 (mass -> 0 gives M == 1), one chi mode, one g mode: exactly two output modes (oracle pin 4)
+    cfg = I.Config("one", 16, 16, 2, 1, 1, [I.Species(mass=1e-30)], seed=3)
+    geo = I.geometry_arrays(cfg)
+    nakx, naky = cfg.nakx, cfg.naky
+    G = np.zeros(cfg.g_shape, np.complex64)
+    Phi = np.zeros(cfg.phi_shape, np.complex64)
+    (pa, pb), (qa, qb) = (2, 1), (-1, 3)
+    cp, gq = np.complex64(0.75 - 0.25j), np.complex64(-0.5 + 1.0j)
+    Phi[:, pa, pb] = cp
+    G[0, 0, 0, :, qa + nakx, qb] = gq
+    grid = _grid(cfg, geo)
+    out = _gpu_nl(torch_cuda, grid, G, Phi)
+    cross = (cfg.dkx * pa) * (cfg.dky * qb) - (cfg.dky * pb) * (cfg.dkx * qa)
+    expect = np.zeros_like(out, dtype=np.complex128)
+    expect[0, 0, 0, :, pa + qa, pb + qb] = -cross * complex(cp) * complex(gq)
+    expect[0, 0, 0, :, (qa - pa) + nakx, qb - pb] = cross * np.conj(complex(cp)) * complex(gq)
+    assert np.max(np.abs(out - expect)) < 2e-6 * np.max(np.abs(expect))
+    grid.close()
+
+
+def test_cyclone_parity_full_array_and_sampled_definition(torch_cuda):
+    cfg = I.named_config("cyclone")
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = _grid(cfg, geo)
+    out = _gpu_nl(torch_cuda, grid, G, Phi)
+    assert np.all(np.isfinite(out))
+    # full array against the pseudo-spectral oracle path (several tiles, ragged 127 x 22 planes)
+    ref = _oracle_nl(cfg, geo, G, Phi, method="dft")
+    err = O.relative_max_error(out, ref)
+    assert err <= TOL, err
+    for m in range(cfg.Nm):
+        assert O.relative_max_error(out[:, m], ref[:, m]) <= TOL
+    # sampled planes against the definition (direct convolution)
+    planes = [(0, 0, 0), (0, 3, 11), (0, 7, 23)]
+    refc = _oracle_nl(cfg, geo, G, Phi, method="conv_c", planes=planes)
+    for (s, m, z) in planes:
+        e = np.max(np.abs(out[s, m, :, z] - refc[s, m, :, z])) / np.max(np.abs(refc[s, m, :, z]))
+        assert e <= TOL, (s, m, z, e)
+    # free-energy invariant on the GPU result (holds at any size)
+    W = O.free_energy_moment(G.astype(np.complex128), out.astype(np.complex128))
+    scale = np.einsum("smlzxy->smz", np.abs(G.astype(np.complex128)) * np.abs(out))
+    assert np.max(np.abs(W) / scale) < 2e-5
+    grid.close()
+
+
+@pytest.mark.parametrize("name,planes", [
+    ("kinetic", [(0, 0, 0), (1, 0, 5), (1, 7, 31), (0, 4, 16)]),
+    ("hires", [(0, 0, 0), (0, 15, 31), (0, 6, 9)]),
+    ("stellarator", [(0, 0, 0), (0, 11, 127), (0, 5, 64)]),
+    ("w7x-shape", [(0, 0, 0), (0, 7, 100)]),
+])
+def test_large_configs_sampled_planes(torch_cuda, name, planes):
+    """Full-size runs in the bench's launch configuration; the oracle evaluates sampled (s,m,z) planes."""
+    torch = torch_cuda
+    cfg = I.named_config(name)
+    geo = I.geometry_arrays(cfg)
+    sm = sorted({(s, m) for (s, m, z) in planes} | {(s, 0) for s in range(cfg.Ns)})
+    G = I.make_state(cfg, geo, planes=sm)           # only the sampled (s,m) slabs are non-zero
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = _grid(cfg, geo)
+    out = _gpu_nl(torch, grid, G, Phi)
+    ref = _oracle_nl(cfg, geo, G, Phi, method="dft", planes=planes)
+    for (s, m, z) in planes:
+        a, r = out[s, m, :, z], ref[s, m, :, z]
+        assert np.all(np.isfinite(a))
+        e = np.max(np.abs(a - r)) / np.max(np.abs(r))
+        assert e <= TOL, (name, s, m, z, e)
+    # slabs that were zero on input must be exactly zero on output (bilinearity)
+    zero_sm = [(s, m) for s in range(cfg.Ns) for m in range(cfg.Nm) if (s, m) not in sm]
+    if zero_sm:
+        s, m = zero_sm[0]
+        assert np.all(out[s, m] == 0)
+    grid.close()
+
+
+def test_zero_input_and_error_paths(torch_cuda):
+    torch = torch_cuda
+    from paper_2209_06731_b200 import binding as B
+    cfg = I.named_config("tiny")
+    grid = _grid(cfg, I.geometry_arrays(cfg))
+    g = torch.zeros(cfg.g_shape, dtype=torch.complex64, device="cuda")
+    phi = torch.zeros(cfg.phi_shape, dtype=torch.complex64, device="cuda")
+    out = torch.full_like(g, float("nan"))
+    grid.nonlinear_rhs(g, phi, out)
+    torch.cuda.synchronize()
+    assert torch.all(out == 0)
+    with pytest.raises(B.GxError) as e:
+        B.gx_nonlinear_rhs(grid.h, g.data_ptr(), phi.data_ptr(), g.data_ptr())
+    assert e.value.code == B.GX_ERR_ARG
+    with pytest.raises(B.GxError) as e:
+        B.gx_nonlinear_rhs(grid.h, None, phi.data_ptr(), out.data_ptr())
+    assert e.value.code == B.GX_ERR_ARG
+    grid.close()
+    for bad in [(15, 16), (16, 2), (16, 34)]:
+        with pytest.raises(B.GxError) as e:
+            B.gx_grid_create(bad[0], bad[1], 4, 2, 2, 1)
+        assert e.value.code == B.GX_ERR_ARG
+    with pytest.raises(B.GxError) as e:
+        B.gx_grid_create(48, 48, 4, 2, 2, 1)       # valid size, no kernel instantiation
+    assert e.value.code == B.GX_ERR_UNSUPPORTED
+    h = B.gx_grid_create(16, 16, 4, 2, 2, 1)
+    with pytest.raises(B.GxError) as e:
+        B.gx_nonlinear_rhs(h, g.data_ptr(), phi.data_ptr(), out.data_ptr())
+    assert e.value.code == B.GX_ERR_STATE
+    B.gx_grid_destroy(h)
+
+
+def test_host_entry_point_matches_device_entry_point(torch_cuda):
+    torch = torch_cuda
+    cfg = I.named_config("tiny")
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = _grid(cfg, geo)
+    out_dev = _gpu_nl(torch, grid, G, Phi)
+    gh, ph = torch.from_numpy(G).pin_memory(), torch.from_numpy(Phi).pin_memory()
+    oh = torch.empty_like(gh).pin_memory()
+    grid.nonlinear_rhs_host(gh, ph, oh)
+    assert np.array_equal(oh.numpy(), out_dev)
+    grid.close()
+
+
+def test_field_solve_parity(torch_cuda):
+    torch = torch_cuda
+    for name in ["tiny", "cyclone"]:
+        cfg = I.named_config(name)
+        geo = I.geometry_arrays(cfg)
+        G = I.make_state(cfg, geo, planes=[(s, 0) for s in range(cfg.Ns)])
+        grid = _grid(cfg, geo)
+        g = torch.from_numpy(G).cuda()
+        phi = torch.empty(cfg.phi_shape, dtype=torch.complex64, device="cuda")
+        grid.field_solve(g, phi)
+        torch.cuda.synchronize()
+        ref = O.field_solve(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, tau_fac=cfg.tau_fac)
+        assert O.relative_max_error(phi.cpu().numpy(), ref) <= TOL
+        grid.close()
