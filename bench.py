@@ -1,0 +1,324 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the nonlinear E×B hot path (gx_nonlinear_rhs) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config cyclone] [--impl reference]
+
+One "step" = one gx_nonlinear_rhs call (all rows a1-a8 of DESIGN.md) on one batch of seeded synthetic
+input of the named configuration.  Prints ONE JSON line (rank 0).  Timing: CUDA events on the launch
+stream, bracketed by barrier + synchronize, max over ranks.  The inputs rotate through buffer sets
+whose total size exceeds the 126 MB L2 so that g is read from and out written to HBM every step.
+
+--impl reference times the fp64 CPU oracle (oracle/gx_oracle.py, as it stands) on a bounded sample
+of the same workload on the host cores; it is a deliberately slow baseline, not the target.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2209_06731_b200 import dist as D          # noqa: E402
+from paper_2209_06731_b200 import inputs as I        # noqa: E402
+
+METRIC = "nonlinear_rhs_evals_per_s"
+UNIT = "evals/s"
+FP32_LANES_PER_SM = 128
+L2_BYTES = 126e6
+
+
+def workload_name(cfg):
+    return (f"{cfg.name}: Nx={cfg.Nx} Ny={cfg.Ny} Nz={cfg.Nz} Nl={cfg.Nl} Nm={cfg.Nm} Ns={cfg.Ns} "
+            f"(nakx={cfg.nakx} naky={cfg.naky} J={cfg.nj})")
+
+
+# ------------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons with NVML in a thread while the timed region runs."""
+
+    def __init__(self, index=0, period=0.01):
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self.period, self._stop, self._thr, self.ok = period, threading.Event(), None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def _run(self):
+        nv = self.nv
+        names = {"hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
+                 "hw_power_brake_slowdown": 0x80, "sw_power_cap": 0x4}
+        while not self._stop.is_set():
+            try:
+                self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
+                r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for k, bit in names.items():
+                    if r & bit:
+                        self.reasons.add(k)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def __enter__(self):
+        if self.ok:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+        return self
+
+    def __exit__(self, *a):
+        self._stop.set()
+        if self._thr:
+            self._thr.join()
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "samples": 0}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------- CPU oracle leg
+def oracle_sample(cfg, geo, budget_s=12.0):
+    """Times oracle.nonlinear_rhs (pseudo-spectral naive-DFT path, fp64, as it stands) on a bounded sample
+    of the workload: whole evaluations when one fits the budget, else a subset of the independent
+    (s,m,z) planes scaled to a whole evaluation.  -> (evals/s, description, seconds spent)."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import gx_oracle as O
+    sm_all = [(s, m) for s in range(cfg.Ns) for m in range(cfg.Nm)]
+    small = int(np.prod(cfg.g_shape)) <= 4_500_000
+    sm_sel = sm_all if small else sm_all[:: max(1, len(sm_all) // 4)][:4]
+    need_sm = sorted(set(sm_sel) | {(s, 0) for s in range(cfg.Ns)})
+    G = I.make_state(cfg, geo, planes=None if small else need_sm)
+    Phi = O.field_solve(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, tau_fac=cfg.tau_fac,
+                        adiabatic=(cfg.Ns == 1)).astype(np.complex64)
+    n_all = len(sm_all) * cfg.Nz
+    cand = [(s, m, z) for (s, m) in sm_sel for z in range(cfg.Nz)]
+
+    def run(planes):
+        return O.nonlinear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species,
+                               method="dft", planes=planes)
+
+    probe = cand[:: max(1, len(cand) // 4)][:4]
+    t0 = time.perf_counter()
+    run(probe)
+    per_plane = (time.perf_counter() - t0) / len(probe)
+    if small and per_plane * n_all <= budget_s:
+        n = max(1, int(budget_s / (per_plane * n_all)))
+        t0 = time.perf_counter()
+        for _ in range(n):
+            run(None)
+        dt = time.perf_counter() - t0
+        return n / dt, f"{n} whole evaluations ({n_all} (s,m,z) planes each); oracle path B (naive DFT, fp64)", dt
+    k = max(len(probe), min(len(cand), int(budget_s / per_plane)))
+    planes = cand[:: max(1, len(cand) // k)][:k]
+    t0 = time.perf_counter()
+    run(planes)
+    dt = time.perf_counter() - t0
+    return ((len(planes) / n_all) / dt,
+            f"{len(planes)} of {n_all} independent (s,m,z) planes, scaled to a whole evaluation; "
+            f"oracle path B (naive DFT, fp64)", dt)
+
+
+def host_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = max([p.get("num_threads", 1) for p in threadpool_info()] + [1])
+        return int(n)
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank, _, world = D.env_world()
+    if rank != 0:
+        return 0
+    cfg = I.named_config(args.config)
+    geo = I.geometry_arrays(cfg)
+    steps = max(1, min(args.steps, 3))
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(cfg, geo, budget_s=2.0)
+    vals, secs, sample = [], 0.0, ""
+    for _ in range(steps):
+        v, sample, dt = oracle_sample(cfg, geo, budget_s=10.0)
+        vals.append(v)
+        secs += dt
+    value = float(np.mean(vals))
+    cores = host_threads()
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 / value, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(cfg), "note": "fp64 CPU oracle on host cores; bounded sample per step"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------- GPU leg
+def run_gpu(args):
+    import torch
+    from paper_2209_06731_b200 import binding as B
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product path has no CPU fallback)")
+    rank, local_rank, world = D.init("nccl") if int(os.environ.get("WORLD_SIZE", "1")) > 1 else (0, 0, 1)
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    cfg = I.named_config(args.config)
+    geo = I.geometry_arrays(cfg)
+    m0, m1, Nm_global = D.hermite_block(cfg.Nm, rank, world)      # weak scaling: one Hermite block per rank
+    grid = B.Grid(cfg, geo)
+    flops = grid.query(B.GX_Q_NL_FLOPS)
+    alg_bytes = grid.query(B.GX_Q_NL_BYTES)
+    launches_per_call = grid.query(B.GX_Q_LAUNCHES_PER_NL)
+
+    # seeded state of this rank's Hermite block; phi from the library's own field solve (product path)
+    cfg_rank = I.Config(**{**cfg.__dict__, "seed": cfg.seed + 1000 * rank})
+    g_elems = int(np.prod(cfg.g_shape))
+    set_bytes = 2 * g_elems * 8 + int(np.prod(cfg.phi_shape)) * 8
+    nsets = max(2, int(np.ceil(4.2 * L2_BYTES / set_bytes)))
+    nsets = min(nsets, max(2, int(40e9 // set_bytes)))
+    G0 = I.make_state(cfg_rank, geo)
+    g_host = torch.from_numpy(G0)
+    gs, phis, outs = [], [], []
+    for k in range(nsets):
+        g = g_host.to(dev)
+        if k:
+            g.mul_(1.0 + 0.01 * k)          # distinct contents per set, same spectrum
+        phi = torch.empty(cfg.phi_shape, dtype=torch.complex64, device=dev)
+        grid.field_solve(g, phi)
+        gs.append(g); phis.append(phi); outs.append(torch.empty_like(g))
+    torch.cuda.synchronize()
+
+    def step(i):
+        k = i % nsets
+        grid.nonlinear_rhs(gs[k], phis[k], outs[k])
+
+    for i in range(args.warmup):
+        step(i)
+    torch.cuda.synchronize()
+    D.barrier()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clk:
+        torch.cuda.synchronize()
+        ev0.record()
+        for i in range(args.steps):
+            step(i)
+        ev1.record()
+        torch.cuda.synchronize()
+    D.barrier()
+    sec = ev0.elapsed_time(ev1) * 1e-3
+    value, sec_max = D.aggregate_throughput(float(args.steps), sec, device=dev)
+    assert all(torch.isfinite(o.real).all() for o in outs[:2])
+
+    # per-kernel durations, live, same launch configuration (events around each kernel)
+    B.gx_profile_set(grid.h, 1)
+    nprof = min(args.steps, 200)
+    for i in range(nprof):
+        step(i)
+    kms, ncalls = B.gx_profile_get(grid.h)
+    B.gx_profile_set(grid.h, 0)
+    kern_us = [1e3 * t / max(ncalls, 1) for t in kms]
+
+    # end-to-end through the host entry point: pinned host buffers, H2D + compute + D2H every step
+    gh = g_host.pin_memory()
+    ph = phis[0].cpu().pin_memory()
+    oh = torch.empty_like(gh).pin_memory()
+    e2e_steps = max(3, min(args.steps, 30))
+    for _ in range(3):
+        grid.nonlinear_rhs_host(gh, ph, oh)
+    torch.cuda.synchronize()
+    D.barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        grid.nonlinear_rhs_host(gh, ph, oh)          # synchronises before returning
+    torch.cuda.synchronize()
+    e2e_sec = time.perf_counter() - t0
+    e2e_value, _ = D.aggregate_throughput(float(e2e_steps), e2e_sec, device=dev)
+
+    line = None
+    if rank == 0:
+        peaks = {}
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        except Exception:
+            pass
+        clocks = clk.summary()
+        sm_max = peaks.get("sm_max_mhz") or clocks.get("sm_max_mhz") or 1965.0
+        n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+        peak_tflops = n_sm * FP32_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
+        # dominant kernel: bracket_kernel.  Its algorithmic flops = whole-call flops minus the chi planes'
+        # transforms and multiplies (SURVEY 8d formula with nT = 3P) -- see DESIGN.md "Roofline".
+        P = cfg.Ns * cfg.Nm * cfg.Nz * cfg.nj
+        SZJ = cfg.Ns * cfg.Nz * cfg.nj
+        fft = 5 * cfg.Nx * np.log2(cfg.Nx) * cfg.naky + 2.5 * cfg.Ny * np.log2(cfg.Ny) * cfg.Nx
+        nk = cfg.nakx * cfg.naky
+        br_flops = 3 * P * fft + 3 * cfg.Nx * cfg.Ny * P + (4 * cfg.nj * cfg.Nl) * nk * cfg.Ns * cfg.Nm * cfg.Nz + 4 * nk * P
+        br_sec = kern_us[1] * 1e-6
+        achieved = br_flops / br_sec / 1e12 if br_sec > 0 else 0.0
+        traffic = None
+        try:
+            traffic = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get(cfg.name, {}).get("bracket_kernel")
+        except Exception:
+            pass
+        roofline = {"bound": "alu", "kernel": "bracket_kernel", "achieved": achieved, "peak": peak_tflops,
+                    "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": traffic,
+                    "peak_source": f"{n_sm} SMs x 128 FP32 lanes x 2 x {sm_max:.0f} MHz (max SM clock, MEASURED_PEAKS.json)",
+                    "kernel_us": {"chi_planes": kern_us[0], "bracket": kern_us[1], "laguerre_inverse": kern_us[2]},
+                    "kernel_share_of_step": kern_us[1] / max(sum(kern_us), 1e-9),
+                    "whole_call": {"alg_flops": flops, "alg_bytes": alg_bytes,
+                                   "frac_of_fp32_peak": flops * value / world / 1e12 / peak_tflops,
+                                   "hbm_gbs": alg_bytes * value / world / 1e9,
+                                   "hbm_peak_gbs": peaks.get("hbm_gbs")}}
+        cpu_v, cpu_sample, _ = (oracle_sample(cfg, geo, budget_s=12.0) if world == 1 and not args.skip_cpu_baseline
+                                  else (None, "skipped (N>1 or --skip-cpu-baseline)", 0))
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+                "warmup": args.warmup, "ms_per_step": 1e3 * sec_max / args.steps, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+                "config": {"workload": workload_name(cfg), "hermite_moments_global": Nm_global,
+                           "parallelism": f"hermite-block x{world}, no collective",
+                           "l2": f"inputs rotate through {nsets} buffer sets ({nsets * set_bytes / 1e6:.0f} MB > 126 MB L2)",
+                           "grid_point_moments_per_s": value * cfg.grid_point_moments,
+                           "phi": "gx_field_solve on device (Boltzmann electrons)" if cfg.Ns == 1 else "gx_field_solve on device"},
+                "clocks": clocks,
+                "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (g_elems + int(np.prod(cfg.phi_shape))) * 8,
+                        "d2h_bytes_per_step": g_elems * 8, "steps": e2e_steps},
+                "gpu_launches": launches_per_call * args.steps,
+                "roofline": roofline,
+                "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
+                                 "sample": cpu_sample}}
+        print(json.dumps(line))
+    grid.close()
+    D.finalize()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=100)
+    ap.add_argument("--config", default="cyclone", choices=I.CONFIG_NAMES + ["w7x-shape"])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--skip-cpu-baseline", action="store_true", help="omit the oracle timing (ncu passes)")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3
+    return run_reference(args) if args.impl == "reference" else run_gpu(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

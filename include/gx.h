@@ -125,6 +125,13 @@ int gx_export_maps(gx_grid* g, int* kx_index, int* ky_index, int* pad_row, unsig
  * T [nj*Nl], Tinv [Nl*nj], M [Ns*Nz*nj*nakx*naky] (needs geometry set; may be NULL). */
 int gx_export_tables(gx_grid* g, float* T, float* Tinv, float* M);
 
+/* Per-kernel timing for the roofline report.  While enabled, every gx_nonlinear_rhs records CUDA
+ * events on the launch stream around each of its kernels.  gx_profile_get synchronises those events,
+ * adds the elapsed milliseconds of [0] chi planes, [1] bracket, [2] inverse Laguerre to ms[0..2],
+ * writes the number of profiled calls to *calls, and resets the accumulators. */
+int gx_profile_set(gx_grid* g, int enabled);
+int gx_profile_get(gx_grid* g, double* ms, long long* calls);
+
 const char* gx_last_error(gx_grid* g);
 
 #ifdef __cplusplus

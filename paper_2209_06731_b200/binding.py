@@ -22,7 +22,7 @@ GX_OK, GX_ERR_ARG, GX_ERR_STATE, GX_ERR_UNSUPPORTED, GX_ERR_CUDA, GX_ERR_ALLOC =
 EXPORTED = ["gx_grid_create", "gx_grid_destroy", "gx_box_set", "gx_species_set", "gx_adiabatic_set",
             "gx_dissipation_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_host",
             "gx_field_solve", "gx_rhs", "gx_linear_rhs", "gx_query", "gx_export_maps",
-            "gx_export_tables", "gx_last_error"]
+            "gx_export_tables", "gx_profile_set", "gx_profile_get", "gx_last_error"]
 
 _lib = None
 
@@ -58,6 +58,8 @@ def load():
     lib.gx_query.argtypes = [vp, i, C.POINTER(C.c_longlong)]
     lib.gx_export_maps.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.gx_export_tables.argtypes = [vp, vp, vp, vp]
+    lib.gx_profile_set.argtypes = [vp, i]
+    lib.gx_profile_get.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
     lib.gx_last_error.argtypes = [vp]
     lib.gx_last_error.restype = C.c_char_p
     for name in EXPORTED:
@@ -163,6 +165,18 @@ def gx_export_tables(h, Nl, want_M_elems=0):
     M = np.zeros(want_M_elems, np.float32) if want_M_elems else None
     _check(h, load().gx_export_tables(h, T.ctypes.data, Tinv.ctypes.data, None if M is None else M.ctypes.data))
     return T, Tinv, M
+
+
+def gx_profile_set(h, enabled):
+    _check(h, load().gx_profile_set(h, int(enabled)))
+
+
+def gx_profile_get(h):
+    """-> (ms[3] summed over the profiled calls: chi, bracket, laguerre-inverse; number of calls)"""
+    ms = (C.c_double * 3)(0.0, 0.0, 0.0)
+    n = C.c_longlong()
+    _check(h, load().gx_profile_get(h, ms, C.byref(n)))
+    return [ms[0], ms[1], ms[2]], n.value
 
 
 # ---- convenience wrapper (marshalling only) -------------------------------------------------------

@@ -149,6 +149,9 @@ struct gx_grid {
     gx::LinTables lin;                                                  // linear-term tables
     float2* dphi_rhs = nullptr;                                         // phi of gx_rhs
     size_t bytes = 0;
+    bool profile = false;
+    std::vector<cudaEvent_t> ev_pool;          // 4 events per profiled call
+    size_t ev_used = 0;
     std::string err;
 };
 
@@ -280,6 +283,7 @@ int gx_grid_destroy(gx_grid* g) {
     cudaFree(g->dT); cudaFree(g->dTinv); cudaFree(g->dM); cudaFree(g->dtwx); cudaFree(g->dtwy);
     cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
     cudaFree(g->dphi_rhs);
+    for (auto e : g->ev_pool) cudaEventDestroy(e);
     gx::lin_tables_free(g->lin);
     delete g;
     return GX_OK;
@@ -410,13 +414,48 @@ int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* o
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const NlParams p = make_params(g, g_dev, phi_dev, out_dev);
     const int szj = g->Ns * g->Nz * g->J;
+    cudaEvent_t* ev = nullptr;
+    if (g->profile) {
+        if (g->ev_used + 4 > g->ev_pool.size()) {
+            const size_t old = g->ev_pool.size();
+            g->ev_pool.resize(old + 4 * 256);
+            for (size_t i = old; i < g->ev_pool.size(); ++i) GX_CUDA(g, cudaEventCreate(&g->ev_pool[i]));
+        }
+        ev = &g->ev_pool[g->ev_used];
+        g->ev_used += 4;
+        GX_CUDA(g, cudaEventRecord(ev[0], st));
+    }
     GX_CUDA(g, g->ks->launch_chi(p, szj, st));
+    if (ev) GX_CUDA(g, cudaEventRecord(ev[1], st));
     GX_CUDA(g, g->ks->launch_bracket(p, szj * g->Nm, st));
+    if (ev) GX_CUDA(g, cudaEventRecord(ev[2], st));
     dim3 grid((unsigned)((g->nk + 255) / 256), (unsigned)(g->Ns * g->Nm * g->Nz));
     if (g->Nl <= 4) gx::laguerre_inverse_kernel<4, 5><<<grid, 256, 0, st>>>(p, (int)g->nk);
     else if (g->Nl <= 8) gx::laguerre_inverse_kernel<8, 11><<<grid, 256, 0, st>>>(p, (int)g->nk);
     else gx::laguerre_inverse_kernel<16, 23><<<grid, 256, 0, st>>>(p, (int)g->nk);
     GX_CUDA(g, cudaGetLastError());
+    if (ev) GX_CUDA(g, cudaEventRecord(ev[3], st));
+    return GX_OK;
+}
+
+int gx_profile_set(gx_grid* g, int enabled) {
+    if (!g) return GX_ERR_ARG;
+    g->profile = enabled != 0;
+    return GX_OK;
+}
+
+int gx_profile_get(gx_grid* g, double* ms, long long* calls) {
+    if (!g || !ms || !calls) return GX_ERR_ARG;
+    *calls = (long long)(g->ev_used / 4);
+    for (size_t c = 0; c < g->ev_used; c += 4) {
+        GX_CUDA(g, cudaEventSynchronize(g->ev_pool[c + 3]));
+        for (int k = 0; k < 3; ++k) {
+            float t = 0.f;
+            GX_CUDA(g, cudaEventElapsedTime(&t, g->ev_pool[c + k], g->ev_pool[c + k + 1]));
+            ms[k] += t;
+        }
+    }
+    g->ev_used = 0;
     return GX_OK;
 }
 
