@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libgx.so")
+LIB_PATH = os.environ.get("GX_LIBRARY_PATH") or os.path.join(_HERE, "libgx.so")
 
 GX_OK, GX_ERR_ARG, GX_ERR_STATE, GX_ERR_UNSUPPORTED, GX_ERR_CUDA, GX_ERR_ALLOC = 0, -1, -2, -3, -4, -5
 (GX_Q_NAKX, GX_Q_NAKY, GX_Q_NJ, GX_Q_G_ELEMS, GX_Q_PHI_ELEMS, GX_Q_WORKSPACE_BYTES,

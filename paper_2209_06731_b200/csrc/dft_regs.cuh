@@ -59,17 +59,24 @@ template <int N, int S> __device__ __forceinline__ float2 twiddle(float2 v, int 
     return make_float2(fmaf(-v.y, s, v.x * c), fmaf(v.x, s, v.y * c));
 }
 
-template <int N, int S> struct Dft;
+// ZM: bit n set <=> input v[n] is known to be zero at compile time (2/3-rule padding).  The IEEE rules
+// forbid the compiler from folding x + 0 (sign of zero), so the base cases skip those adds explicitly;
+// a size that ignores ZM is still correct because the masked inputs really hold 0.
+template <int N, int S, unsigned ZM = 0u> struct Dft;
 
-template <int S> struct Dft<2, S> {
+__device__ __forceinline__ float2 cneg(float2 a) { return make_float2(-a.x, -a.y); }
+
+template <int S, unsigned ZM> struct Dft<2, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[2]) {
+        constexpr bool z0 = ZM & 1u, z1 = ZM & 2u;
         const float2 a = v[0], b = v[1];
-        v[0] = cadd(a, b);
-        v[1] = csub(a, b);
+        if constexpr (z1) { v[1] = a; }                       // (a, a); also covers both zero
+        else if constexpr (z0) { v[0] = b; v[1] = cneg(b); }
+        else { v[0] = cadd(a, b); v[1] = csub(a, b); }
     }
 };
 
-template <int S> struct Dft<3, S> {
+template <int S, unsigned ZM> struct Dft<3, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[3]) {
         const float2 t = cadd(v[1], v[2]);
         const float2 d = csub(v[1], v[2]);
@@ -82,54 +89,80 @@ template <int S> struct Dft<3, S> {
     }
 };
 
-template <int S> struct Dft<4, S> {
+template <int S, unsigned ZM> struct Dft<4, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[4]) {
-        const float2 a = cadd(v[0], v[2]), b = csub(v[0], v[2]);
-        const float2 c = cadd(v[1], v[3]), d = mul_i<S>(csub(v[1], v[3]));
-        v[0] = cadd(a, c);
-        v[1] = cadd(b, d);
-        v[2] = csub(a, c);
-        v[3] = csub(b, d);
+        constexpr bool z0 = ZM & 1u, z1 = ZM & 2u, z2 = ZM & 4u, z3 = ZM & 8u;
+        float2 a, b, c, d;                                    // a = v0+v2, b = v0-v2, c = v1+v3, d = v1-v3
+        if constexpr (z2) { a = v[0]; b = v[0]; }
+        else if constexpr (z0) { a = v[2]; b = cneg(v[2]); }
+        else { a = cadd(v[0], v[2]); b = csub(v[0], v[2]); }
+        if constexpr (z3) { c = v[1]; d = v[1]; }
+        else if constexpr (z1) { c = v[3]; d = cneg(v[3]); }
+        else { c = cadd(v[1], v[3]); d = csub(v[1], v[3]); }
+        d = mul_i<S>(d);
+        if constexpr (z1 && z3) { v[0] = a; v[1] = b; v[2] = a; v[3] = b; }
+        else if constexpr (z0 && z2) { v[0] = c; v[1] = d; v[2] = cneg(c); v[3] = cneg(d); }
+        else { v[0] = cadd(a, c); v[1] = cadd(b, d); v[2] = csub(a, c); v[3] = csub(b, d); }
     }
 };
 
 // One Cooley-Tukey split N = A*B:  n = n1*B + n2,  k = k1 + A*k2.
-template <int N, int A, int B, int S> __device__ __forceinline__ void dft_split(float2 (&v)[N]) {
+template <int A, int B, unsigned ZM, int n2> __host__ __device__ constexpr unsigned sub_mask_first() {
+    unsigned m = 0;
+    for (int n1 = 0; n1 < A; ++n1)
+        if (ZM & (1u << (n1 * B + n2))) m |= 1u << n1;
+    return m;
+}
+template <int A, int B, unsigned ZM> __host__ __device__ constexpr unsigned sub_mask_second() {   // column n2 entirely zero
+    unsigned m = 0;
+    for (int n2 = 0; n2 < B; ++n2) {
+        bool all = true;
+        for (int n1 = 0; n1 < A; ++n1)
+            if (!(ZM & (1u << (n1 * B + n2)))) all = false;
+        if (all) m |= 1u << n2;
+    }
+    return m;
+}
+
+template <int N, int A, int B, int S, unsigned ZM, int n2>
+__device__ __forceinline__ void dft_split_col(const float2 (&v)[N], float2 (&y)[N]) {
+    float2 t[A];
+#pragma unroll
+    for (int n1 = 0; n1 < A; ++n1) t[n1] = v[n1 * B + n2];
+    Dft<A, S, sub_mask_first<A, B, ZM, n2>()>::run(t);
+#pragma unroll
+    for (int k1 = 0; k1 < A; ++k1) y[k1 * B + n2] = twiddle<N, S>(t[k1], n2 * k1);
+    if constexpr (n2 + 1 < B) dft_split_col<N, A, B, S, ZM, n2 + 1>(v, y);
+}
+
+template <int N, int A, int B, int S, unsigned ZM = 0u> __device__ __forceinline__ void dft_split(float2 (&v)[N]) {
     static_assert(A * B == N, "bad split");
     float2 y[N];
-#pragma unroll
-    for (int n2 = 0; n2 < B; ++n2) {
-        float2 t[A];
-#pragma unroll
-        for (int n1 = 0; n1 < A; ++n1) t[n1] = v[n1 * B + n2];
-        Dft<A, S>::run(t);
-#pragma unroll
-        for (int k1 = 0; k1 < A; ++k1) y[k1 * B + n2] = twiddle<N, S>(t[k1], n2 * k1);
-    }
+    dft_split_col<N, A, B, S, ZM, 0>(v, y);
 #pragma unroll
     for (int k1 = 0; k1 < A; ++k1) {
         float2 u[B];
 #pragma unroll
         for (int n2 = 0; n2 < B; ++n2) u[n2] = y[k1 * B + n2];
-        Dft<B, S>::run(u);
+        Dft<B, S, sub_mask_second<A, B, ZM>()>::run(u);
 #pragma unroll
         for (int k2 = 0; k2 < B; ++k2) v[k1 + A * k2] = u[k2];
     }
 }
 
-template <int S> struct Dft<6, S> {
-    __device__ __forceinline__ static void run(float2 (&v)[6]) { dft_split<6, 2, 3, S>(v); }
+template <int S, unsigned ZM> struct Dft<6, S, ZM> {
+    __device__ __forceinline__ static void run(float2 (&v)[6]) { dft_split<6, 2, 3, S, ZM>(v); }
 };
-template <int S> struct Dft<8, S> {
-    __device__ __forceinline__ static void run(float2 (&v)[8]) { dft_split<8, 2, 4, S>(v); }
+template <int S, unsigned ZM> struct Dft<8, S, ZM> {
+    __device__ __forceinline__ static void run(float2 (&v)[8]) { dft_split<8, 2, 4, S, ZM>(v); }
 };
-template <int S> struct Dft<12, S> {
-    __device__ __forceinline__ static void run(float2 (&v)[12]) { dft_split<12, 3, 4, S>(v); }
+template <int S, unsigned ZM> struct Dft<12, S, ZM> {
+    __device__ __forceinline__ static void run(float2 (&v)[12]) { dft_split<12, 3, 4, S, ZM>(v); }
 };
-template <int S> struct Dft<16, S> {
-    __device__ __forceinline__ static void run(float2 (&v)[16]) { dft_split<16, 4, 4, S>(v); }
+template <int S, unsigned ZM> struct Dft<16, S, ZM> {
+    __device__ __forceinline__ static void run(float2 (&v)[16]) { dft_split<16, 4, 4, S, ZM>(v); }
 };
 
-template <int N, int S> __device__ __forceinline__ void dft(float2 (&v)[N]) { Dft<N, S>::run(v); }
+template <int N, int S, unsigned ZM = 0u> __device__ __forceinline__ void dft(float2 (&v)[N]) { Dft<N, S, ZM>::run(v); }
 
 }  // namespace gx

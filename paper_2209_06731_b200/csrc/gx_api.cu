@@ -40,6 +40,19 @@ template <class C> cudaError_t launch_chi_t(const NlParams& p, int units, cudaSt
     gx::chi_planes_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
     return cudaGetLastError();
 }
+// Launch with the programmatic-stream-serialization attribute (PDL): the grid may begin before the
+// previous kernel in the stream has finished; the kernel itself waits (griddepcontrol.wait) before it
+// reads that kernel's output.
+template <class... Args, class... Act>
+cudaError_t launch_pdl(void (*kernel)(Args...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Act... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
 template <class C> cudaError_t launch_bracket_t(const NlParams& p, int units, cudaStream_t st) {
     static bool attr = false;
     if (!attr) {
@@ -48,26 +61,42 @@ template <class C> cudaError_t launch_bracket_t(const NlParams& p, int units, cu
         if (e != cudaSuccess) return e;
         attr = true;
     }
-    gx::bracket_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
-    return cudaGetLastError();
+    return launch_pdl(gx::bracket_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
 }
-template <class C> constexpr KernelSet make_set() {
-    return KernelSet{C::NX, C::NY, C::SMEM_BYTES, &launch_chi_t<C>, &launch_bracket_t<C>};
+template <class CB, class CC> constexpr KernelSet make_set() {
+    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
+                  "chi and bracket kernels must share the transform radices (same permuted real-space order)");
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, &launch_chi_t<CC>, &launch_bracket_t<CB>};
 }
 
-//                         NX   NY  RX1 RX2 RY1 RY2  RB   NT MINB STAGE
-using Cfg16x16   = gx::PlaneCfg<16, 16, 4, 4, 4, 4, 16, 64, 1, true>;
-using Cfg64x64   = gx::PlaneCfg<64, 64, 8, 8, 8, 8, 64, 256, 2, true>;
-using Cfg128x64  = gx::PlaneCfg<128, 64, 16, 8, 8, 8, 64, 256, 2, true>;
-using Cfg192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, 64, 256, 2, true>;
-using Cfg256x64  = gx::PlaneCfg<256, 64, 16, 16, 8, 8, 64, 256, 1, true>;
-using Cfg256x96  = gx::PlaneCfg<256, 96, 16, 16, 8, 12, 64, 256, 1, true>;
-using Cfg192x192 = gx::PlaneCfg<192, 192, 16, 12, 12, 16, 16, 256, 1, false>;
-using Cfg64x192  = gx::PlaneCfg<64, 192, 8, 8, 12, 16, 32, 256, 1, true>;
+#ifndef GX_BR_NT
+#define GX_BR_NT 448
+#endif
+#ifndef GX_BR_MINB
+#define GX_BR_MINB 2
+#endif
+#ifndef GX_CHI_NT
+#define GX_CHI_NT 512
+#endif
+#ifndef GX_BR_RB
+#define GX_BR_RB 64
+#endif
+//                  NX   NY  RX1 RX2 RY1 RY2  RB   NT MINB STAGE     (B = bracket kernel, C = chi kernel)
+using B16x16   = gx::PlaneCfg<16, 16, 4, 4, 4, 4, 16, 64, 1, true>;
+using B64x64   = gx::PlaneCfg<64, 64, 8, 8, 8, 8, 64, 256, 2, true>;
+using B128x64  = gx::PlaneCfg<128, 64, 16, 8, 8, 8, 64, GX_BR_NT, GX_BR_MINB, true>;
+using C128x64  = gx::PlaneCfg<128, 64, 16, 8, 8, 8, 64, GX_CHI_NT, 1, true>;
+using B192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, GX_BR_RB, GX_BR_NT, GX_BR_MINB, true>;
+using C192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, 64, GX_CHI_NT, 1, true>;
+using B256x64  = gx::PlaneCfg<256, 64, 16, 16, 8, 8, 64, 256, 1, true>;
+using B256x96  = gx::PlaneCfg<256, 96, 16, 16, 8, 12, 64, 256, 1, true>;
+using B192x192 = gx::PlaneCfg<192, 192, 16, 12, 12, 16, 16, 256, 1, false>;
+using B64x192  = gx::PlaneCfg<64, 192, 8, 8, 12, 16, 32, 256, 1, true>;
 
 const KernelSet kKernelSets[] = {
-    make_set<Cfg16x16>(),  make_set<Cfg64x64>(),  make_set<Cfg128x64>(),  make_set<Cfg192x64>(),
-    make_set<Cfg256x64>(), make_set<Cfg256x96>(), make_set<Cfg192x192>(), make_set<Cfg64x192>(),
+    make_set<B16x16, B16x16>(),   make_set<B64x64, B64x64>(),     make_set<B128x64, C128x64>(),
+    make_set<B192x64, C192x64>(), make_set<B256x64, B256x64>(),   make_set<B256x96, B256x96>(),
+    make_set<B192x192, B192x192>(), make_set<B64x192, B64x192>(),
 };
 
 const KernelSet* find_set(int Nx, int Ny) {
@@ -145,6 +174,8 @@ struct gx_grid {
     // device
     float *dT = nullptr, *dTinv = nullptr, *dM = nullptr;
     float2 *dtwx = nullptr, *dtwy = nullptr, *ddchi = nullptr, *dbhat = nullptr;
+    unsigned* dcount = nullptr;
+    unsigned calls = 0;                         // number of gx_nonlinear_rhs calls issued (counter epoch)
     float2 *dgbuf = nullptr, *dphibuf = nullptr, *doutbuf = nullptr;   // for the *_host entry point
     gx::LinTables lin;                                                  // linear-term tables
     float2* dphi_rhs = nullptr;                                         // phi of gx_rhs
@@ -195,6 +226,7 @@ NlParams make_params(gx_grid* g, const void* gd, const void* phid, void* outd) {
     p.M = g->dM;
     p.T = g->dT;
     p.Tinv = g->dTinv;
+    p.count = g->dcount;
     p.twx = g->dtwx;
     p.twy = g->dtwy;
     p.dkx = (float)g->dkx;
@@ -275,13 +307,15 @@ int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out
     if ((rc = dev_alloc(g, &g->dM, szj * g->nk))) return rc;
     if ((rc = dev_alloc(g, &g->ddchi, szj * Nx * Ny))) return rc;
     if ((rc = dev_alloc(g, &g->dbhat, szj * Nm * g->nk))) return rc;
+    if ((rc = dev_alloc(g, &g->dcount, (size_t)Ns * Nm * Nz))) return rc;
+    GX_CUDA(g, cudaMemset(g->dcount, 0, (size_t)Ns * Nm * Nz * sizeof(unsigned)));
     return GX_OK;
 }
 
 int gx_grid_destroy(gx_grid* g) {
     if (!g) return GX_ERR_ARG;
     cudaFree(g->dT); cudaFree(g->dTinv); cudaFree(g->dM); cudaFree(g->dtwx); cudaFree(g->dtwy);
-    cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
+    cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dcount); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
     cudaFree(g->dphi_rhs);
     for (auto e : g->ev_pool) cudaEventDestroy(e);
     gx::lin_tables_free(g->lin);
@@ -429,11 +463,23 @@ int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* o
     if (ev) GX_CUDA(g, cudaEventRecord(ev[1], st));
     GX_CUDA(g, g->ks->launch_bracket(p, szj * g->Nm, st));
     if (ev) GX_CUDA(g, cudaEventRecord(ev[2], st));
-    dim3 grid((unsigned)((g->nk + 255) / 256), (unsigned)(g->Ns * g->Nm * g->Nz));
-    if (g->Nl <= 4) gx::laguerre_inverse_kernel<4, 5><<<grid, 256, 0, st>>>(p, (int)g->nk);
-    else if (g->Nl <= 8) gx::laguerre_inverse_kernel<8, 11><<<grid, 256, 0, st>>>(p, (int)g->nk);
-    else gx::laguerre_inverse_kernel<16, 23><<<grid, 256, 0, st>>>(p, (int)g->nk);
-    GX_CUDA(g, cudaGetLastError());
+    {
+        const int vec = (g->nk % 2 == 0) ? 2 : 1;
+        const int nkv = (int)(g->nk / vec);
+        dim3 grid((unsigned)((nkv + 255) / 256), (unsigned)(g->Ns * g->Nm * g->Nz));
+        const int nk = (int)g->nk;
+        g->calls += 1;
+        const unsigned target = g->calls * (unsigned)g->J;
+        cudaError_t e;
+#define GX_LAGINV(L, J)                                                                                        \
+    e = (vec == 2) ? launch_pdl(gx::laguerre_inverse_kernel<L, J, 2>, grid, dim3(256), 0, st, p, nk, target)  \
+                   : launch_pdl(gx::laguerre_inverse_kernel<L, J, 1>, grid, dim3(256), 0, st, p, nk, target)
+        if (g->Nl <= 4) GX_LAGINV(4, 5);
+        else if (g->Nl <= 8) GX_LAGINV(8, 11);
+        else GX_LAGINV(16, 23);
+#undef GX_LAGINV
+        GX_CUDA(g, e);
+    }
     if (ev) GX_CUDA(g, cudaEventRecord(ev[3], st));
     return GX_OK;
 }

@@ -8,7 +8,7 @@
 //   bracket_kernel      unit (s,m,z,j):  gt = sum_l T[j][l] G_l (a2) -> (i kx, i ky) (a3) -> inverse 2D FFT
 //                                        (a4) -> bracket with the chi pairs (a5) -> forward 2D FFT (a6)
 //                                        -> 2/3-rule truncation (a7) -> Bhat_j(k) in the workspace
-//   laguerre_inverse_kernel  (s,m,z):    out_l = - sum_j Tinv[l][j] Bhat_j (a8)
+//   laguerre_inverse_kernel  (s,m,z):    out_l = - sum_j Tinv[l][j] Bhat_j (a8), overlapping the bracket tail
 //
 // FFT design (differs from the paper's cuFFT calls):
 //  * The two real fields d_x f and d_y f are transformed as ONE complex field
@@ -26,6 +26,8 @@
 //  * The y transforms run on batches of RB x-rows through a scratch tile S[y][row]; lanes map to
 //    rows, so every shared access is either contiguous or has the odd stride 2*naky-1.
 #pragma once
+#include <type_traits>
+
 #include "dft_regs.cuh"
 
 namespace gx {
@@ -41,6 +43,14 @@ struct PlaneCfg {
     static constexpr int W_ELEMS = NX * NCOL;
     static constexpr int S_ELEMS = (STAGE && NK > NY * RB) ? NK : NY * RB;
     static constexpr int SMEM_BYTES = (W_ELEMS + S_ELEMS + NX + NY) * (int)sizeof(float2);
+    // compile-time zero masks of the first inverse passes: input n = n1*R2 + n2 is padding for every n2
+    static constexpr unsigned zero_mask(int R1, int R2, int N, int KK) {
+        unsigned m = 0;
+        for (int n1 = 0; n1 < R1; ++n1)
+            if (!(n1 * R2 <= KK || n1 * R2 + R2 - 1 >= N - KK)) m |= 1u << n1;
+        return m;
+    }
+    static constexpr unsigned ZMX = zero_mask(RX1, RX2, NX, K), ZMY = zero_mask(RY1, RY2, NY, Q);
     static_assert(RX1 * RX2 == NX && RY1 * RY2 == NY, "radix split");
     static_assert(NX % RB == 0 && RB % 2 == 0 && NX % 2 == 0, "row batches");
     static_assert(SMEM_BYTES <= 232448, "plane does not fit in shared memory");
@@ -55,6 +65,7 @@ struct NlParams {
     const float* M;       // [s][z][j][kx][ky]
     const float* T;       // [j][l]
     const float* Tinv;    // [l][j]
+    unsigned* count;      // [s][m][z] arrival counters of the J node-units (monotonic: +J per call)
     const float2* twx;    // e^{+2 pi i t/NX}
     const float2* twy;
     float dkx, dky, scale;
@@ -63,39 +74,62 @@ struct NlParams {
 
 // ------------------------------------------------------------------------------------------------
 // inverse x transform of U(k) = (i kx - ky) f(k) on the 2*naky-1 non-zero columns.
-// fetch(i, q): compact f at kx row i, ky column q >= 0.
-template <class C, class Fetch>
+// F: compact f, [NAKX][NAKY], in shared memory (STAGE) or global memory.
+// Element classes of input n = n1*R2 + n2 are resolved at compile time per n1: always kept with
+// kx >= 0, always kept with kx < 0, always padding, or decided by n2 at run time (at most two n1).
+// For column q < 0 the reality condition gives f(a,q) = conj f(-a,-q): row index and the sign of the
+// imaginary part flip, which keeps every address of the form base + compile-time offset.
+template <class C, bool GLOBAL_F>
 __device__ __forceinline__ void x_inverse(float2* __restrict__ W, const float2* __restrict__ twx,
-                                          float dkx, float dky, Fetch fetch) {
+                                          float dkx, float dky, const float2* __restrict__ F) {
     constexpr int NX = C::NX, K = C::K, NCOL = C::NCOL, NAKY = C::NAKY, NAKX = C::NAKX;
     constexpr int R1 = C::RX1, R2 = C::RX2;
     // pass 1: for each (n2, column): DFT_R1 over n1 of input n = n1*R2+n2, twiddle, in-place slot
     for (int t = threadIdx.x; t < R2 * NCOL; t += C::NT) {
         const int n2 = t / NCOL, c = t - n2 * NCOL;
-        const int q = c < NAKY ? c : c - NCOL;
-        const int qa = q < 0 ? -q : q;
-        const float kyq = dky * (float)q;
+        const bool neg = c >= NAKY;                       // column q < 0
+        const int qa = neg ? NCOL - c : c;                // |q|
+        const float kyq = neg ? -dky * (float)qa : dky * (float)qa;
+        const float sgn = neg ? -1.f : 1.f;               // conj for q < 0
+        // compact row of mode a (or of -a when q < 0), as base + n1 * step
+        //   kx >= 0 branch, a = n:        q>=0: row  n            q<0: row NAKX - n   (n = 0 -> row 0)
+        //   kx <  0 branch, a = n - NX:   q>=0: row  n - NX + NAKX  q<0: row NX - n
+        const int stepP = neg ? -R2 * NAKY : R2 * NAKY;
+        const float2* __restrict__ FP = F + (neg ? (NAKX - n2) * NAKY : n2 * NAKY) + qa;
+        const float2* __restrict__ FN = F + (neg ? (NX - n2) * NAKY : (n2 - NX + NAKX) * NAKY) + qa;
+        const float an2 = (float)n2, an2n = (float)(n2 - NX);   // integers: sums below are exact in fp32
         float2 v[R1];
 #pragma unroll
         for (int n1 = 0; n1 < R1; ++n1) {
-            const int n = n1 * R2 + n2;
+            const int lo = n1 * R2, hi = n1 * R2 + R2 - 1;           // range of n over n2 (compile time)
+            const bool allP = hi <= K, someP = lo <= K;              // kept with kx >= 0
+            const bool allN = lo >= NX - K, someN = hi >= NX - K;    // kept with kx < 0
             v[n1] = make_float2(0.f, 0.f);
-            if (n1 * R2 <= K || n1 * R2 + R2 - 1 >= NX - K) {        // compile-time prune of all-zero n1
-                int a = 0;
-                bool nz = false;
-                if (n <= K) { a = n; nz = true; }
-                else if (n >= NX - K) { a = n - NX; nz = true; }
-                if (nz) {
-                    const int as = q >= 0 ? a : -a;
-                    const int i = as >= 0 ? as : as + NAKX;
-                    float2 f = fetch(i, qa);
-                    if (q < 0) f.y = -f.y;
-                    const float kxa = dkx * (float)a;
-                    v[n1] = make_float2(-kyq * f.x - kxa * f.y, kxa * f.x - kyq * f.y);
+            if (someP || someN) {
+                float2 f = make_float2(0.f, 0.f);
+                float kxa = 0.f;
+                if (someP) {
+                    const bool isP = allP || (lo + n2 <= K);
+                    const float2* ptr = FP + n1 * stepP;
+                    if (n1 == 0 && neg && n2 == 0) ptr = F + qa;     // mode a = 0: -a is row 0, not NAKX
+                    if (isP) {
+                        f = GLOBAL_F ? __ldg(ptr) : *ptr;
+                        kxa = dkx * (an2 + (float)lo);
+                    }
                 }
+                if (someN) {
+                    const bool isN = allN || (lo + n2 >= NX - K);
+                    if (isN) {
+                        const float2* ptr = FN + n1 * stepP;
+                        f = GLOBAL_F ? __ldg(ptr) : *ptr;
+                        kxa = dkx * (an2n + (float)lo);
+                    }
+                }
+                const float fy = sgn * f.y;
+                v[n1] = make_float2(fmaf(-kyq, f.x, -kxa * fy), fmaf(kxa, f.x, -kyq * fy));
             }
         }
-        dft<R1, +1>(v);
+        dft<R1, +1, C::ZMX>(v);
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1)
             W[(k1 * R2 + n2) * NCOL + c] = k1 == 0 ? v[0] : cmul(v[k1], twx[n2 * k1]);
@@ -114,6 +148,13 @@ __device__ __forceinline__ void x_inverse(float2* __restrict__ W, const float2* 
     __syncthreads();
 }
 
+template <class C>
+__device__ __forceinline__ void x_inverse_global_rw(float2* __restrict__ W, const float2* __restrict__ twx,
+                                                    float dkx, float dky, const float2* F) {
+    __threadfence_block();
+    x_inverse<C, false>(W, twx, dkx, dky, F);        // plain ld: data was written by this CTA
+}
+
 // y inverse pass 1 for a batch of RB rows: W rows (2*naky-1 non-zero inputs) -> S[(k1*RY2+n2)*RB + r]
 template <class C, bool PAIRED>
 __device__ __forceinline__ void y_inverse_pass1(const float2* __restrict__ W, float2* __restrict__ S,
@@ -124,17 +165,18 @@ __device__ __forceinline__ void y_inverse_pass1(const float2* __restrict__ W, fl
         const int n2 = t / RB, r = t - n2 * RB;
         const int row = PAIRED ? (r < HB ? bt * HB + r : bt * HB + (r - HB) + NX / 2) : bt * RB + r;
         const float2* __restrict__ Wr = W + row * NCOL;
+        const float2* __restrict__ WP = Wr + n2;                  // ky >= 0: column n
+        const float2* __restrict__ WN = Wr + n2 - NY + NCOL;      // ky <  0: column n - NY + NCOL
         float2 v[R1];
 #pragma unroll
         for (int n1 = 0; n1 < R1; ++n1) {
-            const int n = n1 * R2 + n2;
+            const int lo = n1 * R2, hi = n1 * R2 + R2 - 1;
+            const bool allP = hi <= Q, someP = lo <= Q, allN = lo >= NY - Q, someN = hi >= NY - Q;
             v[n1] = make_float2(0.f, 0.f);
-            if (n1 * R2 <= Q || n1 * R2 + R2 - 1 >= NY - Q) {
-                if (n <= Q) v[n1] = Wr[n];
-                else if (n >= NY - Q) v[n1] = Wr[n - NY + NCOL];
-            }
+            if (someP && (allP || lo + n2 <= Q)) v[n1] = WP[lo];
+            if (someN && (allN || lo + n2 >= NY - Q)) v[n1] = WN[lo];
         }
-        dft<R1, +1>(v);
+        dft<R1, +1, C::ZMY>(v);
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1)
             S[(k1 * R2 + n2) * RB + r] = k1 == 0 ? v[0] : cmul(v[k1], twy[n2 * k1]);
@@ -179,6 +221,119 @@ __device__ __forceinline__ void x_forward(float2* __restrict__ W, const float2* 
     }
 }
 
+// Programmatic dependent launch (sm_90+): the dependent grid may start while the primary still runs;
+// it must not touch the primary's output before pdl_wait().  Both are no-ops without the launch attribute.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+
+// S[i] = sum_l coef[l] * planes[l*lstride + i], i < NK: 4 positions x 4 planes = 16 independent 8-byte
+// loads in flight per thread (the loop is latency-bound otherwise: ncu r01 showed 35% of the bracket
+// kernel's stall samples here).
+template <class C>
+__device__ __forceinline__ void stage_combine(float2* __restrict__ S, const float2* __restrict__ planes,
+                                              size_t lstride, const float* __restrict__ coef, int Nl) {
+    constexpr int NK = C::NK, NT = C::NT, U = 4;
+    for (int i0 = threadIdx.x; i0 < NK; i0 += U * NT) {
+        float2 acc[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) acc[u] = make_float2(0.f, 0.f);
+        for (int l0 = 0; l0 < Nl; l0 += 4) {
+            float2 f[4][U];
+#pragma unroll
+            for (int dl = 0; dl < 4; ++dl)
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const int i = i0 + u * NT;
+                    f[dl][u] = (l0 + dl < Nl && i < NK) ? __ldg(planes + (size_t)(l0 + dl) * lstride + i)
+                                                        : make_float2(0.f, 0.f);
+                }
+#pragma unroll
+            for (int dl = 0; dl < 4; ++dl) {
+                const float t = (l0 + dl < Nl) ? __ldg(coef + l0 + dl) : 0.f;
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    acc[u].x = fmaf(t, f[dl][u].x, acc[u].x);
+                    acc[u].y = fmaf(t, f[dl][u].y, acc[u].y);
+                }
+            }
+        }
+#pragma unroll
+        for (int u = 0; u < U; ++u)
+            if (i0 + u * NT < NK) S[i0 + u * NT] = acc[u];
+    }
+}
+
+// ---- TMA bulk staging (cp.async.bulk + mbarrier): the Nl compact planes of one (s,m,z) are contiguous
+// 16-byte aligned chunks of NK*8 bytes; one elected thread copies them into the (still unused) W+S region,
+// everyone waits on the mbarrier, combines them with the Laguerre row T[j][.] in registers and, after a
+// barrier, writes gt into S.  No per-element global load instruction or address arithmetic is issued.
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_%=:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra DONE_%=;\n\t"
+        "bra WAIT_%=;\n\t"
+        "DONE_%=:\n\t}" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+template <class C>
+__device__ __forceinline__ void stage_combine_tma(float2* __restrict__ raw, float2* __restrict__ S,
+                                                  unsigned long long* bar, unsigned& parity,
+                                                  const float2* __restrict__ planes,
+                                                  size_t lstride, const float* __restrict__ coef, int Nl) {
+    constexpr int NK = C::NK, NT = C::NT, NK2 = NK / 2;
+    constexpr int CAP = (C::W_ELEMS + C::S_ELEMS) / NK;          // planes per chunk
+    constexpr int PER = (NK2 + NT - 1) / NT;                     // float4 (2 complex) per thread
+    static_assert(CAP >= 1 && NK % 2 == 0, "TMA staging needs 16-byte planes that fit");
+    const float4* __restrict__ raw4 = reinterpret_cast<const float4*>(raw) + threadIdx.x;
+    float4 acc[PER];
+#pragma unroll
+    for (int u = 0; u < PER; ++u) acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
+    for (int l0 = 0; l0 < Nl; l0 += CAP) {
+        const int nl = min(CAP, Nl - l0);
+        if (threadIdx.x == 0) {
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_expect_tx(bar, (unsigned)(nl * NK * sizeof(float2)));
+            for (int l = 0; l < nl; ++l)
+                bulk_g2s(raw + l * NK, planes + (size_t)(l0 + l) * lstride, NK * sizeof(float2), bar);
+        }
+        mbar_wait(bar, parity);
+        parity ^= 1u;
+        for (int l = 0; l < nl; ++l) {
+            const float t = coef[l0 + l];
+            const float4* __restrict__ src = raw4 + l * NK2;
+#pragma unroll
+            for (int u = 0; u < PER; ++u) {
+                if ((u + 1) * NT <= NK2 || (int)threadIdx.x + u * NT < NK2) {
+                    const float4 f = src[u * NT];
+                    acc[u].x = fmaf(t, f.x, acc[u].x);
+                    acc[u].y = fmaf(t, f.y, acc[u].y);
+                    acc[u].z = fmaf(t, f.z, acc[u].z);
+                    acc[u].w = fmaf(t, f.w, acc[u].w);
+                }
+            }
+        }
+        __syncthreads();                                         // raw region consumed
+    }
+    float4* __restrict__ S4 = reinterpret_cast<float4*>(S) + threadIdx.x;
+#pragma unroll
+    for (int u = 0; u < PER; ++u)
+        if ((u + 1) * NT <= NK2 || (int)threadIdx.x + u * NT < NK2) S4[u * NT] = acc[u];
+}
+
 template <class C>
 __device__ __forceinline__ void load_twiddles(float2* twx_s, float2* twy_s, const NlParams& p) {
     for (int i = threadIdx.x; i < C::NX; i += C::NT) twx_s[i] = p.twx[i];
@@ -198,22 +353,35 @@ __global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_kernel(const NlPara
     const int z = (unit / p.J) % p.Nz;
     const float2* __restrict__ phi = p.phi + (size_t)z * C::NK;
     const float* __restrict__ M = p.M + (size_t)unit * C::NK;
+    pdl_launch_dependents();        // the bracket kernel's prologue (a2-a4 x part) does not read dchi
     load_twiddles<C>(twx, twy, p);
     if constexpr (C::STAGE) {
-        for (int i = threadIdx.x; i < C::NK; i += C::NT) {
-            const float2 f = phi[i];
-            const float m = M[i];
-            S[i] = make_float2(f.x * m, f.y * m);
+        constexpr int U = 4;
+        for (int i0 = threadIdx.x; i0 < C::NK; i0 += U * C::NT) {
+            float2 f[U];
+            float m[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                const int i = i0 + u * C::NT;
+                f[u] = i < C::NK ? __ldg(phi + i) : make_float2(0.f, 0.f);
+                m[u] = i < C::NK ? __ldg(M + i) : 0.f;
+            }
+#pragma unroll
+            for (int u = 0; u < U; ++u)
+                if (i0 + u * C::NT < C::NK) S[i0 + u * C::NT] = make_float2(f[u].x * m[u], f[u].y * m[u]);
         }
         __syncthreads();
-        x_inverse<C>(W, twx, p.dkx, p.dky, [&](int i, int q) { return S[i * C::NAKY + q]; });
+        x_inverse<C, false>(W, twx, p.dkx, p.dky, S);
     } else {
+        // plane too large to stage: chi = M.Phi goes through this unit's own (not yet written) dchi slot
+        float2* __restrict__ tmp = p.dchi + (size_t)unit * C::NX * C::NY;
+        for (int i = threadIdx.x; i < C::NK; i += C::NT) {
+            const float2 f = __ldg(phi + i);
+            const float m = __ldg(M + i);
+            tmp[i] = make_float2(f.x * m, f.y * m);
+        }
         __syncthreads();
-        x_inverse<C>(W, twx, p.dkx, p.dky, [&](int i, int q) {
-            const float2 f = __ldg(phi + i * C::NAKY + q);
-            const float m = __ldg(M + i * C::NAKY + q);
-            return make_float2(f.x * m, f.y * m);
-        });
+        x_inverse_global_rw<C>(W, twx, p.dkx, p.dky, tmp);
     }
     float2* __restrict__ dchi = p.dchi + (size_t)unit * C::NX * C::NY;
     constexpr int R1 = C::RY1, R2 = C::RY2, RB = C::RB;
@@ -254,37 +422,33 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
     const float2* __restrict__ g0 = p.g + ((size_t)(s * p.Nm + m) * p.Nl * p.Nz + z) * NK;
     const float* __restrict__ Tj = p.T + j * p.Nl;
 
+    __shared__ unsigned long long stage_bar;
+    __shared__ float Tsh[16];
+    unsigned bar_parity = 0;
+    if constexpr (C::STAGE && C::NK % 2 == 0) {
+        if (threadIdx.x == 0) mbar_init(&stage_bar, 1);
+        if (threadIdx.x < p.Nl) Tsh[threadIdx.x] = __ldg(Tj + threadIdx.x);
+        __syncthreads();
+    }
+    pdl_launch_dependents();        // inverse-Laguerre grid may become resident once our last wave runs
     load_twiddles<C>(twx, twy, p);
     // ---- a2: forward Laguerre transform l -> node j, fused into the load
     if constexpr (C::STAGE) {
-        for (int i = threadIdx.x; i < NK; i += C::NT) {
-            float2 acc = make_float2(0.f, 0.f);
-            for (int l = 0; l < p.Nl; ++l) {
-                const float tl = __ldg(Tj + l);
-                const float2 f = g0[(size_t)l * lstride + i];
-                acc.x = fmaf(tl, f.x, acc.x);
-                acc.y = fmaf(tl, f.y, acc.y);
-            }
-            S[i] = acc;
-        }
+        if constexpr (C::NK % 2 == 0) stage_combine_tma<C>(W, S, &stage_bar, bar_parity, g0, lstride, Tsh, p.Nl);
+        else stage_combine<C>(S, g0, lstride, Tj, p.Nl);
         __syncthreads();
-        x_inverse<C>(W, twx, p.dkx, p.dky, [&](int i, int q) { return S[i * C::NAKY + q]; });
+        x_inverse<C, false>(W, twx, p.dkx, p.dky, S);
     } else {
+        // plane too large to stage in shared memory: gt goes through this unit's own bhat slot
+        // (written by this CTA, read back by this CTA after the barrier; overwritten by the result later)
+        float2* __restrict__ tmp = p.bhat + (size_t)unit * NK;
+        stage_combine<C>(tmp, g0, lstride, Tj, p.Nl);
         __syncthreads();
-        const int Nl = p.Nl;
-        x_inverse<C>(W, twx, p.dkx, p.dky, [&](int i, int q) {
-            float2 acc = make_float2(0.f, 0.f);
-            for (int l = 0; l < Nl; ++l) {
-                const float tl = __ldg(Tj + l);
-                const float2 f = __ldg(g0 + (size_t)l * lstride + i * C::NAKY + q);
-                acc.x = fmaf(tl, f.x, acc.x);
-                acc.y = fmaf(tl, f.y, acc.y);
-            }
-            return acc;
-        });
+        x_inverse_global_rw<C>(W, twx, p.dkx, p.dky, tmp);
     }
 
     const float2* __restrict__ dchi = p.dchi + (size_t)szj * NX * NY;
+    pdl_wait();                     // chi planes of this call are complete and visible from here on
     for (int bt = 0; bt < C::NBATCH; ++bt) {
         // ---- a4 (y part): rows p and p+NX/2 of the batch
         y_inverse_pass1<C, true>(W, S, twy, bt);
@@ -302,7 +466,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
                 dft<R2, +1>(v);
 #pragma unroll
                 for (int k2 = 0; k2 < R2; ++k2) {
-                    const float2 d = __ldg(dchi + (size_t)(k1 * R2 + k2) * NX + row);
+                    const float2 d = dchi[(size_t)(k1 * R2 + k2) * NX + row];
                     const float b = fmaf(d.y, v[k2].x, -d.x * v[k2].y);   // d_y chi d_x g - d_x chi d_y g
                     if (h == 0) c[k2].x = b; else c[k2].y = b;
                 }
@@ -358,37 +522,58 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
     }
     // ---- a6 (x part) + a7 (keep |kx| <= K)
     x_forward<C>(W, twx, p.bhat + (size_t)unit * NK, p.scale);
+
+    // ---- publish: this node's Bhat plane is complete (release: stores -> fence -> barrier -> atomic).
+    // The inverse-Laguerre grid, already resident under PDL, waits per (s,m,z) on this counter.
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x == 0) atomicAdd(p.count + (s * p.Nm + m) * p.Nz + z, 1u);
 }
 
 // ================================================================================================
-// a8: out[s,m,l,z,k] = - sum_j Tinv[l][j] Bhat[s,z,j,m,k]
-template <int MAXL, int MAXJ>
-__global__ void __launch_bounds__(256) laguerre_inverse_kernel(const NlParams p, int nk) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    const int smz = blockIdx.y;                   // (s*Nm + m)*Nz + z
+// a8: out[s,m,l,z,k] = - sum_j Tinv[l][j] Bhat[s,z,j,m,k].  VEC = 2 complex per thread (16-byte accesses)
+// when nk is even, else 1.  Launched with PDL: blocks become resident during the bracket kernel's last
+// wave and wait until the J node-units of their (s,m,z) have arrived (count >= target; the counters
+// grow by J per call, target = J * call number, so nothing is ever reset).
+template <int MAXL, int MAXJ, int VEC>
+__global__ void __launch_bounds__(256) laguerre_inverse_kernel(const NlParams p, int nk, unsigned target) {
+    using V = typename std::conditional<VEC == 2, float4, float2>::type;
+    const int kv = blockIdx.x * blockDim.x + threadIdx.x;      // index in units of VEC complex
+    const int smz = blockIdx.y;                                 // (s*Nm + m)*Nz + z
     const int z = smz % p.Nz;
     const int m = (smz / p.Nz) % p.Nm;
     const int s = smz / (p.Nz * p.Nm);
     __shared__ float Ti[MAXL * MAXJ];
-    for (int i = threadIdx.x; i < p.Nl * p.J; i += blockDim.x) Ti[i] = p.Tinv[i];
+    for (int i = threadIdx.x; i < p.Nl * p.J; i += blockDim.x) Ti[i] = -__ldg(p.Tinv + i);   // out = -N
+    if (threadIdx.x == 0) {
+        const volatile unsigned* c = p.count + smz;
+        while ((int)(*c - target) < 0) __nanosleep(200);
+        __threadfence();
+    }
     __syncthreads();
-    if (k >= nk) return;
-    float2 b[MAXJ];
+    const int nkv = nk / VEC;
+    if (kv >= nkv) return;
+    V b[MAXJ];
 #pragma unroll
     for (int j = 0; j < MAXJ; ++j)
-        if (j < p.J) b[j] = p.bhat[((size_t)((s * p.Nz + z) * p.J + j) * p.Nm + m) * nk + k];
+        if (j < p.J)
+            b[j] = __ldcg(reinterpret_cast<const V*>(p.bhat + ((size_t)((s * p.Nz + z) * p.J + j) * p.Nm + m) * nk) + kv);
 #pragma unroll
     for (int l = 0; l < MAXL; ++l) {
         if (l < p.Nl) {
-            float2 acc = make_float2(0.f, 0.f);
+            float acc[2 * VEC];
+#pragma unroll
+            for (int c = 0; c < 2 * VEC; ++c) acc[c] = 0.f;
 #pragma unroll
             for (int j = 0; j < MAXJ; ++j)
                 if (j < p.J) {
                     const float t = Ti[l * p.J + j];
-                    acc.x = fmaf(-t, b[j].x, acc.x);
-                    acc.y = fmaf(-t, b[j].y, acc.y);
+                    const float* bj = reinterpret_cast<const float*>(&b[j]);
+#pragma unroll
+                    for (int c = 0; c < 2 * VEC; ++c) acc[c] = fmaf(t, bj[c], acc[c]);
                 }
-            p.out[(((size_t)(s * p.Nm + m) * p.Nl + l) * p.Nz + z) * nk + k] = acc;
+            V* dst = reinterpret_cast<V*>(p.out + (((size_t)(s * p.Nm + m) * p.Nl + l) * p.Nz + z) * nk) + kv;
+            *dst = *reinterpret_cast<V*>(acc);
         }
     }
 }
