@@ -4,6 +4,7 @@
 
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -11,6 +12,7 @@
 #include "../../include/gx.h"
 #include "linear_kernels.cuh"
 #include "nl_kernels.cuh"
+#include "nl_pair_kernels.cuh"
 
 namespace {
 
@@ -25,6 +27,7 @@ struct Species {
 struct KernelSet {
     int Nx, Ny;
     int smem_bytes;
+    int max_nl;          // 0: any Nl; else the set needs Nl <= max_nl (all Laguerre planes staged at once)
     cudaError_t (*launch_chi)(const NlParams&, int units, cudaStream_t);
     cudaError_t (*launch_bracket)(const NlParams&, int units, cudaStream_t);
 };
@@ -63,10 +66,61 @@ template <class C> cudaError_t launch_bracket_t(const NlParams& p, int units, cu
     }
     return launch_pdl(gx::bracket_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
 }
+template <class C> cudaError_t launch_chi_pair_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_pair_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    gx::chi_planes_pair_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
+    return cudaGetLastError();
+}
+template <class C> cudaError_t launch_bracket_pair_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::bracket_pair_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    return launch_pdl(gx::bracket_pair_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
+}
+int sm_count() {
+    static int n = 0;
+    if (!n) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
+    }
+    return n;
+}
+template <class C> cudaError_t launch_bracket_persist_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::bracket_persist_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    const int grid = units < sm_count() ? units : sm_count();
+    return launch_pdl(gx::bracket_persist_kernel<C>, dim3(grid), dim3(C::NT), C::SMEM_BYTES, st, p, units);
+}
+template <class CB, class CC> constexpr KernelSet make_persist_set() {
+    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
+                  "chi and bracket kernels must share the transform radices (same permuted real-space order)");
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, CB::MAXL, &launch_chi_pair_t<CC>, &launch_bracket_persist_t<CB>};
+}
+template <class CB, class CC> constexpr KernelSet make_pair_set() {
+    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
+                  "chi and bracket kernels must share the transform radices (same permuted real-space order)");
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, &launch_chi_pair_t<CC>, &launch_bracket_pair_t<CB>};
+}
 template <class CB, class CC> constexpr KernelSet make_set() {
     static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
                   "chi and bracket kernels must share the transform radices (same permuted real-space order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, &launch_chi_t<CC>, &launch_bracket_t<CB>};
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, &launch_chi_t<CC>, &launch_bracket_t<CB>};
 }
 
 #ifndef GX_BR_NT
@@ -99,7 +153,49 @@ const KernelSet kKernelSets[] = {
     make_set<B192x192, B192x192>(), make_set<B64x192, B64x192>(),
 };
 
-const KernelSet* find_set(int Nx, int Ny) {
+// packed-FP32 family (nl_pair_kernels.cuh): preferred when an instantiation exists
+#ifndef GX_PB_NT
+#define GX_PB_NT 256
+#endif
+#ifndef GX_PC_NT
+#define GX_PC_NT 256
+#endif
+//                   NX   NY  RX1 RX2 RY1 RY2  RB   NT MINB
+using P16x16   = gx::PairCfg<16, 16, 4, 4, 4, 4, 16, 64, 1>;
+using P64x64   = gx::PairCfg<64, 64, 8, 8, 8, 8, 64, 128, 2>;
+using P128x64  = gx::PairCfg<128, 64, 16, 8, 8, 8, 64, GX_PB_NT, 2>;
+using P192x64  = gx::PairCfg<192, 64, 16, 12, 8, 8, 64, GX_PB_NT, 2>;
+using PC192x64 = gx::PairCfg<192, 64, 16, 12, 8, 8, 64, GX_PC_NT, 1>;
+using P256x96  = gx::PairCfg<256, 96, 16, 16, 8, 12, 32, 256, 1>;
+using P64x192  = gx::PairCfg<64, 192, 8, 8, 12, 16, 32, 128, 1>;
+
+#ifndef GX_PS_NW
+#define GX_PS_NW 12
+#endif
+using S192x64  = gx::PersistCfg<192, 64, 16, 12, 8, 8, GX_PS_NW, 4>;
+const KernelSet kPersistSets[] = {
+    make_persist_set<S192x64, PC192x64>(),
+};
+
+const KernelSet kPairSets[] = {
+    make_pair_set<P16x16, P16x16>(),   make_pair_set<P64x64, P64x64>(),   make_pair_set<P128x64, P128x64>(),
+    make_pair_set<P192x64, PC192x64>(), make_pair_set<P256x96, P256x96>(), make_pair_set<P64x192, P64x192>(),
+};
+
+// Three kernel families share the C-ABI ("Kernel families"):
+//   scalar  (nl_kernels.cuh)       block-synchronous, scalar FP32            -- default: fastest measured
+//   pair    (nl_pair_kernels.cuh)  block-synchronous, packed FADD2/FFMA2     -- GX_KERNELS=pair
+//   persist (nl_pair_kernels.cuh)  persistent, warp-asynchronous, packed     -- GX_KERNELS=persist
+// The environment variable is read at gx_grid_create; a family without an instantiation for the grid
+// falls through to the next one.
+const KernelSet* find_set(int Nx, int Ny, int Nl) {
+    const char* fam = std::getenv("GX_KERNELS");
+    if (fam && std::strcmp(fam, "persist") == 0)
+        for (const auto& k : kPersistSets)
+            if (k.Nx == Nx && k.Ny == Ny && Nl <= k.max_nl) return &k;
+    if (fam && (std::strcmp(fam, "pair") == 0 || std::strcmp(fam, "persist") == 0))
+        for (const auto& k : kPairSets)
+            if (k.Nx == Nx && k.Ny == Ny) return &k;
     for (const auto& k : kKernelSets)
         if (k.Nx == Nx && k.Ny == Ny) return &k;
     return nullptr;
@@ -269,7 +365,7 @@ int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out
     g->J = (3 * Nl - 1) / 2;
     g->sp.resize(Ns);
     g->adiabatic = (Ns == 1);
-    g->ks = find_set(Nx, Ny);
+    g->ks = find_set(Nx, Ny, Nl);
     *out = g;                       // returned even on failure below so that gx_last_error works
     if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
 
@@ -611,6 +707,12 @@ int gx_export_tables(gx_grid* g, float* T, float* Tinv, float* M) {
     }
     return GX_OK;
 }
+
+#ifdef GX_PHASE_TIMING
+int gx_debug_phase_clocks(long long* out) {
+    return cudaMemcpyFromSymbol(out, gx::gx_phase_clk, sizeof(long long) * 64 * 32) == cudaSuccess ? 0 : -1;
+}
+#endif
 
 const char* gx_last_error(gx_grid* g) { return g ? g->err.c_str() : "null handle"; }
 

@@ -231,3 +231,27 @@ def test_field_solve_parity(torch_cuda):
         ref = O.field_solve(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, tau_fac=cfg.tau_fac)
         assert O.relative_max_error(phi.cpu().numpy(), ref) <= TOL
         grid.close()
+
+
+@pytest.mark.parametrize("family", ["scalar", "pair", "persist"])
+@pytest.mark.parametrize("name", ["tiny", "cyclone", "kinetic", "w7x-shape"])
+def test_kernel_families_agree_with_oracle(torch_cuda, monkeypatch, family, name):
+    """Every kernel family behind the C-ABI (GX_KERNELS, read at gx_grid_create) meets the same bar;
+    a family without an instantiation for the grid falls through to the next one."""
+    monkeypatch.setenv("GX_KERNELS", family)
+    cfg = I.named_config(name)
+    geo = I.geometry_arrays(cfg)
+    planes = [(0, 0, 0), (cfg.Ns - 1, cfg.Nm - 1, cfg.Nz - 1), (0, cfg.Nm // 2, cfg.Nz // 3)]
+    sm = sorted({(s, m) for (s, m, z) in planes} | {(s, 0) for s in range(cfg.Ns)})
+    G = I.make_state(cfg, geo, planes=sm)
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = _grid(cfg, geo)
+    out = _gpu_nl(torch_cuda, grid, G, Phi)
+    out2 = _gpu_nl(torch_cuda, grid, G, Phi)                 # second call: counters / staging reuse
+    assert np.array_equal(out, out2)
+    ref = _oracle_nl(cfg, geo, G, Phi, method="dft", planes=planes)
+    for (s, m, z) in planes:
+        a, r = out[s, m, :, z], ref[s, m, :, z]
+        e = np.max(np.abs(a - r)) / np.max(np.abs(r))
+        assert e <= TOL, (family, name, s, m, z, e)
+    grid.close()
