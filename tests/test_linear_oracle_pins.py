@@ -1,0 +1,270 @@
+"""Pins of the linear-term oracle (oracle/gx_linear.py) to things other than itself: closed forms,
+library quadrature routines the oracle never calls, conservation identities and hand-computed values.
+Each test names the passage of PAPER.md ("P:nnn") whose transcription it would catch an error in."""
+import math
+
+import numpy as np
+import pytest
+from numpy.polynomial import hermite_e as HE
+from numpy.polynomial import laguerre as LA
+
+import gx_linear as L
+import gx_oracle as O
+
+NX = NY = 16
+NAKX, NAKY = 11, 6
+DKX, DKY, SHAT = 0.13, 0.1, 0.8
+
+
+def _geo(Nz, eps=0.18, q=1.4, drifts=True, flat=False):
+    z = -math.pi + 2 * math.pi * np.arange(Nz) / Nz
+    gradpar = 1.0 / q
+    if flat:
+        bmag = np.ones(Nz)
+        bgrad = np.zeros(Nz)
+    else:
+        bmag = 1.0 / (1.0 + eps * np.cos(z))
+        bgrad = gradpar * eps * np.sin(z) / (1.0 + eps * np.cos(z))          # gradpar d/dz ln B, analytic
+    g = dict(bmag=bmag, gds2=1 + (SHAT * z) ** 2, gds21=-SHAT * SHAT * z, gds22=np.full(Nz, SHAT ** 2),
+             gbdrift=2 * (np.cos(z) + SHAT * z * np.sin(z)) if drifts else np.zeros(Nz),
+             gbdrift0=-2 * SHAT * np.sin(z) if drifts else np.zeros(Nz),
+             bgrad=bgrad, jacobian=1.0 / (gradpar * bmag), gradpar=gradpar)
+    g["cvdrift"], g["cvdrift0"] = g["gbdrift"].copy(), g["gbdrift0"].copy()
+    return g, z
+
+
+def _rand(shape, seed):
+    r = np.random.default_rng(seed)
+    return r.standard_normal(shape) + 1j * r.standard_normal(shape)
+
+
+def _lin(G, Phi, geo, sp, terms, **kw):
+    return L.linear_rhs(G, Phi, NX, NY, DKX, DKY, SHAT, geo, [sp], terms=terms, **kw)
+
+
+def _phi_hermite(m, x):
+    """Orthonormal probabilists' Hermite function He_m(x)/sqrt(m!) (library evaluation)."""
+    c = np.zeros(m + 1)
+    c[m] = 1.0
+    return HE.hermeval(x, c) / math.sqrt(math.factorial(m))
+
+
+# ---------------------------------------------------------------------------- z operators
+def test_spectral_z_derivative_closed_form():
+    Nz = 16
+    z = -math.pi + 2 * math.pi * np.arange(Nz) / Nz
+    D, A = L.dz_matrix(Nz), L.abs_kz_matrix(Nz)
+    assert np.allclose(D @ np.sin(3 * z), 3 * np.cos(3 * z), atol=1e-12)
+    assert np.allclose(D @ np.cos(5 * z), -5 * np.sin(5 * z), atol=1e-12)
+    assert np.allclose(D @ np.cos(8 * z), 0, atol=1e-12)                   # Nyquist dropped (reading L2)
+    assert np.allclose(D @ np.ones(Nz), 0, atol=1e-13)
+    assert np.allclose(A @ np.cos(3 * z), 3 * np.cos(3 * z), atol=1e-12)
+    assert np.allclose(A @ np.cos(8 * z), 8 * np.cos(8 * z), atol=1e-12)   # |k_z| keeps it (reading L6)
+    assert np.allclose(D, -D.T, atol=1e-13) and np.allclose(A, A.T, atol=1e-13)
+
+
+# ---------------------------------------------------------------------------- streaming
+def test_streaming_matrix_elements_are_hermite_x():
+    """-v_t grad_par(sqrt(m+1) H_{m+1} + sqrt(m) H_{m-1}) is -v_t grad_par of 'multiplication by v_par'
+    in the orthonormal Hermite basis: <phi_m' | x | phi_m> by Gauss-Hermite quadrature (numpy)."""
+    Nz, Nm, kz = 8, 6, 2
+    geo, z = _geo(Nz, flat=True, drifts=False)
+    sp = dict(Z=1.0, mass=0.5, temp=2.0, dens=1.0, tprim=0, fprim=0, nu_ss=0)       # v_t = 2
+    x, w = HE.hermegauss(40)
+    w = w / math.sqrt(2 * math.pi)
+    X = np.array([[np.sum(w * _phi_hermite(a, x) * x * _phi_hermite(b, x)) for b in range(Nm)] for a in range(Nm)])
+    for m0 in range(Nm):
+        G = np.zeros((1, Nm, 1, Nz, NAKX, NAKY), complex)
+        G[0, m0, 0] = np.exp(1j * kz * z)[:, None, None]
+        r = _lin(G, np.zeros((Nz, NAKX, NAKY)), geo, sp, ("stream",))
+        for m in range(Nm):
+            expect = -2.0 * geo["gradpar"] * 1j * kz * X[m, m0] * G[0, m0, 0]
+            assert np.allclose(r[0, m, 0], expect, atol=1e-12), (m0, m)
+
+
+def test_streaming_of_the_potential_part_of_H():
+    """H_{l,0} = G_{l,0} + (Z/tau) J_l Phi (Eq. 4.8): with G = 0 only m = 1 moves, by
+    -v_t gradpar i k_z (Z/tau) J_l Phi."""
+    Nz, kz = 8, 1
+    geo, z = _geo(Nz, flat=True, drifts=False)
+    geo = dict(geo, gds2=np.ones(Nz), gds21=np.zeros(Nz))       # z-independent k_perp so that J_l Phi is one harmonic
+    sp = dict(Z=2.0, mass=1.0, temp=0.5, dens=1.0, tprim=0, fprim=0, nu_ss=0)
+    Phi = np.exp(1j * kz * z)[:, None, None] * _rand((1, NAKX, NAKY), 1)
+    r = _lin(np.zeros((1, 3, 2, Nz, NAKX, NAKY)), Phi, geo, sp, ("stream",))
+    kx, ky = DKX * O.kx_index(NX), DKY * O.ky_index(NY)
+    b = O.kperp2(kx, ky, geo["gds2"], geo["gds21"], geo["gds22"], SHAT) * (0.5 * 1.0 / 4.0)
+    vt = math.sqrt(0.5)
+    for l in range(2):
+        Jl = (-b / 2) ** l / math.factorial(l) * np.exp(-b / 2)
+        assert np.allclose(r[0, 1, l], -vt * geo["gradpar"] * 1j * kz * (2.0 / 0.5) * Jl * Phi, atol=1e-12)
+    assert np.all(r[0, 0] == 0) and np.all(r[0, 2] == 0)
+
+
+# ---------------------------------------------------------------------------- streaming + mirror
+def test_streaming_plus_mirror_conserve_free_energy_with_jacobian_weight():
+    """sum_z (1/B) Re sum_{l,m} conj(H) dH/dt = 0: d/dz of (H_m H_{m+1}/B) integrates to zero.  With
+    1/B = 1 + eps cos z and band-limited H the discrete sum is exact; a wrong sign or coefficient in any of
+    the four mirror terms (or the stray bracket of P:213 read differently) breaks it."""
+    Nz, Nm, Nl = 16, 5, 3
+    geo, z = _geo(Nz, drifts=False)
+    sp = dict(Z=1.0, mass=1.0, temp=1.0, dens=1.0, tprim=0, fprim=0, nu_ss=0)
+    amp = _rand((1, Nm, Nl, 5, NAKX, NAKY), 7)
+    G = sum(amp[:, :, :, i, None] * np.exp(1j * kzv * z)[None, None, None, :, None, None]
+            for i, kzv in enumerate([-2, -1, 0, 1, 2]))
+    Phi0 = np.zeros((Nz, NAKX, NAKY))
+    wgt = (1.0 / geo["bmag"])[None, None, None, :, None, None]
+    for terms, must_vanish in [(("stream", "mirror"), True), (("stream",), False), (("mirror",), False)]:
+        r = _lin(G, Phi0, geo, sp, terms)
+        W = np.sum(wgt * np.real(np.conj(G) * r), axis=(1, 2, 3))
+        ref = np.sum(np.abs(G) * np.abs(r), axis=(1, 2, 3))
+        rel = np.max(np.abs(W) / ref)
+        assert (rel < 1e-12) if must_vanish else (rel > 1e-4), (terms, rel)
+
+
+def test_mirror_hand_values():
+    """Mirror force on a single moment (l,m) = (1,1): the four neighbours it feeds and with which weights
+    (read off Eq. 4.9 with the roles of source and target exchanged)."""
+    Nz = 8
+    geo, z = _geo(Nz, drifts=False)
+    sp = dict(Z=1.0, mass=1.0, temp=1.0, dens=1.0, tprim=0, fprim=0, nu_ss=0)
+    G = np.zeros((1, 3, 3, Nz, NAKX, NAKY), complex)
+    src = _rand((Nz, NAKX, NAKY), 3)
+    G[0, 1, 1] = src
+    r = _lin(G, np.zeros((Nz, NAKX, NAKY)), geo, sp, ("mirror",))
+    bg = geo["bgrad"][:, None, None]
+    # target (l,m) receives from H_{1,1}:  (l,m)=(1,0): -(l+1)sqrt(m+1) = -2 ; (2,0): -l sqrt(m+1) = -2
+    #                                      (1,2): +l sqrt(m) = sqrt2 ; (0,2): +(l+1) sqrt(m) = sqrt2
+    assert np.allclose(r[0, 0, 1], -bg * (-2.0) * src)
+    assert np.allclose(r[0, 0, 2], -bg * (-2.0) * src)
+    assert np.allclose(r[0, 2, 1], -bg * math.sqrt(2.0) * src)
+    assert np.allclose(r[0, 2, 0], -bg * math.sqrt(2.0) * src)
+    touched = {(0, 1), (0, 2), (2, 1), (2, 0)}
+    for m in range(3):
+        for l in range(3):
+            if (m, l) not in touched:
+                assert np.all(r[0, m, l] == 0)
+
+
+# ---------------------------------------------------------------------------- drifts
+def test_drift_matrix_elements_by_library_quadrature():
+    """grad-B term = multiplication by mu B in the psi_l basis, curvature term = multiplication by v_par^2
+    in the Hermite basis: matrix elements by Gauss-Laguerre / Gauss-Hermite quadrature (numpy)."""
+    Nz, Nm, Nl = 4, 5, 4
+    geo, z = _geo(Nz, flat=True)
+    sp = dict(Z=-1.0, mass=1.0, temp=2.0, dens=1.0, tprim=0, fprim=0, nu_ss=0)
+    tz = 2.0 / -1.0
+    kx, ky = DKX * O.kx_index(NX), DKY * O.ky_index(NY)
+    wk, wb = L.drift_frequencies(kx, ky, geo, SHAT)
+    xl, wl = LA.laggauss(30)
+    psi = lambda l, x: (-1.0) ** l * LA.lagval(x, np.eye(l + 1)[l])
+    ML = np.array([[np.sum(wl * psi(a, xl) * xl * psi(b, xl)) for b in range(Nl)] for a in range(Nl)])
+    xh, wh = HE.hermegauss(40)
+    wh = wh / math.sqrt(2 * math.pi)
+    MH = np.array([[np.sum(wh * _phi_hermite(a, xh) * xh ** 2 * _phi_hermite(b, xh)) for b in range(Nm)]
+                   for a in range(Nm)])
+    G = _rand((1, Nm, Nl, Nz, NAKX, NAKY), 11)
+    geo_b = dict(geo, cvdrift=np.zeros(Nz), cvdrift0=np.zeros(Nz))
+    geo_k = dict(geo, gbdrift=np.zeros(Nz), gbdrift0=np.zeros(Nz))
+    rb = _lin(G, np.zeros((Nz, NAKX, NAKY)), geo_b, sp, ("drift",))
+    rk = _lin(G, np.zeros((Nz, NAKX, NAKY)), geo_k, sp, ("drift",))
+    assert np.allclose(rb[0], -1j * tz * wb * np.einsum("ab,mbzxy->mazxy", ML, G[0]), atol=1e-11)
+    assert np.allclose(rk[0], -1j * tz * wk * np.einsum("ab,blzxy->alzxy", MH, G[0]), atol=1e-11)
+    # s-alpha closed form of the frequencies (reading L3): w_d = ky (cos z + shat z sin z) - kx sin z
+    zz = z[:, None, None]
+    assert np.allclose(wb, ky[None, None, :] * (np.cos(zz) + SHAT * zz * np.sin(zz)) - kx[None, :, None] * np.sin(zz))
+    # anti-Hermitian: no free-energy change, mode by mode
+    r = _lin(G, np.zeros((Nz, NAKX, NAKY)), geo, sp, ("drift",))
+    assert np.max(np.abs(np.sum(np.real(np.conj(G) * r), axis=(1, 2)))) < 1e-11
+
+
+# ---------------------------------------------------------------------------- drive
+def test_drive_hand_values_at_zero_larmor_radius():
+    Nz = 4
+    geo, z = _geo(Nz, flat=True)
+    sp = dict(Z=1.0, mass=1e-30, temp=1.0, dens=1.0, tprim=6.9, fprim=2.2, nu_ss=0)      # b = 0: J_0 = 1
+    Phi = _rand((Nz, NAKX, NAKY), 5)
+    r = _lin(np.zeros((1, 4, 3, Nz, NAKX, NAKY)), Phi, geo, sp, ("drive",))
+    iky = 1j * (DKY * O.ky_index(NY))[None, None, :]
+    assert np.allclose(r[0, 0, 0], iky * 2.2 * Phi)                 # density gradient drives density
+    assert np.allclose(r[0, 0, 1], iky * 6.9 * Phi)                 # temperature gradient drives T_perp
+    assert np.allclose(r[0, 2, 0], iky * 6.9 * Phi / math.sqrt(2))  # ... and T_par
+    for (m, l) in [(0, 2), (1, 0), (1, 1), (2, 1), (3, 0)]:
+        assert np.max(np.abs(r[0, m, l])) < 1e-25          # b = O(1e-30), not exactly 0
+
+
+# ---------------------------------------------------------------------------- Dougherty
+def test_dougherty_conserves_density_momentum_energy_and_damps_the_rest():
+    Nz, Nm, Nl = 4, 5, 3
+    geo, z = _geo(Nz, flat=True)
+    nu = 0.37
+    sp = dict(Z=1.0, mass=1.0, temp=1.0, dens=1.0, tprim=0, fprim=0, nu_ss=nu)
+    G = _rand((1, Nm, Nl, Nz, NAKX, NAKY), 13)
+    r = _lin(G, np.zeros((Nz, NAKX, NAKY)), geo, sp, ("coll",))
+    k0 = (slice(None), 0, 0)                                   # kx = ky = 0: b = 0
+    s = np.max(np.abs(G))
+    assert np.max(np.abs(r[0, 0, 0][k0])) < 1e-13 * s          # density
+    assert np.max(np.abs(r[0, 1, 0][k0])) < 1e-13 * s          # parallel momentum
+    assert np.max(np.abs(math.sqrt(2) * r[0, 2, 0][k0] + 2 * r[0, 0, 1][k0])) < 1e-12 * s   # T_par + 2 T_perp
+    assert np.allclose(r[0, 3, 1][k0], -nu * (2 * 1 + 3) * G[0, 3, 1][k0])                 # plain damping
+    assert np.allclose(r[0, 4, 2][k0], -nu * (2 * 2 + 4) * G[0, 4, 2][k0])
+    # finite b: the rate of a moment outside the conserved set is -nu (b + 2l + m)
+    kx, ky = DKX * O.kx_index(NX), DKY * O.ky_index(NY)
+    b = O.kperp2(kx, ky, geo["gds2"], geo["gds21"], geo["gds22"], SHAT)
+    assert np.allclose(r[0, 4, 1], -nu * (b + 2 + 4) * G[0, 4, 1])
+    # free energy never grows under like-particle collisions
+    assert np.all(np.sum(np.real(np.conj(G) * r), axis=(1, 2)) <= 1e-12)
+
+
+# ---------------------------------------------------------------------------- hyper-dissipation
+def test_hyper_dissipation_closed_forms():
+    Nz, Nm = 8, 6
+    geo, z = _geo(Nz)
+    sp = dict(Z=1.0, mass=1.0, temp=4.0, dens=1.0, tprim=0, fprim=0, nu_ss=0)          # v_t = 2
+    G = _rand((1, Nm, 1, Nz, NAKX, NAKY), 17)
+    r = _lin(G, np.zeros((Nz, NAKX, NAKY)), geo, sp, ("hypervisc",), D_hyper=0.05, n_hyper=4)
+    kx, ky = DKX * O.kx_index(NX), DKY * O.ky_index(NY)
+    kp2 = (kx[None, :, None] - SHAT * z[:, None, None] * ky[None, None, :]) ** 2 + ky[None, None, :] ** 2
+    rate = r[0, 2, 0] / G[0, 2, 0]
+    assert np.allclose(rate, -0.05 * (kp2 / kp2.max()) ** 4, atol=1e-13)
+    assert abs(rate.real.min() + 0.05) < 1e-13 and np.all(rate[:, 0, 0] == 0)
+    kz = 3
+    G2 = np.zeros_like(G)
+    for m in range(Nm):
+        G2[0, m, 0] = np.exp(1j * kz * z)[:, None, None] * (m + 1)
+    r2 = _lin(G2, np.zeros((Nz, NAKX, NAKY)), geo, sp, ("hypercoll",), f_hyp=1.0)
+    p = Nm / 2
+    nuhyp = 2.5 * (p + 0.5) / (Nm - 1) ** (p + 0.5) * (geo["gradpar"] * kz) * 2.0
+    for m in range(Nm):
+        expect = -nuhyp * m ** p * G2[0, m, 0] if m > 2 else 0 * G2[0, m, 0]
+        assert np.allclose(r2[0, m, 0], expect, atol=1e-12), m
+
+
+# ---------------------------------------------------------------------------- time stepping
+def test_ssp_rk3_is_third_order_taylor_on_linear_problem():
+    lam, dt = -0.7 + 2.0j, 0.1
+    y = L.ssp_rk3_step(1.0 + 0j, dt, lambda v: lam * v)
+    x = lam * dt
+    assert abs(y - (1 + x + x * x / 2 + x ** 3 / 6)) < 1e-15
+    errs = []
+    for n in (20, 40):
+        v = 1.0 + 0j
+        for _ in range(n):
+            v = L.ssp_rk3_step(v, 1.0 / n, lambda u: lam * u)
+        errs.append(abs(v - np.exp(lam)))
+    assert 6.5 < errs[0] / errs[1] < 9.5                      # third order: error ratio ~ 8
+
+
+def test_full_rhs_is_sum_of_parts_and_linear_in_g_without_bracket():
+    Nz = 4
+    geo, z = _geo(Nz)
+    sp = dict(Z=1.0, mass=1.0, temp=1.0, dens=1.0, tprim=6.9, fprim=2.2, nu_ss=0.01)
+    G = 1e-3 * _rand((1, 4, 2, Nz, NAKX, NAKY), 19)
+    K = (NAKX - 1) // 2
+    G[..., 0, 0] = 0
+    G[..., NAKX - 1:K:-1, 0] = np.conj(G[..., 1:K + 1, 0])
+    full = L.rhs(G, NX, NY, DKX, DKY, SHAT, geo, [sp])
+    lin = L.rhs(G, NX, NY, DKX, DKY, SHAT, geo, [sp], nonlinear=False)
+    Phi = O.field_solve(G, NX, NY, DKX, DKY, SHAT, geo, [sp])
+    nl = O.nonlinear_rhs(G, Phi, NX, NY, DKX, DKY, SHAT, geo, [sp], method="conv_np")
+    assert np.allclose(full, lin + nl, atol=1e-14)
+    assert np.allclose(L.rhs(2 * G, NX, NY, DKX, DKY, SHAT, geo, [sp], nonlinear=False), 2 * lin, atol=1e-15)
