@@ -8,6 +8,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <string>
 #include <vector>
@@ -36,23 +37,27 @@ struct LinTables {
     float* fsfac = nullptr;    // [kx]
     float* wz = nullptr;       // [z] jacobian weights, sum 1
     float* bs = nullptr;       // [s][z][k]  b_s
-    float* Dz = nullptr;       // [z][z'] gradpar * spectral d/dz
-    float* Az = nullptr;       // [z][z'] gradpar * spectral |k_z|
+    float* Dz = nullptr;       // [Nz] circulant column of gradpar * spectral d/dz:  D[z][z'] = Dz[(z - z') mod Nz]
+    float* Az = nullptr;       // [Nz] circulant column of |gradpar| * spectral |k_z|
     float* omd = nullptr;      // [2][z][k]  omega_d^kappa, omega_d^gradB
     float* hypv = nullptr;     // [z][k] D (kperp2/kperp2max)^n
     float* bgrad = nullptr;    // [z]
     float qn[kMaxSpecies] = {0}, zt[kMaxSpecies] = {0}, vt[kMaxSpecies] = {0}, tz[kMaxSpecies] = {0};
     float tprim[kMaxSpecies] = {0}, fprim[kMaxSpecies] = {0}, nu[kMaxSpecies] = {0}, nuhyp[kMaxSpecies] = {0};
+    float* mpow = nullptr;     // [Nm] m^p, p = Nm/2 (Eq. 4.27)
+    float2* mom = nullptr;     // [s][3][z][k] workspace: u_par, u_perp, T of the Dougherty operator
     float dky = 0;
+    bool any_nu = false;
     bool built = false;
 };
 
 constexpr int kLinLaunchesFieldSolve = 2;
-constexpr int kLinLaunchesRhs = 1;
+constexpr int kLinLaunchesRhs = 2;
 
 inline void lin_tables_free(LinTables& t) {
     cudaFree(t.Jl); cudaFree(t.invD); cudaFree(t.fsfac); cudaFree(t.wz); cudaFree(t.bs);
     cudaFree(t.Dz); cudaFree(t.Az); cudaFree(t.omd); cudaFree(t.hypv); cudaFree(t.bgrad);
+    cudaFree(t.mpow); cudaFree(t.mom);
     t = LinTables();
 }
 
@@ -117,7 +122,49 @@ inline bool lin_tables_build(const LinHostInput& in, LinTables& t, size_t& bytes
             fsfac[i] = (i == 0 || d == 0.0) ? 0.f : (float)(pref * in.tau_fac / d);
         }
     }
-    (void)K;
+    // ---- linear-term tables (Eq. 4.9-4.18, 4.26-4.28; readings L2-L6 of DESIGN.md)
+    std::vector<float> omd(2 * (size_t)Nz * nk), hypv((size_t)Nz * nk), bgr(Nz), dzc(Nz), azc(Nz), mpow(in.Nm);
+    double kp2max = 0;
+    for (size_t i = 0; i < (size_t)Nz * nk; ++i) kp2max = std::max(kp2max, in.kp2[i]);
+    for (int z = 0; z < Nz; ++z) {
+        bgr[z] = (float)in.bgrad[z];
+        for (int i = 0; i < nakx; ++i) {
+            const double kx = in.dkx * (i <= K ? i : i - nakx);
+            for (int q = 0; q < naky; ++q) {
+                const double ky = in.dky * q;
+                const size_t k = ((size_t)z * nakx + i) * naky + q;
+                omd[k] = (float)(0.5 * (ky * in.cvdrift[z] + kx * in.cvdrift0[z] / in.shat));
+                omd[(size_t)Nz * nk + k] = (float)(0.5 * (ky * in.gbdrift[z] + kx * in.gbdrift0[z] / in.shat));
+                hypv[k] = kp2max > 0 ? (float)(in.D_hyper * std::pow(in.kp2[k] / kp2max, (double)in.n_hyper)) : 0.f;
+            }
+        }
+    }
+    for (int d = 0; d < Nz; ++d) {
+        double sd = 0, sa = 0;
+        for (int kk = 0; kk < Nz; ++kk) {
+            const int kz = kk <= Nz / 2 ? kk : kk - Nz;
+            const double ang = 2.0 * M_PI * (double)kz * d / Nz;
+            if (!(Nz % 2 == 0 && kk == Nz / 2)) sd -= kz * std::sin(ang);   // Nyquist dropped in d/dz
+            sa += std::abs((double)kz) * std::cos(ang);
+        }
+        dzc[d] = (float)(in.gradpar * sd / Nz);
+        azc[d] = (float)(std::abs(in.gradpar) * sa / Nz);
+    }
+    const double p_hyp = 0.5 * in.Nm, m_max = std::max(in.Nm - 1, 1);
+    for (int m = 0; m < in.Nm; ++m) mpow[m] = m > 2 ? (float)std::pow((double)m, p_hyp) : 0.f;
+    t.any_nu = false;
+    for (int s = 0; s < Ns; ++s) {
+        t.nuhyp[s] = (float)(2.5 * in.f_hyp * (p_hyp + 0.5) / std::pow(m_max, p_hyp + 0.5) * std::sqrt(in.species[s].temp / in.species[s].mass));
+        if (in.species[s].nu != 0.0) t.any_nu = true;
+    }
+    if (!lin_upload(&t.omd, omd, bytes, msg) || !lin_upload(&t.hypv, hypv, bytes, msg) ||
+        !lin_upload(&t.bgrad, bgr, bytes, msg) || !lin_upload(&t.Dz, dzc, bytes, msg) ||
+        !lin_upload(&t.Az, azc, bytes, msg) || !lin_upload(&t.mpow, mpow, bytes, msg))
+        return false;
+    {
+        std::vector<float2> zero((size_t)Ns * 3 * Nz * nk, make_float2(0.f, 0.f));
+        if (!lin_upload(&t.mom, zero, bytes, msg)) return false;
+    }
     if (!lin_upload(&t.Jl, Jl, bytes, msg) || !lin_upload(&t.bs, bs, bytes, msg) ||
         !lin_upload(&t.invD, invD, bytes, msg) || !lin_upload(&t.fsfac, fsfac, bytes, msg) ||
         !lin_upload(&t.wz, wz, bytes, msg))
@@ -177,10 +224,191 @@ inline cudaError_t lin_field_solve(const LinTables& t, const float2* g, float2* 
     return cudaGetLastError();
 }
 
+// ------------------------------------------------------------------------------------------------
+// Linear terms of Eq. 4.9 for gx_linear_rhs / gx_rhs.
+// H_{l,m} = G_{l,m} + (Z/tau) J_l Phi delta_{m0} (Eq. 4.8) is formed on the fly; H, G, J vanish outside
+// 0 <= l < Nl, 0 <= m < Nm.
+__device__ __forceinline__ float2 lin_H(const LinTables& t, const float2* __restrict__ g, const float2* __restrict__ phi,
+                                        int s, int l, int m, int z, int k) {
+    if (l < 0 || l >= t.Nl || m < 0 || m >= t.Nm) return make_float2(0.f, 0.f);
+    float2 h = g[((((size_t)s * t.Nm + m) * t.Nl + l) * t.Nz + z) * t.nk + k];
+    if (m == 0) {
+        const float c = t.zt[s] * t.Jl[(((size_t)s * t.Nl + l) * t.Nz + z) * t.nk + k];
+        const float2 f = phi[(size_t)z * t.nk + k];
+        h.x = fmaf(c, f.x, h.x);
+        h.y = fmaf(c, f.y, h.y);
+    }
+    return h;
+}
+__device__ __forceinline__ float lin_J(const LinTables& t, int s, int l, int z, int k) {
+    return (l < 0 || l >= t.Nl) ? 0.f : t.Jl[(((size_t)s * t.Nl + l) * t.Nz + z) * t.nk + k];
+}
+
+// field-particle moments of the Dougherty operator, Eq. 4.14-4.18: mom[s][0..2][z][k]
+__global__ void __launch_bounds__(256) lin_moments_kernel(LinTables t, const float2* __restrict__ g,
+                                                          const float2* __restrict__ phi) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int z = blockIdx.y, s = blockIdx.z;
+    if (k >= t.nk) return;
+    const float b = t.bs[((size_t)s * t.Nz + z) * t.nk + k];
+    const float sb = sqrtf(fmaxf(b, 0.f));
+    float2 up = make_float2(0.f, 0.f), uq = up, tp = up, tq = up;
+    for (int l = 0; l < t.Nl; ++l) {
+        const float jm = lin_J(t, s, l - 1, z, k), j0 = lin_J(t, s, l, z, k), jp = lin_J(t, s, l + 1, z, k);
+        const float2 h0 = lin_H(t, g, phi, s, l, 0, z, k), h1 = lin_H(t, g, phi, s, l, 1, z, k),
+                     h2 = lin_H(t, g, phi, s, l, 2, z, k);
+        const float cq = j0 + jm, ct = l * jm + 2.f * l * j0 + (l + 1.f) * jp;
+        up.x = fmaf(j0, h1.x, up.x); up.y = fmaf(j0, h1.y, up.y);
+        uq.x = fmaf(cq, h0.x, uq.x); uq.y = fmaf(cq, h0.y, uq.y);
+        tp.x = fmaf(j0, h2.x, tp.x); tp.y = fmaf(j0, h2.y, tp.y);
+        tq.x = fmaf(ct, h0.x, tq.x); tq.y = fmaf(ct, h0.y, tq.y);
+    }
+    const float r2 = 1.41421356237309504880f;
+    float2* __restrict__ mo = t.mom + ((size_t)s * 3 * t.Nz + z) * t.nk + k;
+    const size_t st = (size_t)t.Nz * t.nk;
+    mo[0] = up;
+    mo[st] = make_float2(sb * uq.x, sb * uq.y);
+    mo[2 * st] = make_float2((r2 * tp.x + 2.f * tq.x) * (1.f / 3.f), (r2 * tp.y + 2.f * tq.y) * (1.f / 3.f));
+}
+
+constexpr int kLinTK = 32;      // k per block
+constexpr int kLinZG = 8;       // z groups per block
+
+// out[s,m,l,z,k] (+)= linear terms.  Block: one (s,m,l), a tile of kLinTK modes k, all z.  The spectral
+// parallel derivative / |k_par| are circulant Nz x Nz products on tiles staged in shared memory.
+template <bool ACC>
+__global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, const float2* __restrict__ g,
+                                                                 const float2* __restrict__ phi,
+                                                                 float2* __restrict__ out) {
+    extern __shared__ __align__(16) unsigned char lin_smem[];
+    float2* S1 = reinterpret_cast<float2*>(lin_smem);            // [Nz][TK] sqrt(m+1) H_{l,m+1} + sqrt(m) H_{l,m-1}
+    float2* S2 = S1 + (size_t)t.Nz * kLinTK;                     // [Nz][TK] G_{l,m} (hyper-collisions)
+    float* dz = reinterpret_cast<float*>(S2 + (size_t)t.Nz * kLinTK);
+    float* az = dz + t.Nz;
+    const int tk = threadIdx.x % kLinTK, zg = threadIdx.x / kLinTK;
+    const int k = blockIdx.x * kLinTK + tk;
+    const int l = blockIdx.y;
+    const int s = blockIdx.z / t.Nm, m = blockIdx.z % t.Nm;
+    const bool live = k < t.nk;
+    const float sm1 = sqrtf((float)(m + 1)), sm0 = sqrtf((float)m);
+    for (int i = threadIdx.x; i < t.Nz; i += blockDim.x) { dz[i] = t.Dz[i]; az[i] = t.Az[i]; }
+    for (int z = zg; z < t.Nz; z += kLinZG) {
+        float2 c = make_float2(0.f, 0.f), gg = c;
+        if (live) {
+            const float2 hp = lin_H(t, g, phi, s, l, m + 1, z, k), hm = lin_H(t, g, phi, s, l, m - 1, z, k);
+            c = make_float2(sm1 * hp.x + sm0 * hm.x, sm1 * hp.y + sm0 * hm.y);
+            gg = g[((((size_t)s * t.Nm + m) * t.Nl + l) * t.Nz + z) * t.nk + k];
+        }
+        S1[z * kLinTK + tk] = c;
+        S2[z * kLinTK + tk] = gg;
+    }
+    __syncthreads();
+    if (!live) return;
+    const float vt = t.vt[s], tz = t.tz[s], nu = t.nu[s];
+    const float hyp = t.nuhyp[s] * t.mpow[m];
+    const float ky = t.dky * (float)(k % t.naky);
+    const float fl = (float)l, fm = (float)m;
+    for (int z = zg; z < t.Nz; z += kLinZG) {
+        // streaming: -v_t grad_par(...)   and hyper-collisions: -nu_hyp m^p |k_par| G
+        float2 dp = make_float2(0.f, 0.f), ap = dp;
+        for (int zp = 0; zp < t.Nz; ++zp) {
+            int d = z - zp;
+            d += d < 0 ? t.Nz : 0;
+            const float2 a = S1[zp * kLinTK + tk];
+            dp.x = fmaf(dz[d], a.x, dp.x); dp.y = fmaf(dz[d], a.y, dp.y);
+            if (hyp != 0.f) {
+                const float2 b2 = S2[zp * kLinTK + tk];
+                ap.x = fmaf(az[d], b2.x, ap.x); ap.y = fmaf(az[d], b2.y, ap.y);
+            }
+        }
+        float2 r = make_float2(-vt * dp.x - hyp * ap.x, -vt * dp.y - hyp * ap.y);
+        const float2 h00 = lin_H(t, g, phi, s, l, m, z, k);
+        // mirror force
+        {
+            const float2 a = lin_H(t, g, phi, s, l, m + 1, z, k), b2 = lin_H(t, g, phi, s, l - 1, m + 1, z, k),
+                         c = lin_H(t, g, phi, s, l, m - 1, z, k), d2 = lin_H(t, g, phi, s, l + 1, m - 1, z, k);
+            const float ca = -(fl + 1.f) * sm1, cb = -fl * sm1, cc = fl * sm0, cd = (fl + 1.f) * sm0;
+            const float f = -vt * t.bgrad[z];
+            r.x += f * (ca * a.x + cb * b2.x + cc * c.x + cd * d2.x);
+            r.y += f * (ca * a.y + cb * b2.y + cc * c.y + cd * d2.y);
+        }
+        // curvature and grad-B drifts: -i (tau/Z) w (...)
+        {
+            const float wk = t.omd[(size_t)z * t.nk + k], wb = t.omd[((size_t)t.Nz + z) * t.nk + k];
+            const float2 a = lin_H(t, g, phi, s, l, m + 2, z, k), c = lin_H(t, g, phi, s, l, m - 2, z, k);
+            const float2 e = lin_H(t, g, phi, s, l + 1, m, z, k), f2 = lin_H(t, g, phi, s, l - 1, m, z, k);
+            const float cA = sqrtf((fm + 1.f) * (fm + 2.f)), cB = 2.f * fm + 1.f, cC = sqrtf(fm * fmaxf(fm - 1.f, 0.f));
+            const float bx = wk * (cA * a.x + cB * h00.x + cC * c.x) + wb * ((fl + 1.f) * e.x + (2.f * fl + 1.f) * h00.x + fl * f2.x);
+            const float by = wk * (cA * a.y + cB * h00.y + cC * c.y) + wb * ((fl + 1.f) * e.y + (2.f * fl + 1.f) * h00.y + fl * f2.y);
+            r.x += tz * by;          // -i (x + i y) = y - i x
+            r.y -= tz * bx;
+        }
+        const float jm = lin_J(t, s, l - 1, z, k), j0 = lin_J(t, s, l, z, k), jp = lin_J(t, s, l + 1, z, k);
+        const float jt = fl * jm + 2.f * fl * j0 + (fl + 1.f) * jp;
+        // drive (Eq. 4.12, Phi parts): i ky (...) Phi
+        if (m == 0 || m == 2) {
+            const float2 f = phi[(size_t)z * t.nk + k];
+            const float c = m == 0 ? t.fprim[s] * j0 + t.tprim[s] * jt : t.tprim[s] * j0 * 0.70710678118654752440f;
+            r.x -= ky * c * f.y;
+            r.y += ky * c * f.x;
+        }
+        // Dougherty collisions (Eq. 4.13)
+        if (nu != 0.f) {
+            const float b = t.bs[((size_t)s * t.Nz + z) * t.nk + k];
+            const float damp = nu * (b + 2.f * fl + fm);
+            r.x -= damp * h00.x;
+            r.y -= damp * h00.y;
+            if (m <= 2) {
+                const float2* __restrict__ mo = t.mom + ((size_t)s * 3 * t.Nz + z) * t.nk + k;
+                const size_t st = (size_t)t.Nz * t.nk;
+                float2 add = make_float2(0.f, 0.f);
+                if (m == 0) {
+                    const float2 uq = mo[st], tb = mo[2 * st];
+                    const float cu = sqrtf(fmaxf(b, 0.f)) * (j0 + jm), ct = 2.f * jt;
+                    add = make_float2(cu * uq.x + ct * tb.x, cu * uq.y + ct * tb.y);
+                } else if (m == 1) {
+                    const float2 up = mo[0];
+                    add = make_float2(j0 * up.x, j0 * up.y);
+                } else {
+                    const float2 tb = mo[2 * st];
+                    add = make_float2(1.41421356237309504880f * j0 * tb.x, 1.41421356237309504880f * j0 * tb.y);
+                }
+                r.x = fmaf(nu, add.x, r.x);
+                r.y = fmaf(nu, add.y, r.y);
+            }
+        }
+        // hyper-viscosity (Eq. 4.26)
+        {
+            const float hv = t.hypv[(size_t)z * t.nk + k];
+            const float2 gg = S2[z * kLinTK + tk];
+            r.x -= hv * gg.x;
+            r.y -= hv * gg.y;
+        }
+        float2* __restrict__ o = out + ((((size_t)s * t.Nm + m) * t.Nl + l) * t.Nz + z) * t.nk + k;
+        if (ACC) { const float2 prev = *o; r.x += prev.x; r.y += prev.y; }
+        *o = r;
+    }
+}
+
 inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* phi, float2* out, bool accumulate,
                            cudaStream_t st) {
-    (void)t; (void)g; (void)phi; (void)out; (void)accumulate; (void)st;
-    return cudaErrorNotSupported;   // linear terms: next milestone
+    if (!t.built) return cudaErrorNotReady;
+    if (t.any_nu) {
+        dim3 gm((t.nk + 255) / 256, t.Nz, t.Ns);
+        lin_moments_kernel<<<gm, 256, 0, st>>>(t, g, phi);
+    }
+    const size_t smem = (size_t)t.Nz * kLinTK * sizeof(float2) * 2 + 2 * (size_t)t.Nz * sizeof(float);
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(lin_rhs_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    dim3 grid((t.nk + kLinTK - 1) / kLinTK, t.Nl, t.Ns * t.Nm);
+    if (accumulate) lin_rhs_kernel<true><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+    else lin_rhs_kernel<false><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+    return cudaGetLastError();
 }
 
 }  // namespace gx

@@ -255,3 +255,58 @@ def test_kernel_families_agree_with_oracle(torch_cuda, monkeypatch, family, name
         e = np.max(np.abs(a - r)) / np.max(np.abs(r))
         assert e <= TOL, (family, name, s, m, z, e)
     grid.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# linear terms and the full right-hand side against oracle/gx_linear.py
+import gx_linear as OL
+
+
+def _oracle_lin(cfg, geo, G, Phi):
+    return OL.linear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species)
+
+
+@pytest.mark.parametrize("name", ["tiny", "cyclone", "kinetic", "w7x-shape"])
+def test_linear_rhs_parity(torch_cuda, name):
+    torch = torch_cuda
+    cfg = I.named_config(name)
+    if name == "w7x-shape":
+        cfg = I.Config(cfg.name, cfg.Nx, cfg.Ny, cfg.Nz, cfg.Nl, 4, cfg.species, geometry=cfg.geometry, seed=cfg.seed)
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = _grid(cfg, geo)
+    g, phi = torch.from_numpy(G).cuda(), torch.from_numpy(Phi).cuda()
+    out = torch.full_like(g, float("nan"))
+    grid.linear_rhs(g, phi, out)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    ref = _oracle_lin(cfg, geo, G, Phi)
+    assert np.all(np.isfinite(out))
+    assert O.relative_max_error(out, ref) <= TOL
+    for s in range(cfg.Ns):
+        for m in range(cfg.Nm):                                # per-(s,m) slabs: every stencil row is exercised
+            assert O.relative_max_error(out[s, m], ref[s, m]) <= 5 * TOL, (s, m)
+    grid.close()
+
+
+@pytest.mark.parametrize("name", ["tiny", "cyclone"])
+def test_full_rhs_parity(torch_cuda, name):
+    """gx_rhs = field solve + (-N) + linear terms, all on the device, against the oracle's rhs()."""
+    torch = torch_cuda
+    cfg = I.named_config(name)
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    grid = _grid(cfg, geo)
+    g = torch.from_numpy(G).cuda()
+    out = torch.full_like(g, float("nan"))
+    grid.rhs(g, out)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    ref = OL.rhs(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, tau_fac=cfg.tau_fac)
+    assert np.all(np.isfinite(out))
+    assert O.relative_max_error(out, ref) <= TOL
+    # the nonlinear part alone must still be visible at this tolerance (it is not drowned by the linear part)
+    lin = OL.rhs(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, tau_fac=cfg.tau_fac, nonlinear=False)
+    assert O.relative_max_error(lin, ref) > 10 * TOL
+    grid.close()
