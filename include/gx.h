@@ -110,6 +110,12 @@ int gx_field_solve(gx_grid* g, const void* g_dev, void* phi_dev, void* cuda_stre
  * phi is computed internally with gx_field_solve.  Electrostatic (beta_ref = 0). */
 int gx_rhs(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream);
 
+/* One step of the third-order SSP Runge-Kutta scheme the paper uses for the nonlinear runs (P:347,
+ * Shu-Osher form): g1 = g + dt R(g); g2 = 3/4 g + 1/4 (g1 + dt R(g1)); g <- 1/3 g + 2/3 (g2 + dt R(g2)),
+ * R = gx_rhs.  g_dev is updated in place; two state-sized work buffers are owned by the handle
+ * (allocated on first use).  Enqueued on `cuda_stream`; 3 gx_rhs evaluations + 3 fused stage kernels. */
+int gx_ssprk3_step(gx_grid* g, void* g_dev, double dt, void* cuda_stream);
+
 /* Linear part only (gx_rhs without -N), given phi; used to test the linear terms on their own. */
 int gx_linear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream);
 

@@ -21,7 +21,7 @@ GX_OK, GX_ERR_ARG, GX_ERR_STATE, GX_ERR_UNSUPPORTED, GX_ERR_CUDA, GX_ERR_ALLOC =
 
 EXPORTED = ["gx_grid_create", "gx_grid_destroy", "gx_box_set", "gx_species_set", "gx_adiabatic_set",
             "gx_dissipation_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_host",
-            "gx_field_solve", "gx_rhs", "gx_linear_rhs", "gx_query", "gx_export_maps",
+            "gx_field_solve", "gx_rhs", "gx_linear_rhs", "gx_ssprk3_step", "gx_query", "gx_export_maps",
             "gx_export_tables", "gx_profile_set", "gx_profile_get", "gx_last_error"]
 
 _lib = None
@@ -55,6 +55,7 @@ def load():
     lib.gx_field_solve.argtypes = [vp, vp, vp, vp]
     lib.gx_rhs.argtypes = [vp, vp, vp, vp]
     lib.gx_linear_rhs.argtypes = [vp, vp, vp, vp, vp]
+    lib.gx_ssprk3_step.argtypes = [vp, vp, d, vp]
     lib.gx_query.argtypes = [vp, i, C.POINTER(C.c_longlong)]
     lib.gx_export_maps.argtypes = [vp, vp, vp, vp, vp, vp, vp]
     lib.gx_export_tables.argtypes = [vp, vp, vp, vp]
@@ -135,6 +136,10 @@ def gx_rhs(h, g_ptr, out_ptr, stream=0):
 
 def gx_linear_rhs(h, g_ptr, phi_ptr, out_ptr, stream=0):
     _check(h, load().gx_linear_rhs(h, g_ptr, phi_ptr, out_ptr, stream))
+
+
+def gx_ssprk3_step(h, g_ptr, dt, stream=0):
+    _check(h, load().gx_ssprk3_step(h, g_ptr, float(dt), stream))
 
 
 def gx_query(h, what):
@@ -232,6 +237,10 @@ class Grid:
     def linear_rhs(self, g, phi, out):
         gx_linear_rhs(self.h, g.data_ptr(), phi.data_ptr(), out.data_ptr(), self._stream())
         return out
+
+    def ssprk3_step(self, g, dt):
+        gx_ssprk3_step(self.h, g.data_ptr(), dt, self._stream())
+        return g
 
     def export_maps(self):
         c = self.cfg

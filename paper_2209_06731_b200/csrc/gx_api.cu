@@ -2,6 +2,7 @@
 // kernel dispatch.  No CPU compute path exists: every step of the hot path runs in nl_kernels.cuh.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -275,6 +276,7 @@ struct gx_grid {
     float2 *dgbuf = nullptr, *dphibuf = nullptr, *doutbuf = nullptr;   // for the *_host entry point
     gx::LinTables lin;                                                  // linear-term tables
     float2* dphi_rhs = nullptr;                                         // phi of gx_rhs
+    float2 *drk_y = nullptr, *drk_k = nullptr;                          // SSP-RK3 stage and slope buffers
     size_t bytes = 0;
     bool profile = false;
     std::vector<cudaEvent_t> ev_pool;          // 4 events per profiled call
@@ -412,7 +414,7 @@ int gx_grid_destroy(gx_grid* g) {
     if (!g) return GX_ERR_ARG;
     cudaFree(g->dT); cudaFree(g->dTinv); cudaFree(g->dM); cudaFree(g->dtwx); cudaFree(g->dtwy);
     cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dcount); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
-    cudaFree(g->dphi_rhs);
+    cudaFree(g->dphi_rhs); cudaFree(g->drk_y); cudaFree(g->drk_k);
     for (auto e : g->ev_pool) cudaEventDestroy(e);
     gx::lin_tables_free(g->lin);
     delete g;
@@ -651,6 +653,30 @@ int gx_rhs(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream) {
     cudaError_t e = gx::lin_rhs(g->lin, (const float2*)g_dev, g->dphi_rhs, (float2*)out_dev,
                                 /*accumulate=*/true, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(g, e, "gx_rhs");
+    return GX_OK;
+}
+
+int gx_ssprk3_step(gx_grid* g, void* g_dev, double dt, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_dev || !(dt > 0)) return fail(g, GX_ERR_ARG, "gx_ssprk3_step: null pointer or dt <= 0");
+    if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_ssprk3_step: full geometry not set");
+    const size_t n = (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk;
+    int rc;
+    if (!g->drk_y) {
+        if ((rc = dev_alloc(g, &g->drk_y, n))) return rc;
+        if ((rc = dev_alloc(g, &g->drk_k, n))) return rc;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    float2* y0 = (float2*)g_dev;
+    const float h = (float)dt;
+    const int blocks = (int)std::min<size_t>((n + 255) / 256, 148 * 16);
+    if ((rc = gx_rhs(g, y0, g->drk_k, cuda_stream))) return rc;
+    gx::rk_stage_kernel<<<blocks, 256, 0, st>>>(g->drk_y, y0, y0, g->drk_k, 0.f, 1.f, h, n);              // g1
+    if ((rc = gx_rhs(g, g->drk_y, g->drk_k, cuda_stream))) return rc;
+    gx::rk_stage_kernel<<<blocks, 256, 0, st>>>(g->drk_y, y0, g->drk_y, g->drk_k, 0.75f, 0.25f, h, n);    // g2
+    if ((rc = gx_rhs(g, g->drk_y, g->drk_k, cuda_stream))) return rc;
+    gx::rk_stage_kernel<<<blocks, 256, 0, st>>>(y0, y0, g->drk_y, g->drk_k, 1.f / 3.f, 2.f / 3.f, h, n);  // g(t+dt)
+    GX_CUDA(g, cudaGetLastError());
     return GX_OK;
 }
 

@@ -411,4 +411,13 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
     return cudaGetLastError();
 }
 
+// SSP-RK3 stage combine: out = a*y0 + b*(y + dt*k), element-wise; out may alias y0 or y.
+__global__ void __launch_bounds__(256) rk_stage_kernel(float2* out, const float2* y0, const float2* y,
+                                                       const float2* k, float a, float b, float dt, size_t n) {
+    for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
+        const float2 u = y0[i], v = y[i], w = k[i];
+        out[i] = make_float2(fmaf(b, fmaf(dt, w.x, v.x), a * u.x), fmaf(b, fmaf(dt, w.y, v.y), a * u.y));
+    }
+}
+
 }  // namespace gx

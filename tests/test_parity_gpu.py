@@ -310,3 +310,25 @@ def test_full_rhs_parity(torch_cuda, name):
     lin = OL.rhs(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, tau_fac=cfg.tau_fac, nonlinear=False)
     assert O.relative_max_error(lin, ref) > 10 * TOL
     grid.close()
+
+
+def test_ssprk3_steps_parity(torch_cuda):
+    """two SSP-RK3 steps of gx_rhs on the tiny flux tube against the oracle's stepper."""
+    torch = torch_cuda
+    cfg = I.named_config("tiny")
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    grid = _grid(cfg, geo)
+    g = torch.from_numpy(G).cuda()
+    dt = 0.02
+    f = lambda y: OL.rhs(y, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, tau_fac=cfg.tau_fac)
+    ref = G.astype(np.complex128)
+    for _ in range(2):
+        grid.ssprk3_step(g, dt)
+        ref = OL.ssp_rk3_step(ref, dt, f)
+    torch.cuda.synchronize()
+    out = g.cpu().numpy()
+    assert np.all(np.isfinite(out))
+    assert O.relative_max_error(out, ref) <= TOL
+    assert O.relative_max_error(G, ref) > 100 * TOL          # the state really moved
+    grid.close()
