@@ -167,6 +167,54 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------- library reference point
+def cufft_composition(torch, cfg, grid, g, phi, ours, steps=20):
+    """The paper's own design for this step (batched cuFFT + cuBLAS for the Laguerre
+    matrices + pointwise kernels), composed from torch.fft (cuFFT) and torch.einsum (cuBLAS) on the same
+    tables and inputs.  A reference point on the same GPU, not part of the product path.
+    -> (evals/s, max-norm relative difference to `ours`)."""
+    from paper_2209_06731_b200 import binding as B
+    dev = g.device
+    Ns, Nm, Nl, Nz, nakx, naky = cfg.g_shape
+    nj, Nx, Ny = cfg.nj, cfg.Nx, cfg.Ny
+    T, Tinv, M = B.gx_export_tables(grid.h, Nl, Ns * Nz * nj * nakx * naky)
+    Tt = torch.from_numpy(T).to(dev).to(torch.complex64)
+    Ti = torch.from_numpy(Tinv).to(dev).to(torch.complex64)
+    Mt = torch.from_numpy(M.reshape(Ns, Nz, nj, nakx, naky)).to(dev)
+    K = (nakx - 1) // 2
+    kxi = torch.tensor([i if i <= K else i - nakx for i in range(nakx)], device=dev)
+    rows = torch.where(kxi >= 0, kxi, kxi + Nx)
+    ikx = (1j * cfg.dkx * kxi.to(torch.float32)).to(torch.complex64)[:, None]
+    iky = (1j * cfg.dky * torch.arange(naky, device=dev, dtype=torch.float32)).to(torch.complex64)[None, :]
+    Nyc = Ny // 2 + 1
+
+    def to_real(f):
+        pad = torch.zeros(f.shape[:-2] + (Nx, Nyc), dtype=torch.complex64, device=dev)
+        pad[..., rows, :naky] = f
+        return torch.fft.irfft2(pad, s=(Nx, Ny), norm="forward")
+
+    def step():
+        chi = Mt * phi[None, :, None]                                    # [s][z][j][kx][ky]
+        gt = torch.einsum("jl,smlzxy->smzjxy", Tt, g)
+        dxc, dyc = to_real(ikx * chi)[:, None], to_real(iky * chi)[:, None]
+        br = dyc * to_real(ikx * gt) - dxc * to_real(iky * gt)
+        bh = torch.fft.rfft2(br, norm="forward")[..., rows, :naky]
+        return -torch.einsum("lj,smzjxy->smlzxy", Ti, bh)
+
+    out = step()
+    err = float((out - ours).abs().max() / ours.abs().max())
+    for _ in range(2):
+        step()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(steps):
+        step()
+    e1.record()
+    torch.cuda.synchronize()
+    return steps / (e0.elapsed_time(e1) * 1e-3), err
+
+
 # ------------------------------------------------------------------------------- GPU leg
 def run_gpu(args):
     import torch
@@ -249,6 +297,36 @@ def run_gpu(args):
     e2e_sec = time.perf_counter() - t0
     e2e_value, _ = D.aggregate_throughput(float(e2e_steps), e2e_sec, device=dev)
 
+    # the mandated full right-hand side and the SSP-RK3 step, same inputs
+    def timed(fn, n):
+        for _ in range(3):
+            fn(0)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record()
+        for i in range(n):
+            fn(i)
+        b.record()
+        torch.cuda.synchronize()
+        return n / (a.elapsed_time(b) * 1e-3)
+
+    n_aux = max(3, min(args.steps, 200))
+    rhs_rate = timed(lambda i: grid.rhs(gs[i % nsets], outs[i % nsets]), n_aux)
+    g_rk = gs[0].clone()
+    g_rk.mul_(1e-3)                       # small amplitude: 3*n_aux explicit steps at dt=1e-3 stay finite
+    rk_rate = timed(lambda i: grid.ssprk3_step(g_rk, 1e-3), max(3, n_aux // 3))
+    assert torch.isfinite(g_rk.real).all()
+    ref_point = None
+    if rank == 0 and not args.skip_reference_point and g_elems <= 8_000_000:
+        grid.nonlinear_rhs(gs[0], phis[0], outs[0])
+        torch.cuda.synchronize()
+        try:
+            rv, rerr = cufft_composition(torch, cfg, grid, gs[0], phis[0], outs[0])
+            ref_point = {"kind": "cuFFT + cuBLAS composition of the same step (torch.fft / torch.einsum), same GPU",
+                         "value": rv, "unit": UNIT, "rel_diff_to_ours": rerr}
+        except Exception as e:                                  # library leg only; never affects the product numbers
+            ref_point = {"kind": "cuFFT + cuBLAS composition", "error": repr(e)[:200]}
+
     line = None
     if rank == 0:
         peaks = {}
@@ -297,6 +375,10 @@ def run_gpu(args):
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (g_elems + int(np.prod(cfg.phi_shape))) * 8,
                         "d2h_bytes_per_step": g_elems * 8, "steps": e2e_steps},
                 "gpu_launches": launches_per_call * args.steps,
+                "kernel_family": os.environ.get("GX_KERNELS", "scalar"),
+                "gx_rhs": {"value": rhs_rate * world, "unit": "full rhs evals/s (field solve + nonlinear + linear)"},
+                "ssprk3": {"value": rk_rate * world, "unit": "SSP-RK3 steps/s (3 gx_rhs each)"},
+                "reference_point": ref_point,
                 "roofline": roofline,
                 "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
                                  "sample": cpu_sample}}
@@ -314,6 +396,7 @@ def main():
     ap.add_argument("--config", default="cyclone", choices=I.CONFIG_NAMES + ["w7x-shape"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="omit the oracle timing (ncu passes)")
+    ap.add_argument("--skip-reference-point", action="store_true", help="omit the cuFFT+cuBLAS composition")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
