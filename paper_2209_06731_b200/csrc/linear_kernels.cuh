@@ -74,6 +74,10 @@ inline bool lin_upload(T** dst, const std::vector<T>& src, size_t& bytes, std::s
 
 inline bool lin_tables_build(const LinHostInput& in, LinTables& t, size_t& bytes, std::string& msg) {
     if ((int)in.species.size() > kMaxSpecies) { msg = "at most 4 species"; return false; }
+    if ((double)in.Ns * in.Nm * in.Nl * in.Nz * in.nakx * in.naky >= 2147483648.0) {
+        msg = "linear kernels index the state with 32 bits: more than 2^31 coefficients";
+        return false;
+    }
     const int Nz = in.Nz, Nl = in.Nl, Ns = in.Ns, nakx = in.nakx, naky = in.naky;
     const size_t nk = (size_t)nakx * naky;
     const int K = (nakx - 1) / 2;
@@ -195,19 +199,25 @@ __global__ void __launch_bounds__(256) field_solve_kernel(LinTables t, const flo
     phi[(size_t)z * t.nk + k] = (k == 0) ? make_float2(0.f, 0.f) : make_float2(num.x * d, num.y * d);
 }
 
-// adiabatic electrons, ky = 0 rows: phi += fsfac[kx] * <<phi_raw>>_z * invD   (Eq. 6.1 solved for <<phi>>)
-__global__ void __launch_bounds__(128) flux_surface_kernel(LinTables t, float2* __restrict__ phi) {
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;    // kx row
-    if (i >= t.nakx || i == 0) return;
+// adiabatic electrons, ky = 0 rows: phi += fsfac[kx] * <<phi_raw>>_z * invD   (Eq. 6.1 solved for <<phi>>).
+// One warp per kx row; lanes stride over z and reduce by shuffle.
+__global__ void __launch_bounds__(32) flux_surface_kernel(LinTables t, float2* __restrict__ phi) {
+    const int i = blockIdx.x + 1;                           // kx row; row 0 (kx = 0) keeps phi(0,0) = 0
+    if (i >= t.nakx) return;
     const size_t col = (size_t)i * t.naky;
     float2 avg = make_float2(0.f, 0.f);
-    for (int z = 0; z < t.Nz; ++z) {
+    for (int z = threadIdx.x; z < t.Nz; z += 32) {
         const float2 f = phi[(size_t)z * t.nk + col];
         avg.x = fmaf(t.wz[z], f.x, avg.x);
         avg.y = fmaf(t.wz[z], f.y, avg.y);
     }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        avg.x += __shfl_xor_sync(0xffffffffu, avg.x, o);
+        avg.y += __shfl_xor_sync(0xffffffffu, avg.y, o);
+    }
     const float fs = t.fsfac[i];
-    for (int z = 0; z < t.Nz; ++z) {
+    for (int z = threadIdx.x; z < t.Nz; z += 32) {
         const float d = t.invD[(size_t)z * t.nk + col] * fs;
         float2 f = phi[(size_t)z * t.nk + col];
         f.x = fmaf(d, avg.x, f.x);
@@ -220,7 +230,7 @@ inline cudaError_t lin_field_solve(const LinTables& t, const float2* g, float2* 
     if (!t.built) return cudaErrorNotReady;
     dim3 grid((t.nk + 255) / 256, t.Nz);
     field_solve_kernel<<<grid, 256, 0, st>>>(t, g, phi);
-    if (t.adiabatic) flux_surface_kernel<<<(t.nakx + 127) / 128, 128, 0, st>>>(t, phi);
+    if (t.adiabatic && t.nakx > 1) flux_surface_kernel<<<t.nakx - 1, 32, 0, st>>>(t, phi);
     return cudaGetLastError();
 }
 
@@ -231,17 +241,18 @@ inline cudaError_t lin_field_solve(const LinTables& t, const float2* g, float2* 
 __device__ __forceinline__ float2 lin_H(const LinTables& t, const float2* __restrict__ g, const float2* __restrict__ phi,
                                         int s, int l, int m, int z, int k) {
     if (l < 0 || l >= t.Nl || m < 0 || m >= t.Nm) return make_float2(0.f, 0.f);
-    float2 h = g[((((size_t)s * t.Nm + m) * t.Nl + l) * t.Nz + z) * t.nk + k];
+    const unsigned zk = (unsigned)(z * t.nk + k), pl = (unsigned)(t.Nz * t.nk);   // < 2^31 elements (checked at build)
+    float2 h = g[(unsigned)((s * t.Nm + m) * t.Nl + l) * pl + zk];
     if (m == 0) {
-        const float c = t.zt[s] * t.Jl[(((size_t)s * t.Nl + l) * t.Nz + z) * t.nk + k];
-        const float2 f = phi[(size_t)z * t.nk + k];
+        const float c = t.zt[s] * t.Jl[(unsigned)(s * t.Nl + l) * pl + zk];
+        const float2 f = phi[zk];
         h.x = fmaf(c, f.x, h.x);
         h.y = fmaf(c, f.y, h.y);
     }
     return h;
 }
 __device__ __forceinline__ float lin_J(const LinTables& t, int s, int l, int z, int k) {
-    return (l < 0 || l >= t.Nl) ? 0.f : t.Jl[(((size_t)s * t.Nl + l) * t.Nz + z) * t.nk + k];
+    return (l < 0 || l >= t.Nl) ? 0.f : t.Jl[(unsigned)(s * t.Nl + l) * (unsigned)(t.Nz * t.nk) + (unsigned)(z * t.nk + k)];
 }
 
 // field-particle moments of the Dougherty operator, Eq. 4.14-4.18: mom[s][0..2][z][k]
@@ -283,21 +294,25 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
     extern __shared__ __align__(16) unsigned char lin_smem[];
     float2* S1 = reinterpret_cast<float2*>(lin_smem);            // [Nz][TK] sqrt(m+1) H_{l,m+1} + sqrt(m) H_{l,m-1}
     float2* S2 = S1 + (size_t)t.Nz * kLinTK;                     // [Nz][TK] G_{l,m} (hyper-collisions)
-    float* dz = reinterpret_cast<float*>(S2 + (size_t)t.Nz * kLinTK);
-    float* az = dz + t.Nz;
+    float* dz = reinterpret_cast<float*>(S2 + (size_t)t.Nz * kLinTK);   // [2 Nz] column repeated: no wrap test
+    float* az = dz + 2 * t.Nz;
     const int tk = threadIdx.x % kLinTK, zg = threadIdx.x / kLinTK;
     const int k = blockIdx.x * kLinTK + tk;
     const int l = blockIdx.y;
     const int s = blockIdx.z / t.Nm, m = blockIdx.z % t.Nm;
     const bool live = k < t.nk;
     const float sm1 = sqrtf((float)(m + 1)), sm0 = sqrtf((float)m);
-    for (int i = threadIdx.x; i < t.Nz; i += blockDim.x) { dz[i] = t.Dz[i]; az[i] = t.Az[i]; }
+    for (int i = threadIdx.x; i < 2 * t.Nz; i += blockDim.x) {
+        const int d = i < t.Nz ? i : i - t.Nz;
+        dz[i] = t.Dz[d];
+        az[i] = t.Az[d];
+    }
     for (int z = zg; z < t.Nz; z += kLinZG) {
         float2 c = make_float2(0.f, 0.f), gg = c;
         if (live) {
             const float2 hp = lin_H(t, g, phi, s, l, m + 1, z, k), hm = lin_H(t, g, phi, s, l, m - 1, z, k);
             c = make_float2(sm1 * hp.x + sm0 * hm.x, sm1 * hp.y + sm0 * hm.y);
-            gg = g[((((size_t)s * t.Nm + m) * t.Nl + l) * t.Nz + z) * t.nk + k];
+            gg = g[(unsigned)((s * t.Nm + m) * t.Nl + l) * (unsigned)(t.Nz * t.nk) + (unsigned)(z * t.nk + k)];
         }
         S1[z * kLinTK + tk] = c;
         S2[z * kLinTK + tk] = gg;
@@ -311,14 +326,24 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
     for (int z = zg; z < t.Nz; z += kLinZG) {
         // streaming: -v_t grad_par(...)   and hyper-collisions: -nu_hyp m^p |k_par| G
         float2 dp = make_float2(0.f, 0.f), ap = dp;
-        for (int zp = 0; zp < t.Nz; ++zp) {
-            int d = z - zp;
-            d += d < 0 ? t.Nz : 0;
-            const float2 a = S1[zp * kLinTK + tk];
-            dp.x = fmaf(dz[d], a.x, dp.x); dp.y = fmaf(dz[d], a.y, dp.y);
+        {
+            const float* __restrict__ dcol = dz + z + t.Nz;          // dcol[-zp] = D[(z - zp) mod Nz]
+            const float2* __restrict__ s1 = S1 + tk;
+#pragma unroll 4
+            for (int zp = 0; zp < t.Nz; ++zp) {
+                const float w = dcol[-zp];
+                const float2 a = s1[zp * kLinTK];
+                dp.x = fmaf(w, a.x, dp.x); dp.y = fmaf(w, a.y, dp.y);
+            }
             if (hyp != 0.f) {
-                const float2 b2 = S2[zp * kLinTK + tk];
-                ap.x = fmaf(az[d], b2.x, ap.x); ap.y = fmaf(az[d], b2.y, ap.y);
+                const float* __restrict__ acol = az + z + t.Nz;
+                const float2* __restrict__ s2 = S2 + tk;
+#pragma unroll 4
+                for (int zp = 0; zp < t.Nz; ++zp) {
+                    const float w = acol[-zp];
+                    const float2 b2 = s2[zp * kLinTK];
+                    ap.x = fmaf(w, b2.x, ap.x); ap.y = fmaf(w, b2.y, ap.y);
+                }
             }
         }
         float2 r = make_float2(-vt * dp.x - hyp * ap.x, -vt * dp.y - hyp * ap.y);
@@ -384,7 +409,7 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
             r.x -= hv * gg.x;
             r.y -= hv * gg.y;
         }
-        float2* __restrict__ o = out + ((((size_t)s * t.Nm + m) * t.Nl + l) * t.Nz + z) * t.nk + k;
+        float2* __restrict__ o = out + ((unsigned)((s * t.Nm + m) * t.Nl + l) * (unsigned)(t.Nz * t.nk) + (unsigned)(z * t.nk + k));
         if (ACC) { const float2 prev = *o; r.x += prev.x; r.y += prev.y; }
         *o = r;
     }
@@ -397,7 +422,7 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
         dim3 gm((t.nk + 255) / 256, t.Nz, t.Ns);
         lin_moments_kernel<<<gm, 256, 0, st>>>(t, g, phi);
     }
-    const size_t smem = (size_t)t.Nz * kLinTK * sizeof(float2) * 2 + 2 * (size_t)t.Nz * sizeof(float);
+    const size_t smem = (size_t)t.Nz * kLinTK * sizeof(float2) * 2 + 4 * (size_t)t.Nz * sizeof(float);
     static bool attr = false;
     if (!attr) {
         cudaError_t e = cudaFuncSetAttribute(lin_rhs_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
