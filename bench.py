@@ -313,8 +313,10 @@ def run_gpu(args):
     n_aux = max(3, min(args.steps, 200))
     rhs_rate = timed(lambda i: grid.rhs(gs[i % nsets], outs[i % nsets]), n_aux)
     g_rk = gs[0].clone()
-    g_rk.mul_(1e-3)                       # small amplitude: 3*n_aux explicit steps at dt=1e-3 stay finite
-    rk_rate = timed(lambda i: grid.ssprk3_step(g_rk, 1e-3), max(3, n_aux // 3))
+    g_rk.mul_(1e-3)                       # small amplitude; dt from the parallel-streaming CFL (Eq. 5.5)
+    vt_max = max(np.sqrt(sp.temp / sp.mass) for sp in cfg.species)
+    dt_rk = 0.2 / (vt_max * abs(float(geo["gradpar"])) * (cfg.Nz / 2) * np.sqrt(2.0 * cfg.Nm) + 10.0)
+    rk_rate = timed(lambda i: grid.ssprk3_step(g_rk, dt_rk), max(3, n_aux // 3))
     assert torch.isfinite(g_rk.real).all()
     ref_point = None
     if rank == 0 and not args.skip_reference_point and g_elems <= 8_000_000:

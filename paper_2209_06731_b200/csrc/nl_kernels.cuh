@@ -523,11 +523,10 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
     // ---- a6 (x part) + a7 (keep |kx| <= K)
     x_forward<C>(W, twx, p.bhat + (size_t)unit * NK, p.scale);
 
-    // ---- publish: this node's Bhat plane is complete (release: stores -> fence -> barrier -> atomic).
+    // ---- publish: this node's Bhat plane is complete (release: stores -> barrier -> fence -> atomic).
     // The inverse-Laguerre grid, already resident under PDL, waits per (s,m,z) on this counter.
-    __threadfence();
-    __syncthreads();
-    if (threadIdx.x == 0) atomicAdd(p.count + (s * p.Nm + m) * p.Nz + z, 1u);
+    __syncthreads();                 // orders every thread's stores before thread 0's gpu-scope fence (cumulative)
+    if (threadIdx.x == 0) { __threadfence(); atomicAdd(p.count + (s * p.Nm + m) * p.Nz + z, 1u); }
 }
 
 // ================================================================================================
