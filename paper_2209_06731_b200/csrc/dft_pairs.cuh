@@ -69,9 +69,9 @@ template <int N, int S> __device__ __forceinline__ c2 twiddle2(c2 v, int t) {
     return cmul_s(v, c, s);
 }
 
-template <int N, int S, unsigned ZM = 0u> struct Dft2;
+template <int N, int S, zm_t ZM = 0ull> struct Dft2;
 
-template <int S, unsigned ZM> struct Dft2<2, S, ZM> {
+template <int S, zm_t ZM> struct Dft2<2, S, ZM> {
     __device__ __forceinline__ static void run(c2 (&v)[2]) {
         constexpr bool z0 = ZM & 1u, z1 = ZM & 2u;
         const c2 a = v[0], b = v[1];
@@ -81,7 +81,7 @@ template <int S, unsigned ZM> struct Dft2<2, S, ZM> {
     }
 };
 
-template <int S, unsigned ZM> struct Dft2<3, S, ZM> {
+template <int S, zm_t ZM> struct Dft2<3, S, ZM> {
     __device__ __forceinline__ static void run(c2 (&v)[3]) {
         const c2 t = cadd(v[1], v[2]);
         const c2 d = csub(v[1], v[2]);
@@ -96,7 +96,7 @@ template <int S, unsigned ZM> struct Dft2<3, S, ZM> {
     }
 };
 
-template <int S, unsigned ZM> struct Dft2<4, S, ZM> {
+template <int S, zm_t ZM> struct Dft2<4, S, ZM> {
     __device__ __forceinline__ static void run(c2 (&v)[4]) {
         constexpr bool z0 = ZM & 1u, z1 = ZM & 2u, z2 = ZM & 4u, z3 = ZM & 8u;
         c2 a, b, c, d;                                    // a = v0+v2, b = v0-v2, c = v1+v3, d = v1-v3
@@ -112,7 +112,7 @@ template <int S, unsigned ZM> struct Dft2<4, S, ZM> {
     }
 };
 
-template <int N, int A, int B, int S, unsigned ZM, int n2>
+template <int N, int A, int B, int S, zm_t ZM, int n2>
 __device__ __forceinline__ void dft2_split_col(const c2 (&v)[N], c2 (&y)[N]) {
     c2 t[A];
 #pragma unroll
@@ -123,7 +123,7 @@ __device__ __forceinline__ void dft2_split_col(const c2 (&v)[N], c2 (&y)[N]) {
     if constexpr (n2 + 1 < B) dft2_split_col<N, A, B, S, ZM, n2 + 1>(v, y);
 }
 
-template <int N, int A, int B, int S, unsigned ZM = 0u> __device__ __forceinline__ void dft2_split(c2 (&v)[N]) {
+template <int N, int A, int B, int S, zm_t ZM = 0ull> __device__ __forceinline__ void dft2_split(c2 (&v)[N]) {
     static_assert(A * B == N, "bad split");
     c2 y[N];
     dft2_split_col<N, A, B, S, ZM, 0>(v, y);
@@ -138,19 +138,19 @@ template <int N, int A, int B, int S, unsigned ZM = 0u> __device__ __forceinline
     }
 }
 
-template <int S, unsigned ZM> struct Dft2<6, S, ZM> {
+template <int S, zm_t ZM> struct Dft2<6, S, ZM> {
     __device__ __forceinline__ static void run(c2 (&v)[6]) { dft2_split<6, 2, 3, S, ZM>(v); }
 };
-template <int S, unsigned ZM> struct Dft2<8, S, ZM> {
+template <int S, zm_t ZM> struct Dft2<8, S, ZM> {
     __device__ __forceinline__ static void run(c2 (&v)[8]) { dft2_split<8, 2, 4, S, ZM>(v); }
 };
-template <int S, unsigned ZM> struct Dft2<12, S, ZM> {
+template <int S, zm_t ZM> struct Dft2<12, S, ZM> {
     __device__ __forceinline__ static void run(c2 (&v)[12]) { dft2_split<12, 3, 4, S, ZM>(v); }
 };
-template <int S, unsigned ZM> struct Dft2<16, S, ZM> {
+template <int S, zm_t ZM> struct Dft2<16, S, ZM> {
     __device__ __forceinline__ static void run(c2 (&v)[16]) { dft2_split<16, 4, 4, S, ZM>(v); }
 };
 
-template <int N, int S, unsigned ZM = 0u> __device__ __forceinline__ void dft2(c2 (&v)[N]) { Dft2<N, S, ZM>::run(v); }
+template <int N, int S, zm_t ZM = 0ull> __device__ __forceinline__ void dft2(c2 (&v)[N]) { Dft2<N, S, ZM>::run(v); }
 
 }  // namespace gx

@@ -23,50 +23,62 @@ template <int S> __device__ __forceinline__ float2 mul_i(float2 a) {
     return S > 0 ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
 }
 
-// cos(2 pi t / 48), t = 0..47, fp64 values rounded to fp32 at compile time.
-__host__ __device__ constexpr double cos48(int t) {
-    constexpr double C[13] = {1.0,
-                              0.99144486137381041114, 0.96592582628906828675, 0.92387953251128675613,
-                              0.86602540378443864676, 0.79335334029123516458, 0.70710678118654752440,
-                              0.60876142900872063942, 0.5,
-                              0.38268343236508977173, 0.25881904510252076235, 0.13052619222005159155,
-                              0.0};
-    t = ((t % 48) + 48) % 48;
-    if (t > 24) t = 48 - t;          // cos(-a) = cos(a)
-    return t <= 12 ? C[t] : -C[24 - t];
+// cos(2 pi t / 192), t = 0..191, from a quarter-wave table of fp64 values (rounded to fp32 at use).
+// 192 = lcm(48, 64): covers every twiddle of the radices 2..16 (N | 48) and of the 32- and 64-point
+// single-thread transforms.
+__host__ __device__ constexpr double cos192(int t) {
+    constexpr double C[49] = {
+        1.00000000000000000000, 0.99946458747636568454, 0.99785892323860347908, 0.99518472667219692873,
+        0.99144486137381038215, 0.98664333208487897675, 0.98078528040323043058, 0.97387697927733363201,
+        0.96592582628906831221, 0.95694033573220882438, 0.94693012949510568799, 0.93590592675732575678,
+        0.92387953251128673848, 0.91086382492117579091, 0.89687274153268836674, 0.88192126434835504956,
+        0.86602540378443870761, 0.84920218152657889199, 0.83146961230254523567, 0.81284668459161524279,
+        0.79335334029123516508, 0.77301045336273699338, 0.75183980747897738439, 0.72986407269783570850,
+        0.70710678118654757274, 0.68359230202287124545, 0.65934581510006884386, 0.63439328416364548779,
+        0.60876142900872065589, 0.58247769686780215270, 0.55557023301960239969, 0.52806785065036809801,
+        0.50000000000000011102, 0.47139673682599758653, 0.44228869021900124592, 0.41270702980439472052,
+        0.38268343236508983729, 0.35225004792123359998, 0.32143946530316169774, 0.29028467725446249759,
+        0.25881904510252073948, 0.22707626303437344895, 0.19509032201612833135, 0.16289547339458881892,
+        0.13052619222005171218, 0.09801714032956054812, 0.06540312923014326985, 0.03271908282177616450,
+        0.00000000000000000000};
+    t = ((t % 192) + 192) % 192;
+    if (t > 96) t = 192 - t;         // cos(-a) = cos(a)
+    return t <= 48 ? C[t] : -C[96 - t];
 }
-__host__ __device__ constexpr double sin48(int t) { return cos48(t - 12); }
+__host__ __device__ constexpr double sin192(int t) { return cos192(t - 48); }
+__host__ __device__ constexpr double cos48(int t) { return cos192(4 * t); }
+__host__ __device__ constexpr double sin48(int t) { return sin192(4 * t); }
 
 // v *= e^{S 2 pi i t / N} with t, N compile-time after unrolling; trivial cases cost no multiply.
 template <int N, int S> __device__ __forceinline__ float2 twiddle(float2 v, int t) {
-    static_assert(48 % N == 0, "N must divide 48");
-    const int a = ((t * (48 / N)) % 48 + 48) % 48;
+    static_assert(192 % N == 0, "N must divide 192");
+    const int a = ((t * (192 / N)) % 192 + 192) % 192;
     if (a == 0) return v;
-    if (a == 12) return mul_i<S>(v);
-    if (a == 24) return make_float2(-v.x, -v.y);
-    if (a == 36) return mul_i<-S>(v);
-    if (a % 12 == 6) {               // (+-1 +- i)/sqrt(2): two adds, two multiplies
+    if (a == 48) return mul_i<S>(v);
+    if (a == 96) return make_float2(-v.x, -v.y);
+    if (a == 144) return mul_i<-S>(v);
+    if (a % 48 == 24) {               // (+-1 +- i)/sqrt(2): two adds, two multiplies
         const float h = 0.70710678118654752440f;
-        const float cr = (a == 6 || a == 42) ? h : -h;
-        const float ci = ((a == 6 || a == 18) ? h : -h) * (S > 0 ? 1.f : -1.f);
-        // (x+iy)(cr+ici): |cr| = |ci| = h
+        const float cr = (a == 24 || a == 168) ? h : -h;
+        const float ci = ((a == 24 || a == 72) ? h : -h) * (S > 0 ? 1.f : -1.f);
         const float p = v.x * h, q = v.y * h;
         const float sr = cr > 0 ? 1.f : -1.f, si = ci > 0 ? 1.f : -1.f;
         return make_float2(sr * p - si * q, si * p + sr * q);
     }
-    const float c = (float)cos48(a);
-    const float s = (float)sin48(a) * (S > 0 ? 1.f : -1.f);
+    const float c = (float)cos192(a);
+    const float s = (float)sin192(a) * (S > 0 ? 1.f : -1.f);
     return make_float2(fmaf(-v.y, s, v.x * c), fmaf(v.x, s, v.y * c));
 }
 
 // ZM: bit n set <=> input v[n] is known to be zero at compile time (2/3-rule padding).  The IEEE rules
 // forbid the compiler from folding x + 0 (sign of zero), so the base cases skip those adds explicitly;
 // a size that ignores ZM is still correct because the masked inputs really hold 0.
-template <int N, int S, unsigned ZM = 0u> struct Dft;
+typedef unsigned long long zm_t;
+template <int N, int S, zm_t ZM = 0ull> struct Dft;
 
 __device__ __forceinline__ float2 cneg(float2 a) { return make_float2(-a.x, -a.y); }
 
-template <int S, unsigned ZM> struct Dft<2, S, ZM> {
+template <int S, zm_t ZM> struct Dft<2, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[2]) {
         constexpr bool z0 = ZM & 1u, z1 = ZM & 2u;
         const float2 a = v[0], b = v[1];
@@ -76,7 +88,7 @@ template <int S, unsigned ZM> struct Dft<2, S, ZM> {
     }
 };
 
-template <int S, unsigned ZM> struct Dft<3, S, ZM> {
+template <int S, zm_t ZM> struct Dft<3, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[3]) {
         const float2 t = cadd(v[1], v[2]);
         const float2 d = csub(v[1], v[2]);
@@ -89,7 +101,7 @@ template <int S, unsigned ZM> struct Dft<3, S, ZM> {
     }
 };
 
-template <int S, unsigned ZM> struct Dft<4, S, ZM> {
+template <int S, zm_t ZM> struct Dft<4, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[4]) {
         constexpr bool z0 = ZM & 1u, z1 = ZM & 2u, z2 = ZM & 4u, z3 = ZM & 8u;
         float2 a, b, c, d;                                    // a = v0+v2, b = v0-v2, c = v1+v3, d = v1-v3
@@ -107,24 +119,24 @@ template <int S, unsigned ZM> struct Dft<4, S, ZM> {
 };
 
 // One Cooley-Tukey split N = A*B:  n = n1*B + n2,  k = k1 + A*k2.
-template <int A, int B, unsigned ZM, int n2> __host__ __device__ constexpr unsigned sub_mask_first() {
-    unsigned m = 0;
+template <int A, int B, zm_t ZM, int n2> __host__ __device__ constexpr zm_t sub_mask_first() {
+    zm_t m = 0;
     for (int n1 = 0; n1 < A; ++n1)
-        if (ZM & (1u << (n1 * B + n2))) m |= 1u << n1;
+        if (ZM & (1ull << (n1 * B + n2))) m |= 1ull << n1;
     return m;
 }
-template <int A, int B, unsigned ZM> __host__ __device__ constexpr unsigned sub_mask_second() {   // column n2 entirely zero
-    unsigned m = 0;
+template <int A, int B, zm_t ZM> __host__ __device__ constexpr zm_t sub_mask_second() {   // column n2 entirely zero
+    zm_t m = 0;
     for (int n2 = 0; n2 < B; ++n2) {
         bool all = true;
         for (int n1 = 0; n1 < A; ++n1)
-            if (!(ZM & (1u << (n1 * B + n2)))) all = false;
-        if (all) m |= 1u << n2;
+            if (!(ZM & (1ull << (n1 * B + n2)))) all = false;
+        if (all) m |= 1ull << n2;
     }
     return m;
 }
 
-template <int N, int A, int B, int S, unsigned ZM, int n2>
+template <int N, int A, int B, int S, zm_t ZM, int n2>
 __device__ __forceinline__ void dft_split_col(const float2 (&v)[N], float2 (&y)[N]) {
     float2 t[A];
 #pragma unroll
@@ -135,7 +147,7 @@ __device__ __forceinline__ void dft_split_col(const float2 (&v)[N], float2 (&y)[
     if constexpr (n2 + 1 < B) dft_split_col<N, A, B, S, ZM, n2 + 1>(v, y);
 }
 
-template <int N, int A, int B, int S, unsigned ZM = 0u> __device__ __forceinline__ void dft_split(float2 (&v)[N]) {
+template <int N, int A, int B, int S, zm_t ZM = 0ull> __device__ __forceinline__ void dft_split(float2 (&v)[N]) {
     static_assert(A * B == N, "bad split");
     float2 y[N];
     dft_split_col<N, A, B, S, ZM, 0>(v, y);
@@ -150,19 +162,26 @@ template <int N, int A, int B, int S, unsigned ZM = 0u> __device__ __forceinline
     }
 }
 
-template <int S, unsigned ZM> struct Dft<6, S, ZM> {
+template <int S, zm_t ZM> struct Dft<6, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[6]) { dft_split<6, 2, 3, S, ZM>(v); }
 };
-template <int S, unsigned ZM> struct Dft<8, S, ZM> {
+template <int S, zm_t ZM> struct Dft<8, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[8]) { dft_split<8, 2, 4, S, ZM>(v); }
 };
-template <int S, unsigned ZM> struct Dft<12, S, ZM> {
+template <int S, zm_t ZM> struct Dft<12, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[12]) { dft_split<12, 3, 4, S, ZM>(v); }
 };
-template <int S, unsigned ZM> struct Dft<16, S, ZM> {
+template <int S, zm_t ZM> struct Dft<16, S, ZM> {
     __device__ __forceinline__ static void run(float2 (&v)[16]) { dft_split<16, 4, 4, S, ZM>(v); }
 };
 
-template <int N, int S, unsigned ZM = 0u> __device__ __forceinline__ void dft(float2 (&v)[N]) { Dft<N, S, ZM>::run(v); }
+template <int S, zm_t ZM> struct Dft<32, S, ZM> {
+    __device__ __forceinline__ static void run(float2 (&v)[32]) { dft_split<32, 4, 8, S, ZM>(v); }
+};
+template <int S, zm_t ZM> struct Dft<64, S, ZM> {
+    __device__ __forceinline__ static void run(float2 (&v)[64]) { dft_split<64, 8, 8, S, ZM>(v); }
+};
+
+template <int N, int S, zm_t ZM = 0ull> __device__ __forceinline__ void dft(float2 (&v)[N]) { Dft<N, S, ZM>::run(v); }
 
 }  // namespace gx

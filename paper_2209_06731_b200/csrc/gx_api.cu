@@ -14,6 +14,7 @@
 #include "linear_kernels.cuh"
 #include "nl_kernels.cuh"
 #include "nl_pair_kernels.cuh"
+#include "nl_row_kernels.cuh"
 
 namespace {
 
@@ -113,6 +114,32 @@ template <class CB, class CC> constexpr KernelSet make_persist_set() {
                   "chi and bracket kernels must share the transform radices (same permuted real-space order)");
     return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, CB::MAXL, &launch_chi_pair_t<CC>, &launch_bracket_persist_t<CB>};
 }
+template <class C> cudaError_t launch_chi_row_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_row_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    gx::chi_planes_row_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
+    return cudaGetLastError();
+}
+template <class C> cudaError_t launch_bracket_row_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::bracket_row_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    return launch_pdl(gx::bracket_row_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
+}
+template <class CB, class CC> constexpr KernelSet make_row_set() {
+    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1,
+                  "chi and bracket kernels must share the x radices (same permuted x order)");
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, &launch_chi_row_t<CC>, &launch_bracket_row_t<CB>};
+}
 template <class CB, class CC> constexpr KernelSet make_pair_set() {
     static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
                   "chi and bracket kernels must share the transform radices (same permuted real-space order)");
@@ -170,6 +197,20 @@ using PC192x64 = gx::PairCfg<192, 64, 16, 12, 8, 8, 64, GX_PC_NT, 1>;
 using P256x96  = gx::PairCfg<256, 96, 16, 16, 8, 12, 32, 256, 1>;
 using P64x192  = gx::PairCfg<64, 192, 8, 8, 12, 16, 32, 128, 1>;
 
+// row family (nl_row_kernels.cuh): whole y direction of an x row in one thread's registers; NY = 64 only
+#ifndef GX_ROW_NT
+#define GX_ROW_NT 192
+#endif
+#ifndef GX_ROW_MINB
+#define GX_ROW_MINB 2
+#endif
+using R64x64   = gx::RowCfg<64, 64, 8, 8, 64, 2>;
+using R128x64  = gx::RowCfg<128, 64, 16, 8, 128, 2>;
+using R192x64  = gx::RowCfg<192, 64, 16, 12, GX_ROW_NT, GX_ROW_MINB>;
+const KernelSet kRowSets[] = {
+    make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, R192x64>(),
+};
+
 #ifndef GX_PS_NW
 #define GX_PS_NW 12
 #endif
@@ -194,6 +235,9 @@ const KernelSet* find_set(int Nx, int Ny, int Nl) {
     if (fam && std::strcmp(fam, "persist") == 0)
         for (const auto& k : kPersistSets)
             if (k.Nx == Nx && k.Ny == Ny && Nl <= k.max_nl) return &k;
+    if (fam && std::strcmp(fam, "row") == 0)
+        for (const auto& k : kRowSets)
+            if (k.Nx == Nx && k.Ny == Ny) return &k;
     if (fam && (std::strcmp(fam, "pair") == 0 || std::strcmp(fam, "persist") == 0))
         for (const auto& k : kPairSets)
             if (k.Nx == Nx && k.Ny == Ny) return &k;
