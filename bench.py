@@ -354,7 +354,7 @@ def run_gpu(args):
             traffic = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get(cfg.name, {}).get("bracket_kernel")
         except Exception:
             pass
-        roofline = {"bound": "alu", "kernel": "bracket_kernel", "achieved": achieved, "peak": peak_tflops,
+        roofline = {"bound": "alu", "kernel": "bracket kernel of the %s family" % B.FAMILY_NAMES.get(grid.query(B.GX_Q_KERNEL_FAMILY), "?"), "achieved": achieved, "peak": peak_tflops,
                     "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": traffic,
                     "peak_source": f"{n_sm} SMs x 128 FP32 lanes x 2 x {sm_max:.0f} MHz (max SM clock, MEASURED_PEAKS.json)",
                     "kernel_us": {"chi_planes": kern_us[0], "bracket": kern_us[1], "laguerre_inverse": kern_us[2]},
@@ -377,7 +377,7 @@ def run_gpu(args):
                 "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": (g_elems + int(np.prod(cfg.phi_shape))) * 8,
                         "d2h_bytes_per_step": g_elems * 8, "steps": e2e_steps},
                 "gpu_launches": launches_per_call * args.steps,
-                "kernel_family": os.environ.get("GX_KERNELS", "scalar"),
+                "kernel_family": B.FAMILY_NAMES.get(grid.query(B.GX_Q_KERNEL_FAMILY), "?"),
                 "gx_rhs": {"value": rhs_rate * world, "unit": "full rhs evals/s (field solve + nonlinear + linear)"},
                 "ssprk3": {"value": rk_rate * world, "unit": "SSP-RK3 steps/s (3 gx_rhs each)"},
                 "reference_point": ref_point,

@@ -30,6 +30,7 @@ struct KernelSet {
     int Nx, Ny;
     int smem_bytes;
     int max_nl;          // 0: any Nl; else the set needs Nl <= max_nl (all Laguerre planes staged at once)
+    int family;          // GX_FAMILY_* of include/gx.h
     cudaError_t (*launch_chi)(const NlParams&, int units, cudaStream_t);
     cudaError_t (*launch_bracket)(const NlParams&, int units, cudaStream_t);
 };
@@ -112,7 +113,7 @@ template <class C> cudaError_t launch_bracket_persist_t(const NlParams& p, int u
 template <class CB, class CC> constexpr KernelSet make_persist_set() {
     static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
                   "chi and bracket kernels must share the transform radices (same permuted real-space order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, CB::MAXL, &launch_chi_pair_t<CC>, &launch_bracket_persist_t<CB>};
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, CB::MAXL, GX_FAMILY_PERSIST, &launch_chi_pair_t<CC>, &launch_bracket_persist_t<CB>};
 }
 template <class C> cudaError_t launch_chi_row_t(const NlParams& p, int units, cudaStream_t st) {
     static bool attr = false;
@@ -138,17 +139,17 @@ template <class C> cudaError_t launch_bracket_row_t(const NlParams& p, int units
 template <class CB, class CC> constexpr KernelSet make_row_set() {
     static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1,
                   "chi and bracket kernels must share the x radices (same permuted x order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, &launch_chi_row_t<CC>, &launch_bracket_row_t<CB>};
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_ROW, &launch_chi_row_t<CC>, &launch_bracket_row_t<CB>};
 }
 template <class CB, class CC> constexpr KernelSet make_pair_set() {
     static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
                   "chi and bracket kernels must share the transform radices (same permuted real-space order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, &launch_chi_pair_t<CC>, &launch_bracket_pair_t<CB>};
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_PAIR, &launch_chi_pair_t<CC>, &launch_bracket_pair_t<CB>};
 }
 template <class CB, class CC> constexpr KernelSet make_set() {
     static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
                   "chi and bracket kernels must share the transform radices (same permuted real-space order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, &launch_chi_t<CC>, &launch_bracket_t<CB>};
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_SCALAR, &launch_chi_t<CC>, &launch_bracket_t<CB>};
 }
 
 #ifndef GX_BR_NT
@@ -207,8 +208,12 @@ using P64x192  = gx::PairCfg<64, 192, 8, 8, 12, 16, 32, 128, 1>;
 using R64x64   = gx::RowCfg<64, 64, 8, 8, 64, 2>;
 using R128x64  = gx::RowCfg<128, 64, 16, 8, 128, 2>;
 using R192x64  = gx::RowCfg<192, 64, 16, 12, GX_ROW_NT, GX_ROW_MINB>;
+#ifndef GX_ROWCHI_NT
+#define GX_ROWCHI_NT 384
+#endif
+using RC192x64 = gx::RowCfg<192, 64, 16, 12, GX_ROWCHI_NT, 1>;   // chi planes: < 1 wave, more threads for the x passes
 const KernelSet kRowSets[] = {
-    make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, R192x64>(),
+    make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, RC192x64>(),
 };
 
 #ifndef GX_PS_NW
@@ -224,20 +229,20 @@ const KernelSet kPairSets[] = {
     make_pair_set<P192x64, PC192x64>(), make_pair_set<P256x96, P256x96>(), make_pair_set<P64x192, P64x192>(),
 };
 
-// Three kernel families share the C-ABI ("Kernel families"):
-//   scalar  (nl_kernels.cuh)       block-synchronous, scalar FP32            -- default: fastest measured
-//   pair    (nl_pair_kernels.cuh)  block-synchronous, packed FADD2/FFMA2     -- GX_KERNELS=pair
-//   persist (nl_pair_kernels.cuh)  persistent, warp-asynchronous, packed     -- GX_KERNELS=persist
-// The environment variable is read at gx_grid_create; a family without an instantiation for the grid
-// falls through to the next one.
+// Four kernel families share the C-ABI ("Kernel families"):
+//   row     (nl_row_kernels.cuh)   y direction of an x row in one thread's registers (NY = 64)  -- default where instantiated
+//   scalar  (nl_kernels.cuh)       block-synchronous two-pass transforms, scalar FP32            -- default otherwise
+//   pair    (nl_pair_kernels.cuh)  block-synchronous, packed FADD2/FFMA2                         -- GX_KERNELS=pair
+//   persist (nl_pair_kernels.cuh)  persistent, warp-asynchronous, packed                         -- GX_KERNELS=persist
+// GX_KERNELS (read at gx_grid_create) forces a family; one without an instantiation for the grid falls through.
 const KernelSet* find_set(int Nx, int Ny, int Nl) {
     const char* fam = std::getenv("GX_KERNELS");
+    if (!fam || std::strcmp(fam, "row") == 0)
+        for (const auto& k : kRowSets)
+            if (k.Nx == Nx && k.Ny == Ny) return &k;
     if (fam && std::strcmp(fam, "persist") == 0)
         for (const auto& k : kPersistSets)
             if (k.Nx == Nx && k.Ny == Ny && Nl <= k.max_nl) return &k;
-    if (fam && std::strcmp(fam, "row") == 0)
-        for (const auto& k : kRowSets)
-            if (k.Nx == Nx && k.Ny == Ny) return &k;
     if (fam && (std::strcmp(fam, "pair") == 0 || std::strcmp(fam, "persist") == 0))
         for (const auto& k : kPairSets)
             if (k.Nx == Nx && k.Ny == Ny) return &k;
@@ -736,6 +741,7 @@ int gx_query(gx_grid* g, int what, long long* value) {
         case GX_Q_LAUNCHES_PER_NL: *value = 3; break;
         case GX_Q_LAUNCHES_PER_RHS: *value = 3 + gx::kLinLaunchesFieldSolve + gx::kLinLaunchesRhs; break;
         case GX_Q_NL_FLOPS: *value = nl_flops(g); break;
+        case GX_Q_KERNEL_FAMILY: *value = g->ks ? g->ks->family : -1; break;
         case GX_Q_NL_BYTES:
             *value = 8LL * (2LL * g->Ns * g->Nm * g->Nl * g->Nz * g->nk + (long long)g->Nz * g->nk);
             break;

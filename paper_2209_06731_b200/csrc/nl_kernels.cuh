@@ -32,6 +32,16 @@
 
 namespace gx {
 
+// Optional phase timing (development builds only, -DGX_PHASE_TIMING): thread 0 of the first CTAs records
+// clock64() at phase boundaries; read back with gx_debug_phase_clocks().
+#ifdef GX_PHASE_TIMING
+__device__ long long gx_phase_clk[64 * 32];
+#define GX_PHASE(i) do { if (threadIdx.x == 0 && blockIdx.x < 64) gx_phase_clk[blockIdx.x * 32 + (i)] = clock64(); } while (0)
+#else
+#define GX_PHASE(i) do { } while (0)
+#endif
+
+
 template <int NX_, int NY_, int RX1_, int RX2_, int RY1_, int RY2_, int RB_, int NT_, int MINB_, bool STAGE_>
 struct PlaneCfg {
     static constexpr int NX = NX_, NY = NY_, RX1 = RX1_, RX2 = RX2_, RY1 = RY1_, RY2 = RY2_;

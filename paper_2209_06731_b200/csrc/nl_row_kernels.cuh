@@ -133,6 +133,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
     __shared__ unsigned long long stage_bar;
     __shared__ float Tsh[16];
     unsigned bar_parity = 0;
+    GX_PHASE(0);
     if (threadIdx.x == 0) mbar_init(&stage_bar, 1);
     if (threadIdx.x < p.Nl) Tsh[threadIdx.x] = __ldg(p.T + j * p.Nl + threadIdx.x);
     __syncthreads();
@@ -141,11 +142,14 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
     // ---- a2: forward Laguerre transform l -> node j, fused into the TMA-staged load
     stage_combine_tma<C>(W, S, &stage_bar, bar_parity, g0, lstride, Tsh, p.Nl);
     __syncthreads();
+    GX_PHASE(1);
     // ---- a3 + a4 (x part)
     x_inverse<C, false>(W, twx, p.dkx, p.dky, S);
+    GX_PHASE(2);
 
     const float2* __restrict__ dchi = p.dchi + (size_t)szj * NX * NY;
     pdl_wait();                     // chi planes of this call are complete and visible from here on
+    GX_PHASE(3);
     // ---- a4 (y part) + a5 + a6 (y part) + a7 (ky), one x row per thread, all in registers
     for (int row = threadIdx.x; row < NX; row += C::NT) {
         float2* __restrict__ Wr = W + row * C::NCOL;
@@ -155,6 +159,11 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
         float2 d[8], dn[8];
 #pragma unroll
         for (int k2 = 0; k2 < 8; ++k2) d[k2] = __ldg(dc + (8 * k2) * NX);
+#pragma unroll
+        for (int k2 = 0; k2 < 8; ++k2) {       // groups 1 and 2 towards L1 (no registers held)
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(dc + (1 + 8 * k2) * NX));
+            asm volatile("prefetch.global.L1 [%0];" ::"l"(dc + (2 + 8 * k2) * NX));
+        }
         float2 y[64];
         {
             float2 v[64];
@@ -173,6 +182,10 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
 #pragma unroll
                 for (int k2 = 0; k2 < 8; ++k2) dn[k2] = __ldg(dc + (k1 + 1 + 8 * k2) * NX);
             }
+            if (k1 < 5) {
+#pragma unroll
+                for (int k2 = 0; k2 < 8; ++k2) asm volatile("prefetch.global.L1 [%0];" ::"l"(dc + (k1 + 3 + 8 * k2) * NX));
+            }
             float2 u[8];
 #pragma unroll
             for (int n2 = 0; n2 < 8; ++n2) u[n2] = y[k1 * 8 + n2];
@@ -186,11 +199,13 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
         row_forward_real<C>(Wr, b);
     }
     __syncthreads();
+    GX_PHASE(4);
     // ---- a6 (x part) + a7 (keep |kx| <= K)
     x_forward<C>(W, twx, p.bhat + (size_t)unit * NK, p.scale);
 
     // ---- publish (see bracket_kernel)
     __syncthreads();
+    GX_PHASE(5);
     if (threadIdx.x == 0) { __threadfence(); atomicAdd(p.count + (s * p.Nm + m) * p.Nz + z, 1u); }
 }
 
