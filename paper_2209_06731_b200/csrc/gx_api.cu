@@ -141,6 +141,31 @@ template <class CB, class CC> constexpr KernelSet make_row_set() {
                   "chi and bracket kernels must share the x radices (same permuted x order)");
     return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_ROW, &launch_chi_row_t<CC>, &launch_bracket_row_t<CB>};
 }
+template <class C> cudaError_t launch_chi_rowp_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_rowp_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    gx::chi_planes_rowp_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
+    return cudaGetLastError();
+}
+template <class C> cudaError_t launch_bracket_rowp_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::bracket_rowp_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    return launch_pdl(gx::bracket_rowp_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
+}
+template <class CB, class CC> constexpr KernelSet make_rowp_set() {
+    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1, "same permuted x order");
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_ROWP, &launch_chi_rowp_t<CC>, &launch_bracket_rowp_t<CB>};
+}
 template <class CB, class CC> constexpr KernelSet make_pair_set() {
     static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
                   "chi and bracket kernels must share the transform radices (same permuted real-space order)");
@@ -212,6 +237,13 @@ using R192x64  = gx::RowCfg<192, 64, 16, 12, GX_ROW_NT, GX_ROW_MINB>;
 #define GX_ROWCHI_NT 384
 #endif
 using RC192x64 = gx::RowCfg<192, 64, 16, 12, GX_ROWCHI_NT, 1>;   // chi planes: < 1 wave, more threads for the x passes
+using RP192x64  = gx::RowPairCfg<192, 64, 16, 12, GX_ROW_NT, GX_ROW_MINB>;
+using RPC192x64 = gx::RowPairCfg<192, 64, 16, 12, GX_ROWCHI_NT, 1>;
+using RP128x64  = gx::RowPairCfg<128, 64, 16, 8, 128, 2>;
+using RP64x64   = gx::RowPairCfg<64, 64, 8, 8, 64, 2>;
+const KernelSet kRowPairSets[] = {
+    make_rowp_set<RP64x64, RP64x64>(), make_rowp_set<RP128x64, RP128x64>(), make_rowp_set<RP192x64, RPC192x64>(),
+};
 const KernelSet kRowSets[] = {
     make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, RC192x64>(),
 };
@@ -237,6 +269,9 @@ const KernelSet kPairSets[] = {
 // GX_KERNELS (read at gx_grid_create) forces a family; one without an instantiation for the grid falls through.
 const KernelSet* find_set(int Nx, int Ny, int Nl) {
     const char* fam = std::getenv("GX_KERNELS");
+    if (fam && std::strcmp(fam, "rowp") == 0)
+        for (const auto& k : kRowPairSets)
+            if (k.Nx == Nx && k.Ny == Ny) return &k;
     if (!fam || std::strcmp(fam, "row") == 0)
         for (const auto& k : kRowSets)
             if (k.Nx == Nx && k.Ny == Ny) return &k;
