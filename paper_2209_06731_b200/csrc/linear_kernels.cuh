@@ -52,7 +52,7 @@ struct LinTables {
 };
 
 constexpr int kLinLaunchesFieldSolve = 2;
-constexpr int kLinLaunchesRhs = 2;
+constexpr int kLinLaunchesRhs = 3;
 
 inline void lin_tables_free(LinTables& t) {
     cudaFree(t.Jl); cudaFree(t.invD); cudaFree(t.fsfac); cudaFree(t.wz); cudaFree(t.bs);
@@ -287,7 +287,11 @@ constexpr int kLinZG = 8;       // z groups per block
 
 // out[s,m,l,z,k] (+)= linear terms.  Block: one (s,m,l), a tile of kLinTK modes k, all z.  The spectral
 // parallel derivative / |k_par| are circulant Nz x Nz products on tiles staged in shared memory.
-template <bool ACC>
+// ZB = 4: each thread owns blocks of 4 consecutive z and register-blocks the circulant products (one staged
+// value and one new weight per term feed 8 FMAs); ZB = 1 when Nz is not a multiple of 4.
+// DERIV_ONLY: only the two z-operator terms (streaming, hyper-collisions), added to out; the pointwise terms
+// then come from lin_point_kernel.
+template <bool ACC, int ZB, bool DERIV_ONLY = false>
 __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, const float2* __restrict__ g,
                                                                  const float2* __restrict__ phi,
                                                                  float2* __restrict__ out) {
@@ -307,15 +311,38 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
         dz[i] = t.Dz[d];
         az[i] = t.Az[d];
     }
-    for (int z = zg; z < t.Nz; z += kLinZG) {
-        float2 c = make_float2(0.f, 0.f), gg = c;
-        if (live) {
-            const float2 hp = lin_H(t, g, phi, s, l, m + 1, z, k), hm = lin_H(t, g, phi, s, l, m - 1, z, k);
-            c = make_float2(sm1 * hp.x + sm0 * hm.x, sm1 * hp.y + sm0 * hm.y);
-            gg = g[(unsigned)((s * t.Nm + m) * t.Nl + l) * (unsigned)(t.Nz * t.nk) + (unsigned)(z * t.nk + k)];
+    {
+        // staging: 4 z at a time, every load issued before the first use (indices clamped, invalid masked)
+        const unsigned pl = (unsigned)(t.Nz * t.nk);
+        const int kc = live ? k : t.nk - 1;
+        const bool vp = m + 1 < t.Nm, vm = m - 1 >= 0;
+        const unsigned ip = (unsigned)((s * t.Nm + (vp ? m + 1 : m)) * t.Nl + l) * pl,
+                       im = (unsigned)((s * t.Nm + (vm ? m - 1 : m)) * t.Nl + l) * pl,
+                       i0 = (unsigned)((s * t.Nm + m) * t.Nl + l) * pl, ij = (unsigned)(s * t.Nl + l) * pl;
+        const float cp = vp ? sm1 : 0.f, cm = vm ? sm0 : 0.f;
+        const float cphi = (vm && m == 1) ? sm0 * t.zt[s] : 0.f;          // H_{l,0} = G_{l,0} + (Z/tau) J_l Phi
+        for (int zb = zg; zb < t.Nz; zb += 4 * kLinZG) {
+            float2 a[4], b[4], c[4], f[4];
+            float jl[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int z = min(zb + i * kLinZG, t.Nz - 1);
+                const unsigned zk = (unsigned)(z * t.nk + kc);
+                a[i] = g[ip + zk]; b[i] = g[im + zk]; c[i] = g[i0 + zk];
+                f[i] = phi[zk]; jl[i] = t.Jl[ij + zk];
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int z = zb + i * kLinZG;
+                if (z < t.Nz) {
+                    const float w = cphi * jl[i];
+                    S1[z * kLinTK + tk] = live ? make_float2(cp * a[i].x + cm * b[i].x + w * f[i].x,
+                                                             cp * a[i].y + cm * b[i].y + w * f[i].y)
+                                               : make_float2(0.f, 0.f);
+                    S2[z * kLinTK + tk] = live ? c[i] : make_float2(0.f, 0.f);
+                }
+            }
         }
-        S1[z * kLinTK + tk] = c;
-        S2[z * kLinTK + tk] = gg;
     }
     __syncthreads();
     if (!live) return;
@@ -323,30 +350,57 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
     const float hyp = t.nuhyp[s] * t.mpow[m];
     const float ky = t.dky * (float)(k % t.naky);
     const float fl = (float)l, fm = (float)m;
-    for (int z = zg; z < t.Nz; z += kLinZG) {
-        // streaming: -v_t grad_par(...)   and hyper-collisions: -nu_hyp m^p |k_par| G
-        float2 dp = make_float2(0.f, 0.f), ap = dp;
-        {
-            const float* __restrict__ dcol = dz + z + t.Nz;          // dcol[-zp] = D[(z - zp) mod Nz]
-            const float2* __restrict__ s1 = S1 + tk;
+    for (int zb = zg; zb * ZB < t.Nz; zb += kLinZG) {
+      const int z0 = zb * ZB;
+      // streaming: -v_t grad_par(...)   and hyper-collisions: -nu_hyp m^p |k_par| G
+      float2 dpb[ZB], apb[ZB];
+#pragma unroll
+      for (int i = 0; i < ZB; ++i) dpb[i] = apb[i] = make_float2(0.f, 0.f);
+      {
+          auto blocked = [&](const float* __restrict__ col, const float2* __restrict__ sv, float2 (&acc)[ZB]) {
+              const float* __restrict__ dc = col + z0 + t.Nz;          // weight of (z0 + i, zp) = dc[i - zp]
+              if constexpr (ZB == 4) {
+                  float w0 = dc[0], w1 = dc[1], w2 = dc[2], w3 = dc[3];
+                  for (int zp = 0; zp < t.Nz; zp += 4) {
+                      const float2 a0 = sv[zp * kLinTK], a1 = sv[(zp + 1) * kLinTK], a2 = sv[(zp + 2) * kLinTK],
+                                   a3 = sv[(zp + 3) * kLinTK];
+                      const float n0 = dc[-(zp + 1)], n1 = dc[-(zp + 2)], n2 = dc[-(zp + 3)], n3 = dc[-(zp + 4)];
+                      acc[0].x = fmaf(w0, a0.x, acc[0].x); acc[0].y = fmaf(w0, a0.y, acc[0].y);
+                      acc[1].x = fmaf(w1, a0.x, acc[1].x); acc[1].y = fmaf(w1, a0.y, acc[1].y);
+                      acc[2].x = fmaf(w2, a0.x, acc[2].x); acc[2].y = fmaf(w2, a0.y, acc[2].y);
+                      acc[3].x = fmaf(w3, a0.x, acc[3].x); acc[3].y = fmaf(w3, a0.y, acc[3].y);
+                      acc[0].x = fmaf(n0, a1.x, acc[0].x); acc[0].y = fmaf(n0, a1.y, acc[0].y);
+                      acc[1].x = fmaf(w0, a1.x, acc[1].x); acc[1].y = fmaf(w0, a1.y, acc[1].y);
+                      acc[2].x = fmaf(w1, a1.x, acc[2].x); acc[2].y = fmaf(w1, a1.y, acc[2].y);
+                      acc[3].x = fmaf(w2, a1.x, acc[3].x); acc[3].y = fmaf(w2, a1.y, acc[3].y);
+                      acc[0].x = fmaf(n1, a2.x, acc[0].x); acc[0].y = fmaf(n1, a2.y, acc[0].y);
+                      acc[1].x = fmaf(n0, a2.x, acc[1].x); acc[1].y = fmaf(n0, a2.y, acc[1].y);
+                      acc[2].x = fmaf(w0, a2.x, acc[2].x); acc[2].y = fmaf(w0, a2.y, acc[2].y);
+                      acc[3].x = fmaf(w1, a2.x, acc[3].x); acc[3].y = fmaf(w1, a2.y, acc[3].y);
+                      acc[0].x = fmaf(n2, a3.x, acc[0].x); acc[0].y = fmaf(n2, a3.y, acc[0].y);
+                      acc[1].x = fmaf(n1, a3.x, acc[1].x); acc[1].y = fmaf(n1, a3.y, acc[1].y);
+                      acc[2].x = fmaf(n0, a3.x, acc[2].x); acc[2].y = fmaf(n0, a3.y, acc[2].y);
+                      acc[3].x = fmaf(w0, a3.x, acc[3].x); acc[3].y = fmaf(w0, a3.y, acc[3].y);
+                      w3 = n0; w2 = n1; w1 = n2; w0 = n3;
+                  }
+              } else {
 #pragma unroll 4
-            for (int zp = 0; zp < t.Nz; ++zp) {
-                const float w = dcol[-zp];
-                const float2 a = s1[zp * kLinTK];
-                dp.x = fmaf(w, a.x, dp.x); dp.y = fmaf(w, a.y, dp.y);
-            }
-            if (hyp != 0.f) {
-                const float* __restrict__ acol = az + z + t.Nz;
-                const float2* __restrict__ s2 = S2 + tk;
-#pragma unroll 4
-                for (int zp = 0; zp < t.Nz; ++zp) {
-                    const float w = acol[-zp];
-                    const float2 b2 = s2[zp * kLinTK];
-                    ap.x = fmaf(w, b2.x, ap.x); ap.y = fmaf(w, b2.y, ap.y);
-                }
-            }
-        }
+                  for (int zp = 0; zp < t.Nz; ++zp) {
+                      const float w = dc[-zp];
+                      const float2 a = sv[zp * kLinTK];
+                      acc[0].x = fmaf(w, a.x, acc[0].x); acc[0].y = fmaf(w, a.y, acc[0].y);
+                  }
+              }
+          };
+          blocked(dz, S1 + tk, dpb);
+          if (hyp != 0.f) blocked(az, S2 + tk, apb);
+      }
+#pragma unroll
+      for (int zi = 0; zi < ZB; ++zi) {
+        const int z = z0 + zi;
+        const float2 dp = dpb[zi], ap = apb[zi];
         float2 r = make_float2(-vt * dp.x - hyp * ap.x, -vt * dp.y - hyp * ap.y);
+        if constexpr (!DERIV_ONLY) {
         const float2 h00 = lin_H(t, g, phi, s, l, m, z, k);
         // mirror force
         {
@@ -409,9 +463,120 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
             r.x -= hv * gg.x;
             r.y -= hv * gg.y;
         }
+        }
         float2* __restrict__ o = out + ((unsigned)((s * t.Nm + m) * t.Nl + l) * (unsigned)(t.Nz * t.nk) + (unsigned)(z * t.nk + k));
-        if (ACC) { const float2 prev = *o; r.x += prev.x; r.y += prev.y; }
+        if (ACC || DERIV_ONLY) { const float2 prev = *o; r.x += prev.x; r.y += prev.y; }
         *o = r;
+      }
+    }
+}
+
+// Pointwise terms of Eq. 4.9 (mirror, drifts, drive, Dougherty, hyper-viscosity) for ALL l of one (s,m) at
+// one (z,k) per thread: the 5 x Nl stencil values H_{l',m-2..m+2} are loaded once into registers and reused
+// by every l (the per-(l,m) kernel above fetches 13 neighbours per output).  Pure streaming, coalesced in k.
+template <int MAXL, bool ACC>
+__global__ void __launch_bounds__(256) lin_point_kernel(LinTables t, const float2* __restrict__ g,
+                                                        const float2* __restrict__ phi, float2* __restrict__ out) {
+    const unsigned pl = (unsigned)(t.Nz * t.nk);
+    const unsigned zk = blockIdx.x * blockDim.x + threadIdx.x;
+    if (zk >= pl) return;
+    const int s = blockIdx.y / t.Nm, m = blockIdx.y % t.Nm;
+    const int z = zk / t.nk, k = zk - z * t.nk;
+    const float zt = t.zt[s], vt = t.vt[s], tz = t.tz[s], nu = t.nu[s];
+    const float2 f = phi[zk];
+    float J[MAXL + 2];                                     // J[l + 1] = J_l, zero outside 0 <= l < Nl
+    J[0] = 0.f;
+#pragma unroll
+    for (int l = 0; l < MAXL; ++l) J[l + 1] = l < t.Nl ? t.Jl[(unsigned)(s * t.Nl + l) * pl + zk] : 0.f;
+    J[MAXL + 1] = 0.f;
+    // All stencil loads are issued unconditionally (indices clamped, invalid neighbours masked afterwards) so
+    // that the 5 x Nl requests are in flight together: the kernel is latency-bound otherwise.
+    float2 h[5][MAXL + 2];                                 // h[dm + 2][l + 1] = H_{l, m + dm}
+#pragma unroll
+    for (int dm = 0; dm < 5; ++dm) {
+        const int mm = m + dm - 2;
+        const int mc = min(max(mm, 0), t.Nm - 1);
+        h[dm][0] = h[dm][MAXL + 1] = make_float2(0.f, 0.f);
+#pragma unroll
+        for (int l = 0; l < MAXL; ++l)
+            h[dm][l + 1] = g[(unsigned)((s * t.Nm + mc) * t.Nl + min(l, t.Nl - 1)) * pl + zk];
+    }
+    float2 graw[MAXL];                                     // G_{l,m} (hyper-viscosity acts on G, not H)
+#pragma unroll
+    for (int l = 0; l < MAXL; ++l) graw[l] = h[2][l + 1];
+#pragma unroll
+    for (int dm = 0; dm < 5; ++dm) {
+        const int mm = m + dm - 2;
+        const bool mv = mm >= 0 && mm < t.Nm;
+#pragma unroll
+        for (int l = 0; l < MAXL; ++l) {
+            float2 v = h[dm][l + 1];
+            if (!(mv && l < t.Nl)) v = make_float2(0.f, 0.f);
+            else if (mm == 0) { v.x = fmaf(zt * J[l + 1], f.x, v.x); v.y = fmaf(zt * J[l + 1], f.y, v.y); }
+            h[dm][l + 1] = v;
+        }
+    }
+    const float fm = (float)m;
+    const float sm1 = sqrtf(fm + 1.f), sm0 = sqrtf(fm);
+    const float cA = sqrtf((fm + 1.f) * (fm + 2.f)), cB = 2.f * fm + 1.f, cC = sqrtf(fm * fmaxf(fm - 1.f, 0.f));
+    const float bg = -vt * t.bgrad[z];
+    const float wk = tz * t.omd[zk], wb = tz * t.omd[pl + zk];
+    const float hv = t.hypv[zk];
+    const float ky = t.dky * (float)(k % t.naky);
+    const float b = t.bs[(unsigned)s * pl + zk];
+    const float sb = sqrtf(fmaxf(b, 0.f));
+    float2 up = make_float2(0.f, 0.f), uq = up, tb = up;
+    if (nu != 0.f && m <= 2) {
+        const float2* __restrict__ mo = t.mom + (size_t)s * 3 * pl + zk;
+        up = mo[0]; uq = mo[pl]; tb = mo[2 * (size_t)pl];
+    }
+#pragma unroll
+    for (int l = 0; l < MAXL; ++l) {
+        if (l < t.Nl) {
+            const float fl = (float)l;
+            const float2 c0 = h[2][l + 1];
+            // mirror force
+            const float ca = -(fl + 1.f) * sm1, cb = -fl * sm1, cc = fl * sm0, cd = (fl + 1.f) * sm0;
+            float2 r;
+            r.x = bg * (ca * h[3][l + 1].x + cb * h[3][l].x + cc * h[1][l + 1].x + cd * h[1][l + 2].x);
+            r.y = bg * (ca * h[3][l + 1].y + cb * h[3][l].y + cc * h[1][l + 1].y + cd * h[1][l + 2].y);
+            // drifts: -i (tau/Z) w (...)
+            const float bx = wk * (cA * h[4][l + 1].x + cB * c0.x + cC * h[0][l + 1].x) +
+                             wb * ((fl + 1.f) * h[2][l + 2].x + (2.f * fl + 1.f) * c0.x + fl * h[2][l].x);
+            const float by = wk * (cA * h[4][l + 1].y + cB * c0.y + cC * h[0][l + 1].y) +
+                             wb * ((fl + 1.f) * h[2][l + 2].y + (2.f * fl + 1.f) * c0.y + fl * h[2][l].y);
+            r.x += by;
+            r.y -= bx;
+            const float jm = J[l], j0 = J[l + 1], jp = J[l + 2];
+            const float jt = fl * jm + 2.f * fl * j0 + (fl + 1.f) * jp;
+            if (m == 0 || m == 2) {                          // drive
+                const float c = m == 0 ? t.fprim[s] * j0 + t.tprim[s] * jt : t.tprim[s] * j0 * 0.70710678118654752440f;
+                r.x -= ky * c * f.y;
+                r.y += ky * c * f.x;
+            }
+            if (nu != 0.f) {                                 // Dougherty
+                const float damp = nu * (b + 2.f * fl + fm);
+                r.x -= damp * c0.x;
+                r.y -= damp * c0.y;
+                if (m == 0) {
+                    const float cu = sb * (j0 + jm), ct = 2.f * jt;
+                    r.x = fmaf(nu, cu * uq.x + ct * tb.x, r.x);
+                    r.y = fmaf(nu, cu * uq.y + ct * tb.y, r.y);
+                } else if (m == 1) {
+                    r.x = fmaf(nu * j0, up.x, r.x);
+                    r.y = fmaf(nu * j0, up.y, r.y);
+                } else if (m == 2) {
+                    r.x = fmaf(nu * 1.41421356237309504880f * j0, tb.x, r.x);
+                    r.y = fmaf(nu * 1.41421356237309504880f * j0, tb.y, r.y);
+                }
+            }
+            // hyper-viscosity
+            r.x -= hv * graw[l].x;
+            r.y -= hv * graw[l].y;
+            float2* __restrict__ o = out + ((unsigned)((s * t.Nm + m) * t.Nl + l) * pl + zk);
+            if (ACC) { const float2 prev = *o; r.x += prev.x; r.y += prev.y; }
+            *o = r;
+        }
     }
 }
 
@@ -425,14 +590,36 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
     const size_t smem = (size_t)t.Nz * kLinTK * sizeof(float2) * 2 + 4 * (size_t)t.Nz * sizeof(float);
     static bool attr = false;
     if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(lin_rhs_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(lin_rhs_kernel<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<true, 4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<true, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
         if (e != cudaSuccess) return e;
         attr = true;
     }
     dim3 grid((t.nk + kLinTK - 1) / kLinTK, t.Nl, t.Ns * t.Nm);
-    if (accumulate) lin_rhs_kernel<true><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
-    else lin_rhs_kernel<false><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+    const bool b4 = t.Nz % 4 == 0;
+    if (t.Nl <= 8) {
+        // pointwise terms with the stencil in registers, then the z-operator terms added on top
+        dim3 gp((unsigned)(((size_t)t.Nz * t.nk + 255) / 256), t.Ns * t.Nm);
+        if (t.Nl <= 4) {
+            if (accumulate) lin_point_kernel<4, true><<<gp, 256, 0, st>>>(t, g, phi, out);
+            else lin_point_kernel<4, false><<<gp, 256, 0, st>>>(t, g, phi, out);
+        } else {
+            if (accumulate) lin_point_kernel<8, true><<<gp, 256, 0, st>>>(t, g, phi, out);
+            else lin_point_kernel<8, false><<<gp, 256, 0, st>>>(t, g, phi, out);
+        }
+        if (b4) lin_rhs_kernel<true, 4, true><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+        else lin_rhs_kernel<true, 1, true><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+    } else if (accumulate) {
+        if (b4) lin_rhs_kernel<true, 4><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+        else lin_rhs_kernel<true, 1><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+    } else {
+        if (b4) lin_rhs_kernel<false, 4><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+        else lin_rhs_kernel<false, 1><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+    }
     return cudaGetLastError();
 }
 
