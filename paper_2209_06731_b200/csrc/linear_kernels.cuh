@@ -601,8 +601,9 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
     }
     dim3 grid((t.nk + kLinTK - 1) / kLinTK, t.Nl, t.Ns * t.Nm);
     const bool b4 = t.Nz % 4 == 0;
-    if (t.Nl <= 8) {
-        // pointwise terms with the stencil in registers, then the z-operator terms added on top
+    if (t.Nl <= 4) {
+        // pointwise terms with the stencil in registers, then the z-operator terms added on top (measured faster
+        // for Nl <= 4 only: with 8 Laguerre moments the 5 x 10 stencil costs 135 registers and the occupancy)
         dim3 gp((unsigned)(((size_t)t.Nz * t.nk + 255) / 256), t.Ns * t.Nm);
         if (t.Nl <= 4) {
             if (accumulate) lin_point_kernel<4, true><<<gp, 256, 0, st>>>(t, g, phi, out);
