@@ -197,9 +197,18 @@ using C128x64  = gx::PlaneCfg<128, 64, 16, 8, 8, 8, 64, GX_CHI_NT, 1, true>;
 using B192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, GX_BR_RB, GX_BR_NT, GX_BR_MINB, true>;
 using C192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, 64, GX_CHI_NT, 1, true>;
 using B256x64  = gx::PlaneCfg<256, 64, 16, 16, 8, 8, 64, 256, 1, true>;
-using B256x96  = gx::PlaneCfg<256, 96, 16, 16, 8, 12, 64, 256, 1, true>;
-using B192x192 = gx::PlaneCfg<192, 192, 16, 12, 12, 16, 16, 256, 1, false>;
-using B64x192  = gx::PlaneCfg<64, 192, 8, 8, 12, 16, 32, 256, 1, true>;
+#ifndef GX_BIG_NT
+#define GX_BIG_NT 384
+#endif
+using B256x96  = gx::PlaneCfg<256, 96, 16, 16, 8, 12, 64, GX_BIG_NT, 1, true>;
+using B192x192 = gx::PlaneCfg<192, 192, 16, 12, 12, 16, 16, GX_BIG_NT, 1, false>;
+#ifndef GX_W7X_RB
+#define GX_W7X_RB 16
+#endif
+#ifndef GX_W7X_NT
+#define GX_W7X_NT 256
+#endif
+using B64x192  = gx::PlaneCfg<64, 192, 8, 8, 12, 16, GX_W7X_RB, GX_W7X_NT, (GX_W7X_RB <= 16 ? 2 : 1), true>;   // RB 16: 92 KB, two CTAs per SM
 
 const KernelSet kKernelSets[] = {
     make_set<B16x16, B16x16>(),   make_set<B64x64, B64x64>(),     make_set<B128x64, C128x64>(),

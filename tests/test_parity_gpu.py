@@ -332,3 +332,52 @@ def test_ssprk3_steps_parity(torch_cuda):
     assert O.relative_max_error(out, ref) <= TOL
     assert O.relative_max_error(G, ref) > 100 * TOL          # the state really moved
     grid.close()
+
+
+@pytest.mark.parametrize("Nx,Ny,Nz,Nl,Nm,Ns", [
+    (64, 64, 3, 1, 1, 1),      # one Laguerre moment (J = 1), one Hermite moment, odd Nz: degenerate batch sizes
+    (64, 64, 2, 3, 2, 2),      # J = 4, two species on the row family
+    (128, 64, 2, 4, 3, 1),     # odd Nm
+    (256, 64, 1, 2, 2, 1),     # NX = 256 (scalar family), single z
+    (16, 16, 1, 5, 1, 1),      # Nl = 5 -> J = 7 on the smallest plane
+])
+def test_degenerate_and_ragged_shapes(torch_cuda, Nx, Ny, Nz, Nl, Nm, Ns):
+    """Edge shapes through the default kernel family: every (s,m,z) plane against the pseudo-spectral oracle."""
+    sp = [I.Species(), I.Species(Z=-1.0, mass=1.0 / 1836.0, amp=0.05)][:Ns]
+    cfg = I.Config("edge", Nx, Ny, Nz, Nl, Nm, sp, seed=777 + Nx + Nl)
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = _grid(cfg, geo)
+    out = _gpu_nl(torch_cuda, grid, G, Phi)
+    ref = _oracle_nl(cfg, geo, G, Phi, method="dft")
+    assert np.all(np.isfinite(out))
+    assert O.relative_max_error(out, ref) <= TOL
+    grid.close()
+
+
+def test_calls_on_a_side_stream_and_interleaved_grids(torch_cuda):
+    """Two handles used alternately on a non-default stream: per-handle counters and workspaces do not interfere."""
+    torch = torch_cuda
+    cfgs = [I.named_config("tiny"), I.Config("b", 64, 64, 2, 2, 2, [I.Species()], seed=5)]
+    st = torch.cuda.Stream()
+    items = []
+    for cfg in cfgs:
+        geo = I.geometry_arrays(cfg)
+        G = I.make_state(cfg, geo)
+        Phi = _oracle_phi(cfg, geo, G)
+        items.append((cfg, geo, G, Phi, _grid(cfg, geo)))
+    outs = []
+    with torch.cuda.stream(st):
+        bufs = [(torch.from_numpy(G).cuda(), torch.from_numpy(Phi).cuda()) for (_, _, G, Phi, _) in items]
+        for rep in range(3):
+            for (cfg, geo, G, Phi, grid), (g, phi) in zip(items, bufs):
+                out = torch.full_like(g, float("nan"))
+                grid.nonlinear_rhs(g, phi, out)
+                if rep == 2:
+                    outs.append(out)
+    st.synchronize()
+    for (cfg, geo, G, Phi, grid), out in zip(items, outs):
+        ref = _oracle_nl(cfg, geo, G, Phi, method="dft")
+        assert O.relative_max_error(out.cpu().numpy(), ref) <= TOL
+        grid.close()
