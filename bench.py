@@ -395,7 +395,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=100)
-    ap.add_argument("--config", default="cyclone", choices=I.CONFIG_NAMES + ["w7x-shape"])
+    ap.add_argument("--config", default="cyclone", choices=I.CONFIG_NAMES + ["w7x-shape", "nx64", "nx128", "nx192", "nx256"])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="omit the oracle timing (ncu passes)")
     ap.add_argument("--skip-reference-point", action="store_true", help="omit the cuFFT+cuBLAS composition")

@@ -239,8 +239,8 @@ using P64x192  = gx::PairCfg<64, 192, 8, 8, 12, 16, 32, 128, 1>;
 #ifndef GX_ROW_MINB
 #define GX_ROW_MINB 2
 #endif
-using R64x64   = gx::RowCfg<64, 64, 8, 8, 64, 2>;
-using R128x64  = gx::RowCfg<128, 64, 16, 8, 128, 2>;
+using R64x64   = gx::RowCfg<64, 64, 8, 8, 64, 6>;
+using R128x64  = gx::RowCfg<128, 64, 16, 8, 128, 3>;
 using R192x64  = gx::RowCfg<192, 64, 16, 12, GX_ROW_NT, GX_ROW_MINB>;
 #ifndef GX_ROWCHI_NT
 #define GX_ROWCHI_NT 384
@@ -253,8 +253,10 @@ using RP64x64   = gx::RowPairCfg<64, 64, 8, 8, 64, 2>;
 const KernelSet kRowPairSets[] = {
     make_rowp_set<RP64x64, RP64x64>(), make_rowp_set<RP128x64, RP128x64>(), make_rowp_set<RP192x64, RPC192x64>(),
 };
+using R256x64  = gx::RowCfg<256, 64, 16, 16, 256, 1>;
 const KernelSet kRowSets[] = {
     make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, RC192x64>(),
+    make_row_set<R256x64, R256x64>(),
 };
 
 #ifndef GX_PS_NW

@@ -131,6 +131,9 @@ def named_config(name: str) -> Config:
         return Config("w7x-shape", 64, 192, 128, 4, 8,
                       [Species(**ion, tprim=3.0, fprim=1.0, nu_ss=0.01)],
                       geometry="harmonics", seed=BASE_SEED + 5)
+    if name.startswith("nx") and name[2:].isdigit():   # Nx sweep at the Cyclone velocity/parallel resolution (cf. Fig. 10)
+        return Config(name, int(name[2:]), 64, 24, 4, 8, [Species(**ion, tprim=6.9, fprim=2.2, nu_ss=0.01)],
+                      seed=BASE_SEED + 6)
     raise KeyError(name)
 
 
