@@ -23,9 +23,14 @@ with H, G, J == 0 outside 0 <= l < Nl, 0 <= m < Nm (closure by truncation
 Readings of silent / garbled points (rows L1-L8):
   L1  the stray "]" on P:213 is a garble: all four mirror terms multiply grad_par ln B.
   L2  grad_par = gradpar * d/dz with constant gradpar, d/dz spectral on the periodic grid
-      z_i = -pi + 2 pi i/Nz (k_z integer); the Nyquist mode's derivative is zero.  Each (kx,ky) is
-      periodic by itself; the twist-and-shift linking of P:322-327 is not applied (SURVEY App. A:
-      "first implementation").  No end-damping layer (Eq. 4.30 is optional).
+      z_i = -pi + 2 pi i/Nz (k_z integer); the Nyquist mode's derivative is zero.  boundary="periodic":
+      each (kx,ky) is periodic by itself (SURVEY App. A "first implementation").  boundary="linked": the
+      twist-and-shift condition of P:322-327, H(kx,ky,z) = H(kx + dk, ky, z + 2 pi), dk = 2 pi ky shat: the
+      modes kx_0 + n dk (n integer, inside the dealiased set) of one ky form ONE periodic extended domain of
+      L 2 pi, on which mode n holds the segment theta = z - 2 pi n of the ballooning function; the z operators
+      are spectral on that domain (k = j/L, Nyquist dropped in the derivative).  dk is a whole number
+      jtwist*q of kx grid steps because Lx/Ly = jtwist/(2 pi |shat|).  No end-damping layer
+      (Eq. 4.30 is optional, P:333).
   L3  w_d^gradB = (ky gbdrift + kx gbdrift0/shat)/2, w_d^kappa = (ky cvdrift + kx cvdrift0/shat)/2
       (P:229 with Eq. E9-E11: the arrays carry a factor 2 and gbdrift0 a factor shat).
   L4  i w_* = i ky; 1/L_n = fprim, 1/L_T = tprim.
@@ -89,6 +94,67 @@ def abs_kz_matrix(Nz):
     return np.real((ph * k[None, :]) @ np.conj(ph).T) / Nz
 
 
+def ext_operator_matrices(Nz, L):
+    """(d/dzeta, |k_zeta|) on the periodic extended domain of L segments of Nz points (length 2 pi L):
+    explicit DFT sums with k = j/L; the Nyquist mode is dropped in the derivative (reading L2)."""
+    N = Nz * L
+    j = np.array([q if q <= N // 2 else q - N for q in range(N)], dtype=np.float64)
+    kd = j / L
+    if N % 2 == 0:
+        kd = kd.copy()
+        kd[N // 2] = 0.0
+    ph = np.exp(2j * math.pi * np.outer(np.arange(N), np.arange(N)) / N)
+    D = np.real((ph * (1j * kd)[None, :]) @ np.conj(ph).T) / N
+    A = np.real((ph * (np.abs(j) / L)[None, :]) @ np.conj(ph).T) / N
+    return D, A
+
+
+def twist_shift_chains(Nx, Ny, jtwist):
+    """Linked chains of the compact modes under H(kx,ky,z) = H(kx + dk,ky,z + 2 pi) (Eq. 4.29):
+    dk = jtwist*q grid steps for ky index q (sign of jtwist = sign of shat).  Returns a list of
+    (q, [compact kx rows i_0, i_1, ...]) with kx integers p_n = p_0 + n*jtwist*q, p_0 the member with no
+    predecessor inside the dealiased set; ky = 0 modes are chains of length 1."""
+    kxi = [int(v) for v in O.kx_index(Nx)]
+    K = (len(kxi) - 1) // 2
+    row = {p: i for i, p in enumerate(kxi)}
+    chains = []
+    for q in range(len(O.ky_index(Ny))):
+        step = jtwist * q
+        for p in range(-K, K + 1):
+            if step == 0:
+                chains.append((q, [row[p]]))
+                continue
+            if abs(p - step) <= K:          # has a predecessor: not a chain start
+                continue
+            members, pp = [], p
+            while abs(pp) <= K:
+                members.append(row[pp])
+                pp += step
+            chains.append((q, members))
+    return chains
+
+
+def apply_z_operator(f, kind, gradpar, Nx, Ny, boundary="periodic", jtwist=None):
+    """gradpar * d/dz (kind="d") or |gradpar| * |k_z| (kind="a") of f[z][kx][ky] (reading L2)."""
+    Nz = f.shape[0]
+    if boundary == "periodic":
+        M = gradpar * dz_matrix(Nz) if kind == "d" else abs(gradpar) * abs_kz_matrix(Nz)
+        return np.tensordot(M, f, axes=(1, 0))
+    out = np.zeros_like(f, dtype=np.complex128)
+    cache = {}
+    for q, rows in twist_shift_chains(Nx, Ny, jtwist):
+        L = len(rows)
+        if L not in cache:
+            cache[L] = ext_operator_matrices(Nz, L)
+        M = gradpar * cache[L][0] if kind == "d" else abs(gradpar) * cache[L][1]
+        # ballooning order: mode n holds theta = z - 2 pi n, so increasing theta runs through n = L-1, ..., 0
+        ext = np.concatenate([f[:, rows[n], q] for n in range(L - 1, -1, -1)])
+        res = M @ ext
+        for n in range(L):
+            out[:, rows[n], q] = res[(L - 1 - n) * Nz:(L - n) * Nz]
+    return out
+
+
 # ============================================================================ pieces
 def jflr_all(b, Nl):
     """J_l(b) for l = -1..Nl as a dict (zero outside 0 <= l < Nl: P:205)."""
@@ -117,8 +183,17 @@ def drift_frequencies(kx, ky, geo, shat):
     return wk, wb
 
 
+def jtwist_of(dkx, dky, shat):
+    """Signed number of kx grid steps per ky step in the twist-and-shift condition: 2 pi shat dky / dkx."""
+    j = 2.0 * math.pi * shat * dky / dkx
+    if abs(j - round(j)) > 1e-6 or round(j) == 0:
+        raise ValueError("box is not twist-shift quantised: 2 pi shat dky/dkx = %r" % j)
+    return int(round(j))
+
+
 def linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper=0.05, n_hyper=4, f_hyp=1.0,
-               terms=("stream", "mirror", "drift", "drive", "coll", "hypervisc", "hypercoll")):
+               terms=("stream", "mirror", "drift", "drive", "coll", "hypervisc", "hypercoll"),
+               boundary="periodic"):
     """dG/dt from every term of Eq. 4.9 except the nonlinear one (see module header).  fp64.
     G [s][m][l][z][kx][ky], Phi [z][kx][ky]; geo holds the per-z arrays of P:677-694 plus gradpar.
     ``terms`` selects contributions (the pins test them one at a time)."""
@@ -128,14 +203,14 @@ def linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper=0.05, n_hyp
     kx, ky = dkx * O.kx_index(Nx), dky * O.ky_index(Ny)
     kp2 = O.kperp2(kx, ky, geo["gds2"], geo["gds21"], geo["gds22"], shat)
     gradpar = float(geo["gradpar"])
-    Dz = gradpar * dz_matrix(Nz)                                   # grad_par
-    Az = abs(gradpar) * abs_kz_matrix(Nz)                          # |k_par|
+    jtw = jtwist_of(dkx, dky, shat) if boundary == "linked" else None
     bgrad = np.asarray(geo["bgrad"], np.float64)[:, None, None]    # grad_par ln B
     wk, wb = drift_frequencies(kx, ky, geo, shat)
     iky = 1j * ky[None, None, :]
     kp2max = float(np.max(kp2))
     out = np.zeros_like(G)
-    dpar = lambda f: np.tensordot(Dz, f, axes=(1, 0))
+    dpar = lambda f: apply_z_operator(f, "d", gradpar, Nx, Ny, boundary, jtw)          # grad_par
+    kpar = lambda f: apply_z_operator(f, "a", gradpar, Nx, Ny, boundary, jtw)          # |k_par|
     for s, sp in enumerate(species):
         Z, mass, temp = _get(sp, "Z"), _get(sp, "mass"), _get(sp, "temp")
         tprim, fprim, nu = _get(sp, "tprim"), _get(sp, "fprim"), _nu(sp)
@@ -192,18 +267,18 @@ def linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper=0.05, n_hyp
                 if "hypervisc" in terms and D_hyper != 0.0:
                     r -= D_hyper * (kp2 / kp2max) ** n_hyper * G[s, m, l]
                 if "hypercoll" in terms and f_hyp != 0.0 and m > 2:
-                    r -= nuhyp_fac * float(m) ** p_hyp * np.tensordot(Az, G[s, m, l], axes=(1, 0))
+                    r -= nuhyp_fac * float(m) ** p_hyp * kpar(G[s, m, l])
                 out[s, m, l] = r
     return out
 
 
 # ============================================================================ full RHS and time step
 def rhs(G, Nx, Ny, dkx, dky, shat, geo, species, tau_fac=1.0, adiabatic=None, D_hyper=0.05, n_hyper=4,
-        f_hyp=1.0, nonlinear=True, planes=None):
+        f_hyp=1.0, nonlinear=True, planes=None, boundary="periodic"):
     """gx_rhs: Phi from quasineutrality, then -N + linear terms (Eq. 4.9)."""
     adiabatic = (len(species) == 1) if adiabatic is None else adiabatic
     Phi = O.field_solve(G, Nx, Ny, dkx, dky, shat, geo, species, tau_fac=tau_fac, adiabatic=adiabatic)
-    out = linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper, n_hyper, f_hyp)
+    out = linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper, n_hyper, f_hyp, boundary=boundary)
     if nonlinear:
         out = out + O.nonlinear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, method="dft", planes=planes)
     return out

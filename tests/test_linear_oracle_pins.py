@@ -268,3 +268,66 @@ def test_full_rhs_is_sum_of_parts_and_linear_in_g_without_bracket():
     nl = O.nonlinear_rhs(G, Phi, NX, NY, DKX, DKY, SHAT, geo, [sp], method="conv_np")
     assert np.allclose(full, lin + nl, atol=1e-14)
     assert np.allclose(L.rhs(2 * G, NX, NY, DKX, DKY, SHAT, geo, [sp], nonlinear=False), 2 * lin, atol=1e-15)
+
+
+# ---------------------------------------------------------------------------- twist-and-shift linking
+def test_twist_shift_chains_partition_the_modes_and_keep_kperp_continuous():
+    Nx, Ny, shat, dky = 192, 64, 0.8, 0.1
+    jt = max(1, round(2 * math.pi * shat))
+    dkx = 2 * math.pi * shat * dky / jt
+    assert L.jtwist_of(dkx, dky, shat) == 5 and L.jtwist_of(dkx, dky, -shat) == -5
+    with pytest.raises(ValueError):
+        L.jtwist_of(1.07 * dkx, dky, shat)
+    chains = L.twist_shift_chains(Nx, Ny, 5)
+    seen = sorted((i, q) for q, rows in chains for i in rows)
+    assert seen == sorted((i, q) for i in range(127) for q in range(22))          # every mode exactly once
+    assert sorted(len(r) for q, r in chains if q == 1) == [25, 25, 25, 26, 26]       # 127 modes in 5 classes mod 5
+    assert all(len(r) == 1 for q, r in chains if q == 0)
+    kxi = O.kx_index(Nx)
+    z = np.linspace(-math.pi, math.pi, 7)
+    for q, rows in chains:
+        for a, b in zip(rows[:-1], rows[1:]):
+            kxa, kxb, ky = dkx * kxi[a], dkx * kxi[b], dky * q
+            # Eq. 4.29: H(kx,ky,z) = H(kx + dk,ky,z + 2 pi): the s-alpha k_perp^2 = (kx - shat z ky)^2 + ky^2 must agree
+            assert np.allclose((kxa - shat * z * ky) ** 2, (kxb - shat * (z + 2 * math.pi) * ky) ** 2, atol=1e-12)
+
+
+def test_linked_z_operators_closed_form_on_a_ballooning_harmonic():
+    Nz, jt, gradpar = 8, 2, 0.7
+    chains = L.twist_shift_chains(NX, NY, jt)
+    q, rows = max(chains, key=lambda c: len(c[1]))
+    Lc = len(rows)
+    assert Lc >= 3
+    z = -math.pi + 2 * math.pi * np.arange(Nz) / Nz
+    for jmode in (1, -2, 5):
+        kap = jmode / Lc
+        f = np.zeros((Nz, NAKX, NAKY), complex)
+        for n, i in enumerate(rows):
+            f[:, i, q] = np.exp(1j * kap * (z - 2 * math.pi * n))        # mode n holds Psi(theta = z - 2 pi n)
+        d = L.apply_z_operator(f, "d", gradpar, NX, NY, "linked", jt)
+        a = L.apply_z_operator(f, "a", gradpar, NX, NY, "linked", jt)
+        assert np.allclose(d, 1j * kap * gradpar * f, atol=1e-12)
+        assert np.allclose(a, abs(kap) * gradpar * f, atol=1e-12)
+    # ky = 0 (and every unlinked mode) keeps the plain periodic operator; the operator stays anti-symmetric
+    g = _rand((Nz, NAKX, NAKY), 23)
+    dl = L.apply_z_operator(g, "d", gradpar, NX, NY, "linked", jt)
+    dp = L.apply_z_operator(g, "d", gradpar, NX, NY, "periodic")
+    assert np.allclose(dl[:, :, 0], dp[:, :, 0], atol=1e-13)
+    assert not np.allclose(dl[:, :, 1], dp[:, :, 1], atol=1e-3)
+    assert abs(np.sum(np.real(np.conj(g) * dl))) < 1e-11 * np.sum(np.abs(g) ** 2)
+
+
+def test_linked_rhs_differs_only_through_the_z_operators():
+    Nz = 4
+    geo, z = _geo(Nz)
+    dkx = 2 * math.pi * SHAT * DKY / 5
+    sp = dict(Z=1.0, mass=1.0, temp=1.0, dens=1.0, tprim=6.9, fprim=2.2, nu_ss=0.01)
+    G = _rand((1, 5, 2, Nz, NAKX, NAKY), 29)
+    Phi = _rand((Nz, NAKX, NAKY), 31)
+    kw = dict(Nx=NX, Ny=NY, dkx=dkx, dky=DKY, shat=SHAT, geo=geo, species=[sp])
+    a = L.linear_rhs(G, Phi, boundary="linked", **kw)
+    b = L.linear_rhs(G, Phi, boundary="periodic", **kw)
+    local = ("mirror", "drift", "drive", "coll", "hypervisc")
+    assert np.allclose(L.linear_rhs(G, Phi, boundary="linked", terms=local, **kw),
+                       L.linear_rhs(G, Phi, boundary="periodic", terms=local, **kw), atol=0)
+    assert np.allclose(a[..., 0], b[..., 0], atol=1e-12) and not np.allclose(a[..., 1:], b[..., 1:], atol=1e-3)
