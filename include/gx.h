@@ -81,6 +81,13 @@ int gx_species_set(gx_grid* g, int s, double Z, double mass, double temp, double
  * enabled != 0 selects it (requires Ns == 1); tau_fac = T_i/T_e. Default: enabled iff Ns == 1, tau_fac 1. */
 int gx_adiabatic_set(gx_grid* g, int enabled, double tau_fac);
 
+/* Parallel boundary condition of the z operators in gx_rhs / gx_linear_rhs (call before gx_geometry_set):
+ * linked == 0 (default): every (kx,ky) is periodic in z by itself; linked != 0: twist-and-shift (Eq. 4.29,
+ * P:322-327), H(kx,ky,z) = H(kx + dk,ky,z + 2 pi), dk = 2 pi ky shat: the modes kx_0 + n dk inside the dealiased
+ * set form one periodic extended domain on which grad_par and |k_par| are spectral.  Needs a quantised box,
+ * 2 pi shat dky / dkx a non-zero integer; gx_geometry_set returns GX_ERR_ARG otherwise. */
+int gx_boundary_set(gx_grid* g, int linked);
+
 /* Dissipation parameters of gx_rhs: hyper-viscosity D (k_perp^2/k_perp,max^2)^n (Eq. 4.26) and
  * hyper-collisions nu_hyp m^p, p = Nm/2, strength f_hyp (Eq. 4.27-4.28). Defaults 0.05, 4, 1. */
 int gx_dissipation_set(gx_grid* g, double D_hyper, int n_hyper, double f_hyp);

@@ -353,6 +353,7 @@ struct gx_grid {
     double dkx = 0, dky = 0, shat = 1;
     bool box_set = false, geo_set = false;
     bool adiabatic = false;
+    bool linked = false;                        // twist-and-shift linked z operators (gx_boundary_set)
     double tau_fac = 1.0;
     double D_hyper = 0.05, f_hyp = 1.0;
     int n_hyper = 4;
@@ -546,6 +547,13 @@ int gx_adiabatic_set(gx_grid* g, int enabled, double tau_fac) {
     return GX_OK;
 }
 
+int gx_boundary_set(gx_grid* g, int linked) {
+    if (!g) return GX_ERR_ARG;
+    g->linked = linked != 0;
+    g->geo_set = false;
+    return GX_OK;
+}
+
 int gx_dissipation_set(gx_grid* g, double D_hyper, int n_hyper, double f_hyp) {
     if (!g) return GX_ERR_ARG;
     if (D_hyper < 0 || n_hyper < 0 || f_hyp < 0) return fail(g, GX_ERR_ARG, "negative dissipation parameter");
@@ -617,11 +625,13 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
         in.bgrad = g->bgrad.data(); in.jacobian = g->jacobian.data();
         in.adiabatic = g->adiabatic; in.tau_fac = g->tau_fac;
         in.D_hyper = g->D_hyper; in.n_hyper = g->n_hyper; in.f_hyp = g->f_hyp;
+        in.linked = g->linked;
         for (const auto& sp : g->sp)
             in.species.push_back({sp.Z, sp.mass, sp.temp, sp.dens, sp.tprim, sp.fprim, sp.nu});
         std::string msg;
         size_t bytes = 0;
-        if (!gx::lin_tables_build(in, g->lin, bytes, msg)) return fail(g, GX_ERR_CUDA, msg);
+        if (!gx::lin_tables_build(in, g->lin, bytes, msg))
+            return fail(g, msg.find("quantised") != std::string::npos ? GX_ERR_ARG : GX_ERR_CUDA, msg);
         g->bytes += bytes;
         if (!g->dphi_rhs) {
             int rc = dev_alloc(g, &g->dphi_rhs, (size_t)Nz * g->nk);

@@ -24,6 +24,7 @@ struct LinHostInput {
     bool adiabatic;
     double tau_fac, D_hyper, f_hyp;
     int n_hyper;
+    bool linked = false;       // twist-and-shift linked z operators (Eq. 4.29) instead of periodic per mode
     std::vector<LinSpecies> species;
 };
 
@@ -45,6 +46,14 @@ struct LinTables {
     float qn[kMaxSpecies] = {0}, zt[kMaxSpecies] = {0}, vt[kMaxSpecies] = {0}, tz[kMaxSpecies] = {0};
     float tprim[kMaxSpecies] = {0}, fprim[kMaxSpecies] = {0}, nu[kMaxSpecies] = {0}, nuhyp[kMaxSpecies] = {0};
     float* mpow = nullptr;     // [Nm] m^p, p = Nm/2 (Eq. 4.27)
+    // twist-and-shift linking (Eq. 4.29): chains of compact modes forming one periodic extended domain
+    bool linked = false;
+    int nchain = 0, max_ext = 0;   // number of chains, longest extended domain in points (L * Nz)
+    int* chain_off = nullptr;      // [nchain + 1] offsets into chain_mode
+    int* chain_mode = nullptr;     // compact mode index k = kx_row * naky + ky, in order of increasing ballooning angle
+    int* ext_off = nullptr;        // [nchain] offset of the chain's circulant columns in ext_d / ext_a
+    float* ext_d = nullptr;        // per distinct length L: column of gradpar * d/dzeta, L*Nz entries
+    float* ext_a = nullptr;        // per distinct length L: column of |gradpar| * |k_zeta|
     float2* mom = nullptr;     // [s][3][z][k] workspace: u_par, u_perp, T of the Dougherty operator
     float dky = 0;
     bool any_nu = false;
@@ -58,6 +67,7 @@ inline void lin_tables_free(LinTables& t) {
     cudaFree(t.Jl); cudaFree(t.invD); cudaFree(t.fsfac); cudaFree(t.wz); cudaFree(t.bs);
     cudaFree(t.Dz); cudaFree(t.Az); cudaFree(t.omd); cudaFree(t.hypv); cudaFree(t.bgrad);
     cudaFree(t.mpow); cudaFree(t.mom);
+    cudaFree(t.chain_off); cudaFree(t.chain_mode); cudaFree(t.ext_off); cudaFree(t.ext_d); cudaFree(t.ext_a);
     t = LinTables();
 }
 
@@ -168,6 +178,55 @@ inline bool lin_tables_build(const LinHostInput& in, LinTables& t, size_t& bytes
     {
         std::vector<float2> zero((size_t)Ns * 3 * Nz * nk, make_float2(0.f, 0.f));
         if (!lin_upload(&t.mom, zero, bytes, msg)) return false;
+    }
+    t.linked = in.linked;
+    if (in.linked) {
+        const double jt = 2.0 * M_PI * in.shat * in.dky / in.dkx;
+        const int jtw = (int)std::lround(jt);
+        if (std::abs(jt - jtw) > 1e-6 || jtw == 0) { msg = "box is not twist-shift quantised: 2 pi shat dky/dkx is not a non-zero integer"; return false; }
+        std::vector<int> coff{0}, cmode, eoff;
+        std::vector<int> len_off(nakx + 2, -1);
+        std::vector<float> ed, ea;
+        int max_ext = 0;
+        auto row_of = [&](int pidx) { return pidx >= 0 ? pidx : pidx + nakx; };
+        for (int q = 0; q < naky; ++q) {
+            const int step = jtw * q;
+            for (int pidx = -K; pidx <= K; ++pidx) {
+                std::vector<int> members;
+                if (step == 0) members.push_back(pidx);
+                else {
+                    if (std::abs(pidx - step) <= K) continue;            // has a predecessor in the dealiased set
+                    for (int pp = pidx; std::abs(pp) <= K; pp += step) members.push_back(pp);
+                }
+                const int L = (int)members.size();
+                // mode n holds theta = z - 2 pi n: increasing ballooning angle runs n = L-1, ..., 0
+                for (int n = L - 1; n >= 0; --n) cmode.push_back(row_of(members[n]) * naky + q);
+                coff.push_back((int)cmode.size());
+                if (len_off[L] < 0) {
+                    len_off[L] = (int)ed.size();
+                    const int N = L * Nz;
+                    for (int d = 0; d < N; ++d) {
+                        double sd = 0, sa = 0;
+                        for (int jj = 0; jj < N; ++jj) {
+                            const int j = jj <= N / 2 ? jj : jj - N;
+                            const double ang = 2.0 * M_PI * (double)j * d / N;
+                            if (!(N % 2 == 0 && jj == N / 2)) sd -= ((double)j / L) * std::sin(ang);
+                            sa += (std::abs((double)j) / L) * std::cos(ang);
+                        }
+                        ed.push_back((float)(in.gradpar * sd / N));
+                        ea.push_back((float)(std::abs(in.gradpar) * sa / N));
+                    }
+                }
+                eoff.push_back(len_off[L]);
+                max_ext = std::max(max_ext, L * Nz);
+            }
+        }
+        t.nchain = (int)eoff.size();
+        t.max_ext = max_ext;
+        if (!lin_upload(&t.chain_off, coff, bytes, msg) || !lin_upload(&t.chain_mode, cmode, bytes, msg) ||
+            !lin_upload(&t.ext_off, eoff, bytes, msg) || !lin_upload(&t.ext_d, ed, bytes, msg) ||
+            !lin_upload(&t.ext_a, ea, bytes, msg))
+            return false;
     }
     if (!lin_upload(&t.Jl, Jl, bytes, msg) || !lin_upload(&t.bs, bs, bytes, msg) ||
         !lin_upload(&t.invD, invD, bytes, msg) || !lin_upload(&t.fsfac, fsfac, bytes, msg) ||
@@ -294,7 +353,7 @@ constexpr int kLinZG = 8;       // z groups per block
 template <bool ACC, int ZB, bool DERIV_ONLY = false>
 __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, const float2* __restrict__ g,
                                                                  const float2* __restrict__ phi,
-                                                                 float2* __restrict__ out) {
+                                                                 float2* __restrict__ out, const bool skip_z) {
     extern __shared__ __align__(16) unsigned char lin_smem[];
     float2* S1 = reinterpret_cast<float2*>(lin_smem);            // [Nz][TK] sqrt(m+1) H_{l,m+1} + sqrt(m) H_{l,m-1}
     float2* S2 = S1 + (size_t)t.Nz * kLinTK;                     // [Nz][TK] G_{l,m} (hyper-collisions)
@@ -392,8 +451,10 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
                   }
               }
           };
-          blocked(dz, S1 + tk, dpb);
-          if (hyp != 0.f) blocked(az, S2 + tk, apb);
+          if (!skip_z) {                        // linked boundary: the z operators come from lin_zlink_kernel
+              blocked(dz, S1 + tk, dpb);
+              if (hyp != 0.f) blocked(az, S2 + tk, apb);
+          }
       }
 #pragma unroll
       for (int zi = 0; zi < ZB; ++zi) {
@@ -580,6 +641,104 @@ __global__ void __launch_bounds__(256) lin_point_kernel(LinTables t, const float
     }
 }
 
+// Twist-and-shift linked z operators (Eq. 4.29): one block per chain of linked modes and (s,m);
+// the chain's extended periodic domain (L segments of Nz points, in order of increasing ballooning angle) is
+// staged in shared memory for every l in turn and the two circulant products are added to out.
+template <int ZB>
+__global__ void __launch_bounds__(128) lin_zlink_kernel(LinTables t, const float2* __restrict__ g,
+                                                        const float2* __restrict__ phi, float2* __restrict__ out) {
+    extern __shared__ __align__(16) unsigned char lin_smem[];
+    const int c = blockIdx.x;
+    const int s = blockIdx.y / t.Nm, m = blockIdx.y % t.Nm;
+    const int off = t.chain_off[c], L = t.chain_off[c + 1] - off, N = L * t.Nz;
+    float2* S1 = reinterpret_cast<float2*>(lin_smem);            // [N]
+    float2* S2 = S1 + t.max_ext;                                 // [N]
+    float* dcol = reinterpret_cast<float*>(S2 + t.max_ext);      // [2N] column repeated
+    float* acol = dcol + 2 * t.max_ext;
+    int* modes = reinterpret_cast<int*>(acol + 2 * t.max_ext);   // [L]
+    const float* __restrict__ ed = t.ext_d + t.ext_off[c];
+    const float* __restrict__ ea = t.ext_a + t.ext_off[c];
+    const float hyp = t.nuhyp[s] * t.mpow[m], vt = t.vt[s];
+    for (int i = threadIdx.x; i < 2 * N; i += blockDim.x) {
+        const int d = i < N ? i : i - N;
+        dcol[i] = ed[d];
+        acol[i] = ea[d];
+    }
+    for (int i = threadIdx.x; i < L; i += blockDim.x) modes[i] = t.chain_mode[off + i];
+    const unsigned pl = (unsigned)(t.Nz * t.nk);
+    const bool vp = m + 1 < t.Nm, vm = m - 1 >= 0;
+    const float cp = vp ? sqrtf((float)(m + 1)) : 0.f, cm = vm ? sqrtf((float)m) : 0.f;
+    const float cphi = (vm && m == 1) ? cm * t.zt[s] : 0.f;
+    for (int l = 0; l < t.Nl; ++l) {
+        __syncthreads();
+        const unsigned ip = (unsigned)((s * t.Nm + (vp ? m + 1 : m)) * t.Nl + l) * pl,
+                       im = (unsigned)((s * t.Nm + (vm ? m - 1 : m)) * t.Nl + l) * pl,
+                       i0 = (unsigned)((s * t.Nm + m) * t.Nl + l) * pl, ij = (unsigned)(s * t.Nl + l) * pl;
+        for (int i = threadIdx.x; i < N; i += blockDim.x) {
+            const int seg = i / t.Nz, z = i - seg * t.Nz;
+            const unsigned zk = (unsigned)(z * t.nk + modes[seg]);
+            const float2 a = g[ip + zk], b = g[im + zk];
+            float2 v = make_float2(cp * a.x + cm * b.x, cp * a.y + cm * b.y);
+            if (cphi != 0.f) {
+                const float w = cphi * t.Jl[ij + zk];
+                const float2 f = phi[zk];
+                v.x = fmaf(w, f.x, v.x);
+                v.y = fmaf(w, f.y, v.y);
+            }
+            S1[i] = v;
+            S2[i] = g[i0 + zk];
+        }
+        __syncthreads();
+        for (int zb = threadIdx.x; zb * ZB < N; zb += blockDim.x) {
+            const int z0 = zb * ZB;
+            float2 dp[ZB], ap[ZB];
+#pragma unroll
+            for (int i = 0; i < ZB; ++i) dp[i] = ap[i] = make_float2(0.f, 0.f);
+            auto blocked = [&](const float* __restrict__ col, const float2* __restrict__ sv, float2 (&acc)[ZB]) {
+                const float* __restrict__ dc = col + z0 + N;               // weight of (z0 + i, zp) = dc[i - zp]
+                if constexpr (ZB == 4) {
+                    float w0 = dc[0], w1 = dc[1], w2 = dc[2], w3 = dc[3];
+                    for (int zp = 0; zp < N; zp += 4) {
+                        const float2 a0 = sv[zp], a1 = sv[zp + 1], a2 = sv[zp + 2], a3 = sv[zp + 3];
+                        const float n0 = dc[-(zp + 1)], n1 = dc[-(zp + 2)], n2 = dc[-(zp + 3)], n3 = dc[-(zp + 4)];
+                        acc[0].x = fmaf(w0, a0.x, acc[0].x); acc[0].y = fmaf(w0, a0.y, acc[0].y);
+                        acc[1].x = fmaf(w1, a0.x, acc[1].x); acc[1].y = fmaf(w1, a0.y, acc[1].y);
+                        acc[2].x = fmaf(w2, a0.x, acc[2].x); acc[2].y = fmaf(w2, a0.y, acc[2].y);
+                        acc[3].x = fmaf(w3, a0.x, acc[3].x); acc[3].y = fmaf(w3, a0.y, acc[3].y);
+                        acc[0].x = fmaf(n0, a1.x, acc[0].x); acc[0].y = fmaf(n0, a1.y, acc[0].y);
+                        acc[1].x = fmaf(w0, a1.x, acc[1].x); acc[1].y = fmaf(w0, a1.y, acc[1].y);
+                        acc[2].x = fmaf(w1, a1.x, acc[2].x); acc[2].y = fmaf(w1, a1.y, acc[2].y);
+                        acc[3].x = fmaf(w2, a1.x, acc[3].x); acc[3].y = fmaf(w2, a1.y, acc[3].y);
+                        acc[0].x = fmaf(n1, a2.x, acc[0].x); acc[0].y = fmaf(n1, a2.y, acc[0].y);
+                        acc[1].x = fmaf(n0, a2.x, acc[1].x); acc[1].y = fmaf(n0, a2.y, acc[1].y);
+                        acc[2].x = fmaf(w0, a2.x, acc[2].x); acc[2].y = fmaf(w0, a2.y, acc[2].y);
+                        acc[3].x = fmaf(w1, a2.x, acc[3].x); acc[3].y = fmaf(w1, a2.y, acc[3].y);
+                        acc[0].x = fmaf(n2, a3.x, acc[0].x); acc[0].y = fmaf(n2, a3.y, acc[0].y);
+                        acc[1].x = fmaf(n1, a3.x, acc[1].x); acc[1].y = fmaf(n1, a3.y, acc[1].y);
+                        acc[2].x = fmaf(n0, a3.x, acc[2].x); acc[2].y = fmaf(n0, a3.y, acc[2].y);
+                        acc[3].x = fmaf(w0, a3.x, acc[3].x); acc[3].y = fmaf(w0, a3.y, acc[3].y);
+                        w3 = n0; w2 = n1; w1 = n2; w0 = n3;
+                    }
+                } else {
+                    for (int zp = 0; zp < N; ++zp) {
+                        const float w = dc[-zp];
+                        acc[0].x = fmaf(w, sv[zp].x, acc[0].x); acc[0].y = fmaf(w, sv[zp].y, acc[0].y);
+                    }
+                }
+            };
+            blocked(dcol, S1, dp);
+            if (hyp != 0.f) blocked(acol, S2, ap);
+#pragma unroll
+            for (int i = 0; i < ZB; ++i) {
+                const int zi = z0 + i, seg = zi / t.Nz, z = zi - seg * t.Nz;
+                float2* __restrict__ o = out + (i0 + (unsigned)(z * t.nk + modes[seg]));
+                const float2 prev = *o;
+                *o = make_float2(prev.x - vt * dp[i].x - hyp * ap[i].x, prev.y - vt * dp[i].y - hyp * ap[i].y);
+            }
+        }
+    }
+}
+
 inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* phi, float2* out, bool accumulate,
                            cudaStream_t st) {
     if (!t.built) return cudaErrorNotReady;
@@ -601,7 +760,8 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
     }
     dim3 grid((t.nk + kLinTK - 1) / kLinTK, t.Nl, t.Ns * t.Nm);
     const bool b4 = t.Nz % 4 == 0;
-    if (t.Nl <= 4) {
+    const bool split = t.Nl <= 4 || t.linked;
+    if (split && t.Nl <= 8) {
         // pointwise terms with the stencil in registers, then the z-operator terms added on top (measured faster
         // for Nl <= 4 only: with 8 Laguerre moments the 5 x 10 stencil costs 135 registers and the occupancy)
         dim3 gp((unsigned)(((size_t)t.Nz * t.nk + 255) / 256), t.Ns * t.Nm);
@@ -612,14 +772,30 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
             if (accumulate) lin_point_kernel<8, true><<<gp, 256, 0, st>>>(t, g, phi, out);
             else lin_point_kernel<8, false><<<gp, 256, 0, st>>>(t, g, phi, out);
         }
-        if (b4) lin_rhs_kernel<true, 4, true><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
-        else lin_rhs_kernel<true, 1, true><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+        if (!t.linked) {
+            if (b4) lin_rhs_kernel<true, 4, true><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false);
+            else lin_rhs_kernel<true, 1, true><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false);
+        }
     } else if (accumulate) {
-        if (b4) lin_rhs_kernel<true, 4><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
-        else lin_rhs_kernel<true, 1><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+        if (b4) lin_rhs_kernel<true, 4><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, t.linked);
+        else lin_rhs_kernel<true, 1><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, t.linked);
     } else {
-        if (b4) lin_rhs_kernel<false, 4><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
-        else lin_rhs_kernel<false, 1><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out);
+        if (b4) lin_rhs_kernel<false, 4><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, t.linked);
+        else lin_rhs_kernel<false, 1><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, t.linked);
+    }
+    if (t.linked) {
+        const size_t sm = (size_t)t.max_ext * (2 * sizeof(float2) + 4 * sizeof(float)) + (size_t)(t.max_ext / t.Nz) * sizeof(int);
+        static bool attr2 = false;
+        if (!attr2) {
+            cudaError_t e = cudaFuncSetAttribute(lin_zlink_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+            if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_zlink_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+            if (e != cudaSuccess) return e;
+            attr2 = true;
+        }
+        if (sm > 200 * 1024) return cudaErrorInvalidConfiguration;
+        dim3 gl(t.nchain, t.Ns * t.Nm);
+        if (b4) lin_zlink_kernel<4><<<gl, 128, sm, st>>>(t, g, phi, out);
+        else lin_zlink_kernel<1><<<gl, 128, sm, st>>>(t, g, phi, out);
     }
     return cudaGetLastError();
 }

@@ -381,3 +381,44 @@ def test_calls_on_a_side_stream_and_interleaved_grids(torch_cuda):
         ref = _oracle_nl(cfg, geo, G, Phi, method="dft")
         assert O.relative_max_error(out.cpu().numpy(), ref) <= TOL
         grid.close()
+
+
+@pytest.mark.parametrize("name", ["tiny", "cyclone", "kinetic"])
+def test_linear_rhs_parity_with_twist_shift_linking(torch_cuda, name):
+    """gx_boundary_set(1): the z operators act on the linked extended domains of Eq. 4.29."""
+    torch = torch_cuda
+    from paper_2209_06731_b200 import binding
+    cfg = I.named_config(name)
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = binding.Grid(cfg, geo, linked=True)
+    g, phi = torch.from_numpy(G).cuda(), torch.from_numpy(Phi).cuda()
+    out = torch.full_like(g, float("nan"))
+    grid.linear_rhs(g, phi, out)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    ref = OL.linear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, boundary="linked")
+    per = OL.linear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, boundary="periodic")
+    assert np.all(np.isfinite(out))
+    assert O.relative_max_error(out, ref) <= TOL
+    assert O.relative_max_error(per, ref) > 100 * TOL           # the linking really changes the answer
+    for s in range(cfg.Ns):
+        for m in range(cfg.Nm):
+            assert O.relative_max_error(out[s, m], ref[s, m]) <= 5 * TOL, (s, m)
+    grid.close()
+
+
+def test_linked_boundary_needs_a_quantised_box(torch_cuda):
+    from paper_2209_06731_b200 import binding as B
+    cfg = I.named_config("tiny")
+    geo = I.geometry_arrays(cfg)
+    h = B.gx_grid_create(cfg.Nx, cfg.Ny, cfg.Nz, cfg.Nl, cfg.Nm, 1)
+    B.gx_box_set(h, cfg.dky, 1.0123 * cfg.dkx, cfg.shat)
+    B.gx_species_set(h, 0, 1.0, 1.0, 1.0, 1.0)
+    B.gx_boundary_set(h, 1)
+    with pytest.raises(B.GxError) as e:
+        B.gx_geometry_set(h, geo["bmag"], geo["gds2"], geo["gds21"], geo["gds22"], geo["gbdrift"], geo["gbdrift0"],
+                          geo["cvdrift"], geo["cvdrift0"], geo["bgrad"], geo["jacobian"], geo["gradpar"])
+    assert e.value.code == B.GX_ERR_ARG
+    B.gx_grid_destroy(h)
