@@ -312,6 +312,13 @@ def run_gpu(args):
 
     n_aux = max(3, min(args.steps, 200))
     rhs_rate = timed(lambda i: grid.rhs(gs[i % nsets], outs[i % nsets]), n_aux)
+    rhs_linked_rate = None
+    try:                                  # same right-hand side with twist-and-shift linked z operators (Eq. 4.29)
+        grid_l = B.Grid(cfg, geo, linked=True)
+        rhs_linked_rate = timed(lambda i: grid_l.rhs(gs[i % nsets], outs[i % nsets]), n_aux)
+        grid_l.close()
+    except B.GxError:
+        pass
     g_rk = gs[0].clone()
     g_rk.mul_(1e-3)                       # small amplitude; dt from the parallel-streaming CFL (Eq. 5.5)
     vt_max = max(np.sqrt(sp.temp / sp.mass) for sp in cfg.species)
@@ -378,7 +385,8 @@ def run_gpu(args):
                         "d2h_bytes_per_step": g_elems * 8, "steps": e2e_steps},
                 "gpu_launches": launches_per_call * args.steps,
                 "kernel_family": B.FAMILY_NAMES.get(grid.query(B.GX_Q_KERNEL_FAMILY), "?"),
-                "gx_rhs": {"value": rhs_rate * world, "unit": "full rhs evals/s (field solve + nonlinear + linear)"},
+                "gx_rhs": {"value": rhs_rate * world, "unit": "full rhs evals/s (field solve + nonlinear + linear)",
+                           "twist_shift_linked": None if rhs_linked_rate is None else rhs_linked_rate * world},
                 "ssprk3": {"value": rk_rate * world, "unit": "SSP-RK3 steps/s (3 gx_rhs each)"},
                 "reference_point": ref_point,
                 "roofline": roofline,

@@ -52,6 +52,8 @@ struct LinTables {
     int* chain_off = nullptr;      // [nchain + 1] offsets into chain_mode
     int* chain_mode = nullptr;     // compact mode index k = kx_row * naky + ky, in order of increasing ballooning angle
     int* ext_off = nullptr;        // [nchain] offset of the chain's circulant columns in ext_d / ext_a
+    int* zwork = nullptr;          // [nzwork] (chain << 8 | slice): slices of kZlinkSlice outputs, longest chains first
+    int nzwork = 0, nzwork_long = 0, short_ext = 0;   // items [0, nzwork_long) have more than short_ext points
     float* ext_d = nullptr;        // per distinct length L: column of gradpar * d/dzeta, L*Nz entries
     float* ext_a = nullptr;        // per distinct length L: column of |gradpar| * |k_zeta|
     float2* mom = nullptr;     // [s][3][z][k] workspace: u_par, u_perp, T of the Dougherty operator
@@ -60,6 +62,7 @@ struct LinTables {
     bool built = false;
 };
 
+constexpr int kZlinkThreads = 64, kZlinkSlice = 4 * kZlinkThreads;   // outputs per block of lin_zlink_kernel
 constexpr int kLinLaunchesFieldSolve = 2;
 constexpr int kLinLaunchesRhs = 3;
 
@@ -67,7 +70,7 @@ inline void lin_tables_free(LinTables& t) {
     cudaFree(t.Jl); cudaFree(t.invD); cudaFree(t.fsfac); cudaFree(t.wz); cudaFree(t.bs);
     cudaFree(t.Dz); cudaFree(t.Az); cudaFree(t.omd); cudaFree(t.hypv); cudaFree(t.bgrad);
     cudaFree(t.mpow); cudaFree(t.mom);
-    cudaFree(t.chain_off); cudaFree(t.chain_mode); cudaFree(t.ext_off); cudaFree(t.ext_d); cudaFree(t.ext_a);
+    cudaFree(t.chain_off); cudaFree(t.chain_mode); cudaFree(t.ext_off); cudaFree(t.ext_d); cudaFree(t.ext_a); cudaFree(t.zwork);
     t = LinTables();
 }
 
@@ -223,6 +226,20 @@ inline bool lin_tables_build(const LinHostInput& in, LinTables& t, size_t& bytes
         }
         t.nchain = (int)eoff.size();
         t.max_ext = max_ext;
+        std::vector<int> order(t.nchain), work;
+        for (int c = 0; c < t.nchain; ++c) order[c] = c;
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return coff[a + 1] - coff[a] > coff[b + 1] - coff[b]; });
+        for (int c : order) {
+            const int N = (coff[c + 1] - coff[c]) * Nz;
+            for (int sl = 0; sl * kZlinkSlice < N; ++sl) work.push_back((c << 8) | sl);
+        }
+        t.nzwork = (int)work.size();
+        t.short_ext = std::min(max_ext, 4 * Nz);
+        t.nzwork_long = 0;
+        for (int w : work)
+            if ((coff[(w >> 8) + 1] - coff[w >> 8]) * Nz > t.short_ext) t.nzwork_long++;
+        if (max_ext > 255 * kZlinkSlice) { msg = "extended domain too long for the slice encoding"; return false; }
+        if (!lin_upload(&t.zwork, work, bytes, msg)) return false;
         if (!lin_upload(&t.chain_off, coff, bytes, msg) || !lin_upload(&t.chain_mode, cmode, bytes, msg) ||
             !lin_upload(&t.ext_off, eoff, bytes, msg) || !lin_upload(&t.ext_d, ed, bytes, msg) ||
             !lin_upload(&t.ext_a, ea, bytes, msg))
@@ -641,21 +658,23 @@ __global__ void __launch_bounds__(256) lin_point_kernel(LinTables t, const float
     }
 }
 
-// Twist-and-shift linked z operators (Eq. 4.29): one block per chain of linked modes and (s,m);
-// the chain's extended periodic domain (L segments of Nz points, in order of increasing ballooning angle) is
-// staged in shared memory for every l in turn and the two circulant products are added to out.
+// Twist-and-shift linked z operators (Eq. 4.29): one block per (slice of a chain of linked modes,
+// l, (s,m)); the chain's extended periodic domain (L segments of Nz points, in order of increasing ballooning
+// angle) is staged in shared memory and the two circulant products of the slice's outputs are added to out.
 template <int ZB>
-__global__ void __launch_bounds__(128) lin_zlink_kernel(LinTables t, const float2* __restrict__ g,
-                                                        const float2* __restrict__ phi, float2* __restrict__ out) {
+__global__ void __launch_bounds__(kZlinkThreads) lin_zlink_kernel(LinTables t, const float2* __restrict__ g,
+                                                                  const float2* __restrict__ phi,
+                                                                  float2* __restrict__ out, const int work0,
+                                                                  const int cap) {
     extern __shared__ __align__(16) unsigned char lin_smem[];
-    const int c = blockIdx.x;
-    const int s = blockIdx.y / t.Nm, m = blockIdx.y % t.Nm;
+    const int c = t.zwork[work0 + blockIdx.x] >> 8, slice = t.zwork[work0 + blockIdx.x] & 255;
+    const int s = blockIdx.z / t.Nm, m = blockIdx.z % t.Nm;
     const int off = t.chain_off[c], L = t.chain_off[c + 1] - off, N = L * t.Nz;
     float2* S1 = reinterpret_cast<float2*>(lin_smem);            // [N]
-    float2* S2 = S1 + t.max_ext;                                 // [N]
-    float* dcol = reinterpret_cast<float*>(S2 + t.max_ext);      // [2N] column repeated
-    float* acol = dcol + 2 * t.max_ext;
-    int* modes = reinterpret_cast<int*>(acol + 2 * t.max_ext);   // [L]
+    float2* S2 = S1 + cap;                                       // [N]   (cap >= N: points the launch provides for)
+    float* dcol = reinterpret_cast<float*>(S2 + cap);            // [2N] column repeated
+    float* acol = dcol + 2 * cap;
+    int* modes = reinterpret_cast<int*>(acol + 2 * cap);         // [L]
     const float* __restrict__ ed = t.ext_d + t.ext_off[c];
     const float* __restrict__ ea = t.ext_a + t.ext_off[c];
     const float hyp = t.nuhyp[s] * t.mpow[m], vt = t.vt[s];
@@ -669,7 +688,8 @@ __global__ void __launch_bounds__(128) lin_zlink_kernel(LinTables t, const float
     const bool vp = m + 1 < t.Nm, vm = m - 1 >= 0;
     const float cp = vp ? sqrtf((float)(m + 1)) : 0.f, cm = vm ? sqrtf((float)m) : 0.f;
     const float cphi = (vm && m == 1) ? cm * t.zt[s] : 0.f;
-    for (int l = 0; l < t.Nl; ++l) {
+    {
+        const int l = blockIdx.y;
         __syncthreads();
         const unsigned ip = (unsigned)((s * t.Nm + (vp ? m + 1 : m)) * t.Nl + l) * pl,
                        im = (unsigned)((s * t.Nm + (vm ? m - 1 : m)) * t.Nl + l) * pl,
@@ -689,8 +709,8 @@ __global__ void __launch_bounds__(128) lin_zlink_kernel(LinTables t, const float
             S2[i] = g[i0 + zk];
         }
         __syncthreads();
-        for (int zb = threadIdx.x; zb * ZB < N; zb += blockDim.x) {
-            const int z0 = zb * ZB;
+        const int lo = slice * kZlinkSlice, hi = min(N, lo + kZlinkSlice);
+        for (int z0 = lo + threadIdx.x * ZB; z0 < hi; z0 += blockDim.x * ZB) {
             float2 dp[ZB], ap[ZB];
 #pragma unroll
             for (int i = 0; i < ZB; ++i) dp[i] = ap[i] = make_float2(0.f, 0.f);
@@ -784,7 +804,6 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
         else lin_rhs_kernel<false, 1><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, t.linked);
     }
     if (t.linked) {
-        const size_t sm = (size_t)t.max_ext * (2 * sizeof(float2) + 4 * sizeof(float)) + (size_t)(t.max_ext / t.Nz) * sizeof(int);
         static bool attr2 = false;
         if (!attr2) {
             cudaError_t e = cudaFuncSetAttribute(lin_zlink_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -792,10 +811,18 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
             if (e != cudaSuccess) return e;
             attr2 = true;
         }
-        if (sm > 200 * 1024) return cudaErrorInvalidConfiguration;
-        dim3 gl(t.nchain, t.Ns * t.Nm);
-        if (b4) lin_zlink_kernel<4><<<gl, 128, sm, st>>>(t, g, phi, out);
-        else lin_zlink_kernel<1><<<gl, 128, sm, st>>>(t, g, phi, out);
+        // two launches: the few long chains with room for the longest extended domain, the many short ones
+        // (up to 4 links) with a small footprint so that 32 blocks fit an SM
+        const int w0[2] = {0, t.nzwork_long}, wn[2] = {t.nzwork_long, t.nzwork - t.nzwork_long};
+        const int cap[2] = {t.max_ext, t.short_ext};
+        for (int part = 0; part < 2; ++part) {
+            if (wn[part] <= 0) continue;
+            const size_t sm = (size_t)cap[part] * (2 * sizeof(float2) + 4 * sizeof(float)) + (size_t)(cap[part] / t.Nz) * sizeof(int);
+            if (sm > 200 * 1024) return cudaErrorInvalidConfiguration;
+            dim3 gl(wn[part], t.Nl, t.Ns * t.Nm);
+            if (b4) lin_zlink_kernel<4><<<gl, kZlinkThreads, sm, st>>>(t, g, phi, out, w0[part], cap[part]);
+            else lin_zlink_kernel<1><<<gl, kZlinkThreads, sm, st>>>(t, g, phi, out, w0[part], cap[part]);
+        }
     }
     return cudaGetLastError();
 }
