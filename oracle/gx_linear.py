@@ -46,7 +46,11 @@ streaming eigenvalues = Gauss-Hermite nodes; drift matrices' eigenvalues = Gauss
 squared Gauss-Hermite nodes (library quadrature routines the oracle does not call); 1/B-weighted
 free-energy identity of streaming + mirror; anti-Hermiticity of the drift terms; Dougherty conservation of
 density, momentum and energy at k_perp = 0 and its damping rates; hand values of the drive; closed forms
-of both hyper-dissipation terms; SSP-RK3 order on dy/dt = lambda y.
+of both hyper-dissipation terms; SSP-RK3 order on dy/dt = lambda y.  Finite Larmor radius: every coefficient
+of the Dougherty field-particle terms (Eq. 4.13-4.17) against the velocity-space operator Eq. 2.5-2.8 by
+library Gauss-Laguerre x Gauss-Hermite quadrature at b up to 0.25, Phi != 0, B != 1, Z, m, tau != 1; the
+drive's 1/L_n and 1/L_T brackets at finite b against the Maxwellian-gradient integrals; w_d^kappa with
+cvdrift != gbdrift against the s-alpha closed form.
 """
 from __future__ import annotations
 

@@ -34,6 +34,11 @@ Pins (tests/test_oracle_pins.py): Gauss-Laguerre J=2 closed form and moment exac
 Tinv*T = I; Eq. 4.7 closed form of the Laguerre-projected J0; sum_l J_l^2 -> I0(b)e^-b;
 single-mode bracket closed form; convolution == pseudo-spectral; free-energy invariant;
 b=0 reduction; Hermitian ky=0 output; the paper's printed dealiased counts.
+What pins the gyroaverage table INSIDE nonlinear_rhs (the factor 2 of alpha_s = sqrt(2 muB b_s), the
+1/B^2 and tau m/Z^2 of b_s): test_nonlinear_rhs_single_modes_finite_b_closed_form -- Phi and G_0 one
+Fourier mode each, J = 40 nodes, bmag != 1, Z, m, tau != 1, expected value -J_l(b_p) (p x q) Phi_p g_q with
+b_p written out by hand and J_l the closed form of Eq. 4.7 typed into the test; and
+test_b_species_hand_values.  field_solve with tau_fac != 1: test_field_solve_tau_fac_residual.
 Nothing here is "parity unpinned".
 """
 from __future__ import annotations
@@ -331,7 +336,7 @@ def nonlinear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, method="dft", pl
         if (s, z) not in Mcache:
             b = b_species(kp2[z:z + 1], np.asarray(geo["bmag"])[z:z + 1], Z, mass, temp)[0]
             if gyro == "exact":
-                Mcache[(s, z)] = np.stack([_sp.j0(np.sqrt(2.0 * xj * b)) for xj in x])
+                Mcache[(s, z)] = gyro_table(b[None], x)[0]                   # [j][kx][ky]
             else:
                 Mcache[(s, z)] = np.stack([sum(psi(l, xj) * jflr(l, b) for l in range(Nl)) for xj in x])
         M = Mcache[(s, z)]

@@ -8,6 +8,8 @@ import pytest
 from numpy.polynomial import hermite_e as HE
 from numpy.polynomial import laguerre as LA
 
+from scipy.special import eval_laguerre as special_eval_laguerre, j0 as special_j0, j1 as special_j1
+
 import gx_linear as L
 import gx_oracle as O
 
@@ -213,6 +215,127 @@ def test_dougherty_conserves_density_momentum_energy_and_damps_the_rest():
     assert np.allclose(r[0, 4, 1], -nu * (b + 2 + 4) * G[0, 4, 1])
     # free energy never grows under like-particle collisions
     assert np.all(np.sum(np.real(np.conj(G) * r), axis=(1, 2)) <= 1e-12)
+
+
+def _velocity_space_quadrature(nt=60, nv=40):
+    """Library quadrature in (mu B, v_par): d^3v F_M -> sum over (t_i, v_j) with weights wt_i wv_j, where
+    int_0^inf e^-t dt and int e^{-v^2/2}/sqrt(2 pi) dv are the two measures (Eq. 2.2; Eq. 4.1)."""
+    t, wt = LA.laggauss(nt)
+    v, wv = HE.hermegauss(nv)
+    return t, wt, v, wv / math.sqrt(2 * math.pi)
+
+
+def _finite_b_setup(Nl, Nm, seed):
+    """Two z points with B != 1, a species with Z, m, tau != 1, b_s between 0 and ~0.25 over the modes."""
+    Nz = 2
+    geo = dict(bmag=np.array([1.0, 1.3]), gds2=np.array([1.1, 0.8]), gds21=np.array([0.15, -0.2]),
+               gds22=np.array([0.64, 0.9]), gbdrift=np.zeros(Nz), gbdrift0=np.zeros(Nz), cvdrift=np.zeros(Nz),
+               cvdrift0=np.zeros(Nz), bgrad=np.zeros(Nz), jacobian=np.array([1.0, 1.0 / 1.3]), gradpar=0.7)
+    Zs, ms, ts = 2.0, 1.5, 0.8
+    kx, ky = DKX * O.kx_index(NX), DKY * O.ky_index(NY)
+    kxx, kyy = kx[None, :, None], ky[None, None, :]
+    kp2 = (kyy ** 2 * geo["gds2"][:, None, None] + 2 * kxx * kyy * geo["gds21"][:, None, None] / SHAT
+           + kxx ** 2 * geo["gds22"][:, None, None] / SHAT ** 2)
+    b = kp2 * ts * ms / (Zs ** 2 * geo["bmag"][:, None, None] ** 2)          # P:85, by hand
+    G = _rand((1, Nm, Nl, Nz, NAKX, NAKY), seed)
+    Phi = _rand((Nz, NAKX, NAKY), seed + 1)
+    # H_{l,m} = G_{l,m} + (Z/tau) J_l Phi delta_m0 (Eq. 4.8, P:207), J_l typed out from Eq. 4.7 (P:202)
+    H = G[0].copy()
+    for l in range(Nl):
+        H[0, l] += (Zs / ts) * ((-b / 2) ** l / math.factorial(l) * np.exp(-b / 2)) * Phi
+    return geo, (Zs, ms, ts), b, G, Phi, H, ky
+
+
+def test_dougherty_field_particle_terms_from_the_velocity_space_operator_at_finite_b():
+    """Eq. 2.5-2.8 evaluated in velocity space by library Gauss-Laguerre x Gauss-Hermite quadrature
+    and projected with Eq. 4.1: the field-particle moments u_par, u_perp, T_par, T_perp (Eq. 4.14-4.17,
+    P:251-258) of h = sum_{l,m} H_{l,m} psi_l phi_m F_M and the Laguerre-Hermite transform of
+    ( T [(v^2-1) + 2(muB-1)] J0 + u_par v J0 + u_perp v_perp J1 ) F_M, at finite b, Phi != 0, B != 1.
+    Nl = 6 and b <= 0.25 keep the one difference -- the paper sets J_l = 0 for l >= Nl, the integral
+    does not -- below 1e-6.  A wrong sign, power of b, index shift or H<->G in Eq. 4.13-4.17 fails."""
+    Nl, Nm, nu = 6, 4, 0.37
+    geo, (Zs, ms, ts), b, G, Phi, H, _ = _finite_b_setup(Nl, Nm, 41)
+    assert 0.2 < b.max() < 0.3
+    sp = dict(Z=Zs, mass=ms, temp=ts, dens=1.0, tprim=0, fprim=0, nu_ss=nu)
+    r = _lin(G, Phi, geo, sp, ("coll",))[0]                                  # [m][l][z][kx][ky]
+    t, wt, v, wv = _velocity_space_quadrature()
+    psi = np.array([(-1.0) ** l * special_eval_laguerre(l, t) for l in range(Nl)])      # [l][t]
+    phi = np.array([_phi_hermite(m, v) for m in range(Nm)])                              # [m][v]
+    alpha = np.sqrt(2.0 * t[None, None, None, :] * b[..., None])                         # [z][kx][ky][t]
+    J0, J1 = special_j0(alpha), special_j1(alpha)
+    vperp = np.sqrt(2.0 * t)
+    # hhat(t, v) = sum H_{l,m} psi_l(t) phi_m(v): h = hhat F_M
+    hhat = np.einsum("mlzxy,lt,mv->zxytv", H, psi, phi)
+    W = wt[:, None] * wv[None, :]                                                        # [t][v]
+    upar = np.einsum("zxytv,zxyt,v,tv->zxy", hhat, J0, v, W)
+    uperp = np.einsum("zxytv,zxyt,t,tv->zxy", hhat, J1, vperp, W)
+    Tpar = np.einsum("zxytv,zxyt,v,tv->zxy", hhat, J0, v ** 2 - 1, W)
+    Tperp = np.einsum("zxytv,zxyt,t,tv->zxy", hhat, J0, t - 1, W)
+    Tbar = (Tpar + 2 * Tperp) / 3                                                        # Eq. 2.8 / 4.18
+    one_t, one_v = np.ones_like(t), np.ones_like(v)
+    bracket = (Tbar[..., None, None] * ((v ** 2 - 1)[None, :] * one_t[:, None] + 2 * (t - 1)[:, None] * one_v[None, :])
+               * J0[..., None]
+               + upar[..., None, None] * v[None, :] * J0[..., None]
+               + uperp[..., None, None] * (vperp[:, None] * one_v[None, :]) * J1[..., None])          # [z][kx][ky][t][v]
+    FP = np.einsum("zxytv,lt,mv,tv->mlzxy", bracket, psi, phi, W)
+    expect = np.empty_like(r)
+    for m in range(Nm):
+        for l in range(Nl):
+            expect[m, l] = -nu * (b + 2 * l + m) * H[m, l] + nu * FP[m, l]
+    scale = np.max(np.abs(expect))
+    assert np.max(np.abs(r - expect)) < 2e-6 * scale
+    # the field-particle part is not small: without it the comparison fails by O(1e-2)
+    assert np.max(np.abs(nu * FP[:3])) > 1e-2 * scale
+    # and it only reaches m = 0, 1, 2
+    assert np.max(np.abs(FP[3])) < 1e-12 * scale
+
+
+def test_drive_terms_at_finite_larmor_radius_from_the_maxwellian_gradient():
+    """Eq. 4.12, Phi parts: the drive is i w_* <J0 Phi> [1/L_n + (E - 3/2)/L_T] F_M with
+    E = v^2/2 + muB (grad F_M at constant energy, Eq. 2.1-2.2), transformed with Eq. 4.1:
+    D_{l,0} = i ky Phi int psi_l J0 [fprim + tprim (t - 1)] e^-t dt,  D_{l,2} = i ky Phi tprim/sqrt2 int psi_l J0 e^-t dt,
+    by library Gauss-Laguerre quadrature at finite b (the b = 0 hand values are a separate test)."""
+    Nl, Nm = 6, 4
+    geo, (Zs, ms, ts), b, G, Phi, H, ky = _finite_b_setup(Nl, Nm, 43)
+    sp = dict(Z=Zs, mass=ms, temp=ts, dens=1.0, tprim=6.9, fprim=2.2, nu_ss=0)
+    r = _lin(np.zeros_like(G), Phi, geo, sp, ("drive",))[0]
+    t, wt, v, wv = _velocity_space_quadrature()
+    J0 = special_j0(np.sqrt(2.0 * t[None, None, None, :] * b[..., None]))
+    iky = 1j * ky[None, None, :]
+    s0 = np.max(np.abs(6.9 * iky * Phi))
+    for l in range(Nl):
+        psi_l = (-1.0) ** l * special_eval_laguerre(l, t)
+        d0 = np.einsum("zxyt,t->zxy", J0, wt * psi_l * (2.2 + 6.9 * (t - 1.0)))
+        d2 = np.einsum("zxyt,t->zxy", J0, wt * psi_l) * 6.9 / math.sqrt(2.0)
+        assert np.max(np.abs(r[0, l] - iky * d0 * Phi)) < 2e-6 * s0, l
+        assert np.max(np.abs(r[2, l] - iky * d2 * Phi)) < 2e-6 * s0, l
+        assert np.all(r[1, l] == 0) and np.all(r[3, l] == 0)
+    assert np.max(np.abs(r[0, 1])) > 0.05 * s0 and np.max(np.abs(r[0, 2])) > 1e-3 * s0       # finite-b parts are visible
+
+
+def test_curvature_drift_frequency_with_a_pressure_term():
+    """w_d^kappa = (ky cvdrift + kx cvdrift0/shat)/2 (reading L3; Eq. E10-E11) with cvdrift != gbdrift:
+    s-alpha arrays plus a constant pressure-gradient part c0 in cvdrift  =>
+    w_d^kappa = ky (cos z + shat z sin z + c0/2) - kx sin z, w_d^gradB without c0; and the curvature term of
+    Eq. 4.9 is -i (tau/Z) w_d^kappa <phi_m'| v^2 |phi_m> H (Gauss-Hermite matrix elements)."""
+    Nz, Nm, Nl, c0 = 4, 5, 2, 0.6
+    geo, z = _geo(Nz, flat=True)
+    geo = dict(geo, cvdrift=geo["gbdrift"] + c0)
+    kx, ky = DKX * O.kx_index(NX), DKY * O.ky_index(NY)
+    zz = z[:, None, None]
+    wk_hand = ky[None, None, :] * (np.cos(zz) + SHAT * zz * np.sin(zz) + c0 / 2) - kx[None, :, None] * np.sin(zz)
+    wb_hand = ky[None, None, :] * (np.cos(zz) + SHAT * zz * np.sin(zz)) - kx[None, :, None] * np.sin(zz)
+    wk, wb = L.drift_frequencies(kx, ky, geo, SHAT)
+    assert np.allclose(wk, wk_hand, atol=1e-14) and np.allclose(wb, wb_hand, atol=1e-14)
+    sp = dict(Z=-1.0, mass=1.0, temp=2.0, dens=1.0, tprim=0, fprim=0, nu_ss=0)
+    G = _rand((1, Nm, Nl, Nz, NAKX, NAKY), 47)
+    xh, wh = HE.hermegauss(40)
+    wh = wh / math.sqrt(2 * math.pi)
+    MH = np.array([[np.sum(wh * _phi_hermite(a, xh) * xh ** 2 * _phi_hermite(c, xh)) for c in range(Nm)]
+                   for a in range(Nm)])
+    geo_k = dict(geo, gbdrift=np.zeros(Nz), gbdrift0=np.zeros(Nz))
+    rk = _lin(G, np.zeros((Nz, NAKX, NAKY)), geo_k, sp, ("drift",))
+    assert np.allclose(rk[0], -1j * (2.0 / -1.0) * wk_hand * np.einsum("ab,blzxy->alzxy", MH, G[0]), atol=1e-11)
 
 
 # ---------------------------------------------------------------------------- hyper-dissipation (P:300, P:311-316)

@@ -310,8 +310,10 @@ def test_series_gyroaverage_variant_close_to_exact_at_small_b(tiny):
     cfg, geo, G, Phi = tiny
     a = _nl(cfg, geo, G, Phi, gyro="exact", planes=[(0, 0, 4)])
     b = _nl(cfg, geo, G, Phi, gyro="series", planes=[(0, 0, 4)])
-    # the two tables agree where b is small (low k); overall they differ by the Laguerre truncation
-    assert 1e-6 < O.relative_max_error(b, a) < 0.5
+    # the two tables agree where b is small (low k) and differ by the Laguerre truncation elsewhere: the table
+    # difference is bounded term by term in test_series_gyroaverage_variant_within_truncation_bound; here only
+    # that the switch reaches the bracket (the outputs differ, by less than the largest table difference 0.25)
+    assert 1e-4 < O.relative_max_error(b, a) < 0.25
 
 
 def test_more_mu_nodes_do_not_change_polynomial_part(tiny):
@@ -327,6 +329,93 @@ def test_more_mu_nodes_do_not_change_polynomial_part(tiny):
     assert O.relative_max_error(b, a) < 1e-12
     assert O.relative_max_error(c, a) > 1e-3
 
+
+# ------------------------------------------------------------------ gyroaverage table inside nonlinear_rhs
+def _jflr_by_hand(l, b):
+    """Eq. 4.7 typed out again here: (1/l!) (-b/2)^l e^{-b/2}."""
+    return (1.0 / math.factorial(l)) * (-b / 2.0) ** l * math.exp(-b / 2.0)
+
+
+def test_b_species_hand_values():
+    # P:85: b_s = kperp^2 rho_s^2, rho_s = m_s v_ts/(Z_s B), v_ts = sqrt(tau_s/m_s)  =>  rho_s^2 = tau m/(Z^2 B^2)
+    # kperp2 = 2.0, B = 2, Z = 2, m = 3, tau = 0.5:  2.0 * (0.5*3) / (4 * 4) = 0.1875
+    b = O.b_species(np.full((1, 1, 1), 2.0), np.array([2.0]), 2.0, 3.0, 0.5)
+    assert abs(b[0, 0, 0] - 0.1875) < 1e-15
+    # B enters squared and per z
+    b2 = O.b_species(np.full((2, 1, 1), 2.0), np.array([1.0, 3.0]), 1.0, 1.0, 1.0)
+    assert abs(b2[0, 0, 0] - 2.0) < 1e-15 and abs(b2[1, 0, 0] - 2.0 / 9.0) < 1e-15
+
+
+@pytest.mark.parametrize("method", ["conv_np", "dft"])
+def test_nonlinear_rhs_single_modes_finite_b_closed_form(method):
+    """Through nonlinear_rhs itself, at finite Larmor radius: Phi = one Fourier mode p (plus its reality
+    partner), G non-zero only in l' = 0 and there one mode q  =>  gt_j = G_0 for every node (psi_0 = 1),
+    chi_j = J0(sqrt(2 x_j b_p)) Phi, and with many nodes (J = 40) the quadrature sum over j is the Laguerre
+    projection of J0, Eq. 4.7:
+
+        out[l] at k = p+q :  -J_l(b_p) (p_x q_y - p_y q_x) Phi_p g_q
+        out[l] at k = q-p :  +J_l(b_p) (p_x q_y - p_y q_x) conj(Phi_p) g_q        (b(-p) = b(p))
+
+    b_p = kperp2(p,z) tau m / (Z^2 B(z)^2) is written out by hand from P:85 and P:681-686 with B != 1 and
+    Z, m, tau != 1.  Catches: the factor 2 in alpha_s = sqrt(2 muB b_s), 1/B instead of 1/B^2, a wrong
+    rho_s, a table built at the wrong z or for the wrong mode."""
+    Nx = Ny = 16
+    nakx, naky = O.dealiased_counts(Nx, Ny)
+    Nz, Nl, Nm = 3, 3, 2
+    dkx, dky, shat = 0.9, 0.7, 0.8
+    geo = dict(bmag=np.array([1.0, 2.0, 0.7]), gds2=np.array([1.3, 0.9, 2.0]),
+               gds21=np.array([0.2, -0.4, 0.1]), gds22=np.array([0.64, 1.1, 0.8]))
+    Zs, ms, ts = 2.0, 3.0, 0.5
+    sp = [dict(Z=Zs, mass=ms, temp=ts, dens=1.0)]
+    (pa, pb), (qa, qb) = (2, 1), (-1, 3)
+    cp = np.array([0.8 - 0.3j, -0.2 + 0.9j, 1.1 + 0.4j])
+    gq = np.array([[-0.5 + 1.1j, 0.3 - 0.7j, 0.6 + 0.2j], [0.9 + 0.1j, -1.2 + 0.5j, 0.25 - 0.8j]])   # [m][z]
+    Phi = np.zeros((Nz, nakx, naky), complex)
+    G = np.zeros((1, Nm, Nl, Nz, nakx, naky), complex)
+    for z in range(Nz):
+        Phi[z] = _single_mode(nakx, naky, pa, pb, cp[z])
+        for m in range(Nm):
+            G[0, m, 0, z] = _single_mode(nakx, naky, qa, qb, gq[m, z])
+    out = O.nonlinear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, sp, method=method, J=40)
+    px, py, qx, qy = dkx * pa, dky * pb, dkx * qa, dky * qb
+    cross = px * qy - py * qx
+    i_sum, i_dif = (pa + qa) % nakx, (qa - pa) % nakx
+    expect = np.zeros_like(out)
+    bs = []
+    for z in range(Nz):
+        kp2 = py * py * geo["gds2"][z] + 2 * px * py * geo["gds21"][z] / shat + px * px * geo["gds22"][z] / shat ** 2
+        b = kp2 * ts * ms / (Zs ** 2 * geo["bmag"][z] ** 2)
+        bs.append(b)
+        for m in range(Nm):
+            for l in range(Nl):
+                expect[0, m, l, z, i_sum, pb + qb] = -_jflr_by_hand(l, b) * cross * cp[z] * gq[m, z]
+                expect[0, m, l, z, i_dif, qb - pb] = +_jflr_by_hand(l, b) * cross * np.conj(cp[z]) * gq[m, z]
+    assert min(bs) > 0.05 and max(bs) > 0.5          # the Larmor-radius factor is far from 1
+    assert np.max(np.abs(out - expect)) < 1e-9 * np.max(np.abs(expect))
+    assert np.count_nonzero(np.abs(out) > 1e-9) == 2 * Nm * Nl * Nz
+    # with the default node count J = floor((3 Nl - 1)/2) the l' = 0 data only needs the projection of J0 onto
+    # degree < Nl polynomials: out[l] = -(sum_j w_j psi_l(x_j) J0(sqrt(2 x_j b))) C -- library quadrature nodes
+    out_d = O.nonlinear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, sp, method=method)
+    xr, wr = np.polynomial.laguerre.laggauss((3 * Nl - 1) // 2)
+    for z in range(Nz):
+        for l in range(Nl):
+            lag = (-1.0) ** l * special.eval_laguerre(l, xr)
+            proj = np.sum(wr * lag * special.j0(np.sqrt(2 * xr * bs[z])))
+            assert abs(out_d[0, 1, l, z, i_sum, pb + qb] - (-proj * cross * cp[z] * gq[1, z])) < 1e-12
+
+
+def test_series_gyroaverage_variant_within_truncation_bound(tiny):
+    """gyro="series" replaces J0(sqrt(2 x b)) by its Nl-term Laguerre series sum_l psi_l(x) J_l(b); the first
+    neglected term bounds the difference of the tables: |M_exact - M_series| <= sum_{l>=Nl} |psi_l(x_j) J_l(b)|."""
+    cfg, geo, G, Phi = tiny
+    x, w = O.gauss_laguerre(cfg.nj)
+    kx, ky = cfg.dkx * O.kx_index(cfg.Nx), cfg.dky * O.ky_index(cfg.Ny)
+    b = O.b_species(O.kperp2(kx, ky, geo["gds2"], geo["gds21"], geo["gds22"], cfg.shat), geo["bmag"], 1, 1, 1)
+    exact = O.gyro_table(b, x)
+    series = np.stack([sum(O.psi(l, xj) * O.jflr(l, b) for l in range(cfg.Nl)) for xj in x], axis=1)
+    tail = np.stack([sum(np.abs(O.psi(l, xj) * O.jflr(l, b)) for l in range(cfg.Nl, 80)) for xj in x], axis=1)
+    assert np.all(np.abs(exact - series) <= tail + 1e-13)
+    assert np.max(np.abs(exact - series)) > 1e-4          # and the bound is not vacuous
 
 # ------------------------------------------------------------------ field solve
 def test_field_solve_satisfies_eq_6_1(tiny):
@@ -346,6 +435,30 @@ def test_field_solve_satisfies_eq_6_1(tiny):
     res[:, 0, 0] = 0
     assert np.max(np.abs(res)) < 1e-12 * np.max(np.abs(Phi))
     assert np.all(Phi[:, 0, 0] == 0)
+
+
+def test_field_solve_tau_fac_residual(tiny):
+    """Eq. 6.1 with tau_fac = T_i/T_e != 1 (reading R20): sum_l J_l H_{l,0} = tau_fac (Phi - <<Phi>>) + Phi,
+    residual evaluated with J_l typed out from Eq. 4.7 and the flux-surface average written as an explicit
+    jacobian-weighted sum.  tau_fac <-> 1/tau_fac, or tau_fac applied to the wrong term, fails."""
+    cfg, geo, G, _ = tiny
+    tf = 2.5
+    Phi = O.field_solve(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, tau_fac=tf)
+    kx, ky = cfg.dkx * O.kx_index(cfg.Nx), cfg.dky * O.ky_index(cfg.Ny)
+    z = geo["z"][:, None, None]
+    b = ((kx[None, :, None] - cfg.shat * z * ky[None, None, :]) ** 2 + ky[None, None, :] ** 2) / geo["bmag"][:, None, None] ** 2
+    Jl = [(-b / 2) ** l / math.factorial(l) * np.exp(-b / 2) for l in range(cfg.Nl)]
+    Gd = G.astype(np.complex128)
+    lhs = sum(Jl[l] * (Gd[0, 0, l] + Jl[l] * Phi) for l in range(cfg.Nl))
+    jac = geo["jacobian"]
+    fs = np.zeros_like(Phi)
+    fs[:, :, 0] = (np.sum(jac[:, None] * Phi[:, :, 0], axis=0) / np.sum(jac))[None, :]
+    res = lhs - (tf * (Phi - fs) + Phi)
+    res[:, 0, 0] = 0
+    assert np.max(np.abs(res)) < 1e-12 * np.max(np.abs(Phi))
+    wrong = lhs - ((Phi - fs) / tf + Phi)
+    wrong[:, 0, 0] = 0
+    assert np.max(np.abs(wrong)) > 1e-2 * np.max(np.abs(Phi))
 
 
 def test_field_solve_two_species_quasineutrality():
