@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgx.so")
 SOURCES = ["gx_api.cu"]
-HEADERS = ["dft_regs.cuh", "dft_pairs.cuh", "nl_kernels.cuh", "nl_pair_kernels.cuh", "nl_row_kernels.cuh", "linear_kernels.cuh"]
+HEADERS = ["dft_regs.cuh", "dft_pairs.cuh", "dft_packed.cuh", "nl_rx_kernels.cuh", "nl_kernels.cuh", "nl_pair_kernels.cuh", "nl_row_kernels.cuh", "linear_kernels.cuh"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "--extended-lambda", "-Xcompiler", "-fPIC", "-shared"]
 

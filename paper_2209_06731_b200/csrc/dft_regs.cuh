@@ -8,18 +8,24 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <cmath>
+
+#ifndef GX_HD
+#define GX_HD __host__ __device__ __forceinline__     // tests/host_emul runs the same functions on the CPU
+#endif
+
 namespace gx {
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ float2 cmul(float2 a, float2 b) {
+GX_HD float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+GX_HD float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+GX_HD float2 cmul(float2 a, float2 b) {
     return make_float2(fmaf(-a.y, b.y, a.x * b.x), fmaf(a.y, b.x, a.x * b.y));
 }
-__device__ __forceinline__ float2 cmul_conj(float2 a, float2 b) {   // a * conj(b)
+GX_HD float2 cmul_conj(float2 a, float2 b) {   // a * conj(b)
     return make_float2(fmaf(a.y, b.y, a.x * b.x), fmaf(a.y, b.x, -a.x * b.y));
 }
 // multiply by S*i
-template <int S> __device__ __forceinline__ float2 mul_i(float2 a) {
+template <int S> GX_HD float2 mul_i(float2 a) {
     return S > 0 ? make_float2(-a.y, a.x) : make_float2(a.y, -a.x);
 }
 
@@ -50,7 +56,7 @@ __host__ __device__ constexpr double cos48(int t) { return cos192(4 * t); }
 __host__ __device__ constexpr double sin48(int t) { return sin192(4 * t); }
 
 // v *= e^{S 2 pi i t / N} with t, N compile-time after unrolling; trivial cases cost no multiply.
-template <int N, int S> __device__ __forceinline__ float2 twiddle(float2 v, int t) {
+template <int N, int S> GX_HD float2 twiddle(float2 v, int t) {
     static_assert(192 % N == 0, "N must divide 192");
     const int a = ((t * (192 / N)) % 192 + 192) % 192;
     if (a == 0) return v;
@@ -76,10 +82,10 @@ template <int N, int S> __device__ __forceinline__ float2 twiddle(float2 v, int 
 typedef unsigned long long zm_t;
 template <int N, int S, zm_t ZM = 0ull> struct Dft;
 
-__device__ __forceinline__ float2 cneg(float2 a) { return make_float2(-a.x, -a.y); }
+GX_HD float2 cneg(float2 a) { return make_float2(-a.x, -a.y); }
 
 template <int S, zm_t ZM> struct Dft<2, S, ZM> {
-    __device__ __forceinline__ static void run(float2 (&v)[2]) {
+    GX_HD static void run(float2 (&v)[2]) {
         constexpr bool z0 = ZM & 1u, z1 = ZM & 2u;
         const float2 a = v[0], b = v[1];
         if constexpr (z1) { v[1] = a; }                       // (a, a); also covers both zero
@@ -89,7 +95,7 @@ template <int S, zm_t ZM> struct Dft<2, S, ZM> {
 };
 
 template <int S, zm_t ZM> struct Dft<3, S, ZM> {
-    __device__ __forceinline__ static void run(float2 (&v)[3]) {
+    GX_HD static void run(float2 (&v)[3]) {
         const float2 t = cadd(v[1], v[2]);
         const float2 d = csub(v[1], v[2]);
         const float2 m = make_float2(fmaf(-0.5f, t.x, v[0].x), fmaf(-0.5f, t.y, v[0].y));
@@ -102,7 +108,7 @@ template <int S, zm_t ZM> struct Dft<3, S, ZM> {
 };
 
 template <int S, zm_t ZM> struct Dft<4, S, ZM> {
-    __device__ __forceinline__ static void run(float2 (&v)[4]) {
+    GX_HD static void run(float2 (&v)[4]) {
         constexpr bool z0 = ZM & 1u, z1 = ZM & 2u, z2 = ZM & 4u, z3 = ZM & 8u;
         float2 a, b, c, d;                                    // a = v0+v2, b = v0-v2, c = v1+v3, d = v1-v3
         if constexpr (z2) { a = v[0]; b = v[0]; }
@@ -137,7 +143,7 @@ template <int A, int B, zm_t ZM> __host__ __device__ constexpr zm_t sub_mask_sec
 }
 
 template <int N, int A, int B, int S, zm_t ZM, int n2>
-__device__ __forceinline__ void dft_split_col(const float2 (&v)[N], float2 (&y)[N]) {
+GX_HD void dft_split_col(const float2 (&v)[N], float2 (&y)[N]) {
     float2 t[A];
 #pragma unroll
     for (int n1 = 0; n1 < A; ++n1) t[n1] = v[n1 * B + n2];
@@ -147,7 +153,7 @@ __device__ __forceinline__ void dft_split_col(const float2 (&v)[N], float2 (&y)[
     if constexpr (n2 + 1 < B) dft_split_col<N, A, B, S, ZM, n2 + 1>(v, y);
 }
 
-template <int N, int A, int B, int S, zm_t ZM = 0ull> __device__ __forceinline__ void dft_split(float2 (&v)[N]) {
+template <int N, int A, int B, int S, zm_t ZM = 0ull> GX_HD void dft_split(float2 (&v)[N]) {
     static_assert(A * B == N, "bad split");
     float2 y[N];
     dft_split_col<N, A, B, S, ZM, 0>(v, y);
@@ -163,25 +169,25 @@ template <int N, int A, int B, int S, zm_t ZM = 0ull> __device__ __forceinline__
 }
 
 template <int S, zm_t ZM> struct Dft<6, S, ZM> {
-    __device__ __forceinline__ static void run(float2 (&v)[6]) { dft_split<6, 2, 3, S, ZM>(v); }
+    GX_HD static void run(float2 (&v)[6]) { dft_split<6, 2, 3, S, ZM>(v); }
 };
 template <int S, zm_t ZM> struct Dft<8, S, ZM> {
-    __device__ __forceinline__ static void run(float2 (&v)[8]) { dft_split<8, 2, 4, S, ZM>(v); }
+    GX_HD static void run(float2 (&v)[8]) { dft_split<8, 2, 4, S, ZM>(v); }
 };
 template <int S, zm_t ZM> struct Dft<12, S, ZM> {
-    __device__ __forceinline__ static void run(float2 (&v)[12]) { dft_split<12, 3, 4, S, ZM>(v); }
+    GX_HD static void run(float2 (&v)[12]) { dft_split<12, 3, 4, S, ZM>(v); }
 };
 template <int S, zm_t ZM> struct Dft<16, S, ZM> {
-    __device__ __forceinline__ static void run(float2 (&v)[16]) { dft_split<16, 4, 4, S, ZM>(v); }
+    GX_HD static void run(float2 (&v)[16]) { dft_split<16, 4, 4, S, ZM>(v); }
 };
 
 template <int S, zm_t ZM> struct Dft<32, S, ZM> {
-    __device__ __forceinline__ static void run(float2 (&v)[32]) { dft_split<32, 4, 8, S, ZM>(v); }
+    GX_HD static void run(float2 (&v)[32]) { dft_split<32, 4, 8, S, ZM>(v); }
 };
 template <int S, zm_t ZM> struct Dft<64, S, ZM> {
-    __device__ __forceinline__ static void run(float2 (&v)[64]) { dft_split<64, 8, 8, S, ZM>(v); }
+    GX_HD static void run(float2 (&v)[64]) { dft_split<64, 8, 8, S, ZM>(v); }
 };
 
-template <int N, int S, zm_t ZM = 0ull> __device__ __forceinline__ void dft(float2 (&v)[N]) { Dft<N, S, ZM>::run(v); }
+template <int N, int S, zm_t ZM = 0ull> GX_HD void dft(float2 (&v)[N]) { Dft<N, S, ZM>::run(v); }
 
 }  // namespace gx

@@ -15,6 +15,7 @@
 #include "nl_kernels.cuh"
 #include "nl_pair_kernels.cuh"
 #include "nl_row_kernels.cuh"
+#include "nl_rx_kernels.cuh"
 
 namespace {
 
@@ -33,6 +34,9 @@ struct KernelSet {
     int family;          // GX_FAMILY_* of include/gx.h
     cudaError_t (*launch_chi)(const NlParams&, int units, cudaStream_t);
     cudaError_t (*launch_bracket)(const NlParams&, int units, cudaStream_t);
+    bool fused_laguerre = false;   // the bracket kernel writes `out` itself (a8 fused): no third launch
+    // one persistent kernel for the whole call (chi planes + bracket units + a8); launch_chi/bracket unused then
+    cudaError_t (*launch_call)(const NlParams&, unsigned* chi_flag, unsigned epoch, int n_items, cudaStream_t) = nullptr;
 };
 
 template <class C> cudaError_t launch_chi_t(const NlParams& p, int units, cudaStream_t st) {
@@ -253,6 +257,64 @@ using RP64x64   = gx::RowPairCfg<64, 64, 8, 8, 64, 2>;
 const KernelSet kRowPairSets[] = {
     make_rowp_set<RP64x64, RP64x64>(), make_rowp_set<RP128x64, RP128x64>(), make_rowp_set<RP192x64, RPC192x64>(),
 };
+// rx family (nl_rx_kernels.cuh): packed-FP32 x passes, row y direction, fused inverse Laguerre; NY = 64
+template <class C> cudaError_t launch_chi_rx_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_rx_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    gx::chi_planes_rx_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
+    return cudaGetLastError();
+}
+template <class C> cudaError_t launch_bracket_rx_t(const NlParams& p, int units, cudaStream_t st) {
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::bracket_rx_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    return launch_pdl(gx::bracket_rx_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
+}
+template <class CB, class CC> constexpr KernelSet make_rx_set() {
+    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1, "same permuted x order");
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_RX, &launch_chi_rx_t<CC>, &launch_bracket_rx_t<CB>, true};
+}
+template <class C> cudaError_t launch_rxp_t(const NlParams& p, unsigned* chi_flag, unsigned epoch, int n_items, cudaStream_t st) {
+    constexpr int SMEM = 2 * C::STAGE_BYTES + C::NX * 8 + 2 * 16 * 23 * 4;
+    static_assert(SMEM <= 232448, "two plane buffers do not fit in shared memory");
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::nl_rx_persist_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    const int grid = std::min(sm_count(), (n_items + 1) / 2);
+    gx::nl_rx_persist_kernel<C><<<grid, 2 * C::NT, SMEM, st>>>(p, chi_flag, epoch);
+    return cudaGetLastError();
+}
+template <class C> constexpr KernelSet make_rxp_set() {
+    return KernelSet{C::NX, C::NY, 2 * C::STAGE_BYTES, 0, GX_FAMILY_RXP, nullptr, nullptr, true, &launch_rxp_t<C>};
+}
+#ifndef GX_RX_R1
+#define GX_RX_R1 12
+#endif
+using X64x64   = gx::RxCfg<64, 64, 8, 8, 64, 6>;
+using X128x64  = gx::RxCfg<128, 64, 8, 16, 128, 3>;
+using X192x64  = gx::RxCfg<192, 64, GX_RX_R1, 192 / GX_RX_R1, 192, 2>;
+using X256x64  = gx::RxCfg<256, 64, 16, 16, 256, 1>;
+const KernelSet kRxSets[] = {
+    make_rx_set<X64x64, X64x64>(), make_rx_set<X128x64, X128x64>(), make_rx_set<X192x64, X192x64>(),
+    make_rx_set<X256x64, X256x64>(),
+};
+
+const KernelSet kRxpSets[] = {
+    make_rxp_set<X64x64>(), make_rxp_set<X128x64>(), make_rxp_set<X192x64>(),
+};
+
 using R256x64  = gx::RowCfg<256, 64, 16, 16, 256, 1>;
 const KernelSet kRowSets[] = {
     make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, RC192x64>(),
@@ -282,6 +344,12 @@ const KernelSet* find_set(int Nx, int Ny, int Nl) {
     const char* fam = std::getenv("GX_KERNELS");
     if (fam && std::strcmp(fam, "rowp") == 0)
         for (const auto& k : kRowPairSets)
+            if (k.Nx == Nx && k.Ny == Ny) return &k;
+    if (fam && std::strcmp(fam, "rxp") == 0)
+        for (const auto& k : kRxpSets)
+            if (k.Nx == Nx && k.Ny == Ny) return &k;
+    if (fam && std::strcmp(fam, "rx") == 0)
+        for (const auto& k : kRxSets)
             if (k.Nx == Nx && k.Ny == Ny) return &k;
     if (!fam || std::strcmp(fam, "row") == 0)
         for (const auto& k : kRowSets)
@@ -368,6 +436,7 @@ struct gx_grid {
     float *dT = nullptr, *dTinv = nullptr, *dM = nullptr;
     float2 *dtwx = nullptr, *dtwy = nullptr, *ddchi = nullptr, *dbhat = nullptr;
     unsigned* dcount = nullptr;
+    unsigned* dchi_flag = nullptr;              // [s][z][j] epoch of the last call that produced the chi plane (persistent family)
     unsigned calls = 0;                         // number of gx_nonlinear_rhs calls issued (counter epoch)
     float2 *dgbuf = nullptr, *dphibuf = nullptr, *doutbuf = nullptr;   // for the *_host entry point
     gx::LinTables lin;                                                  // linear-term tables
@@ -503,13 +572,15 @@ int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out
     if ((rc = dev_alloc(g, &g->dbhat, szj * Nm * g->nk))) return rc;
     if ((rc = dev_alloc(g, &g->dcount, (size_t)Ns * Nm * Nz))) return rc;
     GX_CUDA(g, cudaMemset(g->dcount, 0, (size_t)Ns * Nm * Nz * sizeof(unsigned)));
+    if ((rc = dev_alloc(g, &g->dchi_flag, szj))) return rc;
+    GX_CUDA(g, cudaMemset(g->dchi_flag, 0, szj * sizeof(unsigned)));
     return GX_OK;
 }
 
 int gx_grid_destroy(gx_grid* g) {
     if (!g) return GX_ERR_ARG;
     cudaFree(g->dT); cudaFree(g->dTinv); cudaFree(g->dM); cudaFree(g->dtwx); cudaFree(g->dtwy);
-    cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dcount); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
+    cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dcount); cudaFree(g->dchi_flag); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
     cudaFree(g->dphi_rhs); cudaFree(g->drk_y); cudaFree(g->drk_k);
     for (auto e : g->ev_pool) cudaEventDestroy(e);
     gx::lin_tables_free(g->lin);
@@ -662,11 +733,18 @@ int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* o
         g->ev_used += 4;
         GX_CUDA(g, cudaEventRecord(ev[0], st));
     }
+    if (g->ks->launch_call) {
+        g->calls += 1;
+        if (ev) GX_CUDA(g, cudaEventRecord(ev[1], st));
+        GX_CUDA(g, g->ks->launch_call(p, g->dchi_flag, g->calls, szj + szj * g->Nm, st));
+        if (ev) { GX_CUDA(g, cudaEventRecord(ev[2], st)); GX_CUDA(g, cudaEventRecord(ev[3], st)); }
+        return GX_OK;
+    }
     GX_CUDA(g, g->ks->launch_chi(p, szj, st));
     if (ev) GX_CUDA(g, cudaEventRecord(ev[1], st));
     GX_CUDA(g, g->ks->launch_bracket(p, szj * g->Nm, st));
     if (ev) GX_CUDA(g, cudaEventRecord(ev[2], st));
-    {
+    if (!g->ks->fused_laguerre) {
         const int vec = (g->nk % 2 == 0) ? 2 : 1;
         const int nkv = (int)(g->nk / vec);
         dim3 grid((unsigned)((nkv + 255) / 256), (unsigned)(g->Ns * g->Nm * g->Nz));
@@ -794,8 +872,8 @@ int gx_query(gx_grid* g, int what, long long* value) {
         case GX_Q_G_ELEMS: *value = (long long)g->Ns * g->Nm * g->Nl * g->Nz * g->nk; break;
         case GX_Q_PHI_ELEMS: *value = (long long)g->Nz * g->nk; break;
         case GX_Q_WORKSPACE_BYTES: *value = (long long)g->bytes; break;
-        case GX_Q_LAUNCHES_PER_NL: *value = 3; break;
-        case GX_Q_LAUNCHES_PER_RHS: *value = 3 + gx::kLinLaunchesFieldSolve + gx::kLinLaunchesRhs; break;
+        case GX_Q_LAUNCHES_PER_NL: *value = (g->ks && g->ks->launch_call) ? 1 : (g->ks && g->ks->fused_laguerre) ? 2 : 3; break;
+        case GX_Q_LAUNCHES_PER_RHS: *value = ((g->ks && g->ks->launch_call) ? 1 : (g->ks && g->ks->fused_laguerre) ? 2 : 3) + gx::kLinLaunchesFieldSolve + gx::kLinLaunchesRhs; break;
         case GX_Q_NL_FLOPS: *value = nl_flops(g); break;
         case GX_Q_KERNEL_FAMILY: *value = g->ks ? g->ks->family : -1; break;
         case GX_Q_NL_BYTES:
@@ -841,6 +919,9 @@ int gx_export_tables(gx_grid* g, float* T, float* Tinv, float* M) {
 }
 
 #ifdef GX_PHASE_TIMING
+int gx_debug_phase2_clocks(long long* out) {
+    return cudaMemcpyFromSymbol(out, gx::gx_phase2_clk, sizeof(long long) * 512 * 8 * 12) == cudaSuccess ? 0 : -1;
+}
 int gx_debug_phase_clocks(long long* out) {
     return cudaMemcpyFromSymbol(out, gx::gx_phase_clk, sizeof(long long) * 64 * 32) == cudaSuccess ? 0 : -1;
 }
