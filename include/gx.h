@@ -57,7 +57,7 @@ enum {
 };
 
 /* Kernel families of the nonlinear path; GX_KERNELS=scalar|pair|persist|row|rowp forces one. */
-enum { GX_FAMILY_SCALAR = 0, GX_FAMILY_PAIR = 1, GX_FAMILY_PERSIST = 2, GX_FAMILY_ROW = 3, GX_FAMILY_ROWP = 4, GX_FAMILY_RX = 5, GX_FAMILY_RXP = 6 };
+enum { GX_FAMILY_SCALAR = 0, GX_FAMILY_PAIR = 1, GX_FAMILY_PERSIST = 2, GX_FAMILY_ROW = 3, GX_FAMILY_ROWP = 4, GX_FAMILY_RX = 5, GX_FAMILY_RXP = 6, GX_FAMILY_RXW = 7 };
 
 /* Create a handle for real-space grid Nx x Ny, Nz field-line points, Nl Laguerre and Nm Hermite
  * moments, Ns species.  Nx, Ny must be even, >= 4, and factor as R1*R2 with R1,R2 in

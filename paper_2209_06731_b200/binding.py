@@ -18,7 +18,7 @@ LIB_PATH = os.environ.get("GX_LIBRARY_PATH") or os.path.join(_HERE, "libgx.so")
 GX_OK, GX_ERR_ARG, GX_ERR_STATE, GX_ERR_UNSUPPORTED, GX_ERR_CUDA, GX_ERR_ALLOC = 0, -1, -2, -3, -4, -5
 (GX_Q_NAKX, GX_Q_NAKY, GX_Q_NJ, GX_Q_G_ELEMS, GX_Q_PHI_ELEMS, GX_Q_WORKSPACE_BYTES,
  GX_Q_LAUNCHES_PER_NL, GX_Q_LAUNCHES_PER_RHS, GX_Q_NL_FLOPS, GX_Q_NL_BYTES, GX_Q_KERNEL_FAMILY) = range(11)
-FAMILY_NAMES = {0: "scalar", 1: "pair", 2: "persist", 3: "row", 4: "rowp", 5: "rx", 6: "rxp"}
+FAMILY_NAMES = {0: "scalar", 1: "pair", 2: "persist", 3: "row", 4: "rowp", 5: "rx", 6: "rxp", 7: "rxw"}
 
 EXPORTED = ["gx_grid_create", "gx_grid_destroy", "gx_box_set", "gx_species_set", "gx_adiabatic_set",
             "gx_dissipation_set", "gx_boundary_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_host",

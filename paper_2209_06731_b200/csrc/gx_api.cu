@@ -296,6 +296,21 @@ template <class C> cudaError_t launch_rxp_t(const NlParams& p, unsigned* chi_fla
     gx::nl_rx_persist_kernel<C><<<grid, 2 * C::NT, SMEM, st>>>(p, chi_flag, epoch);
     return cudaGetLastError();
 }
+template <class C> cudaError_t launch_rxw_t(const NlParams& p, unsigned* chi_flag, unsigned epoch, int n_items, cudaStream_t st) {
+    using L = gx::RxwLayout<C>;
+    static bool attr = false;
+    if (!attr) {
+        cudaError_t e = cudaFuncSetAttribute(gx::nl_rx_pipeline_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::SMEM);
+        if (e != cudaSuccess) return e;
+        attr = true;
+    }
+    const int grid = std::min(sm_count(), n_items);
+    gx::nl_rx_pipeline_kernel<C><<<grid, L::NTHREADS, L::SMEM, st>>>(p, chi_flag, epoch);
+    return cudaGetLastError();
+}
+template <class C> constexpr KernelSet make_rxw_set() {
+    return KernelSet{C::NX, C::NY, gx::RxwLayout<C>::SMEM, 0, GX_FAMILY_RXW, nullptr, nullptr, true, &launch_rxw_t<C>};
+}
 template <class C> constexpr KernelSet make_rxp_set() {
     return KernelSet{C::NX, C::NY, 2 * C::STAGE_BYTES, 0, GX_FAMILY_RXP, nullptr, nullptr, true, &launch_rxp_t<C>};
 }
@@ -311,6 +326,9 @@ const KernelSet kRxSets[] = {
     make_rx_set<X256x64, X256x64>(),
 };
 
+const KernelSet kRxwSets[] = {
+    make_rxw_set<X64x64>(), make_rxw_set<X128x64>(), make_rxw_set<X192x64>(),
+};
 const KernelSet kRxpSets[] = {
     make_rxp_set<X64x64>(), make_rxp_set<X128x64>(), make_rxp_set<X192x64>(),
 };
@@ -344,6 +362,9 @@ const KernelSet* find_set(int Nx, int Ny, int Nl) {
     const char* fam = std::getenv("GX_KERNELS");
     if (fam && std::strcmp(fam, "rowp") == 0)
         for (const auto& k : kRowPairSets)
+            if (k.Nx == Nx && k.Ny == Ny) return &k;
+    if (fam && std::strcmp(fam, "rxw") == 0)
+        for (const auto& k : kRxwSets)
             if (k.Nx == Nx && k.Ny == Ny) return &k;
     if (fam && std::strcmp(fam, "rxp") == 0)
         for (const auto& k : kRxpSets)

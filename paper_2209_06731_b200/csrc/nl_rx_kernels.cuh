@@ -40,7 +40,11 @@ struct RxCfg {
     static constexpr int K = (NX - 1) / 3, Q = (NY - 1) / 3;
     static constexpr int NAKX = 2 * K + 1, NAKY = Q + 1, NK = NAKX * NAKY, NK2 = NK / 2;
     static constexpr int NP = NAKY / 2;              // ky column pairs of the forward x passes
-    static constexpr int RS = NAKY | 1;              // row stride of W4 in float4: odd => conflict-free rows
+    // W4 row stride in float4 = NAKY (even) with the slots of a row XOR-swizzled by bit 2 of the row: rows r..r+7
+    // then hit eight different 16-byte bank groups for a fixed ky (row phase), and a row stays a permutation of
+    // consecutive slots (x passes) -- conflict-free without the padding column (3 KB per plane buffer)
+    static constexpr int RS = NAKY;
+    GX_HD static int widx(int row, int q) { return row * RS + (q ^ ((row >> 2) & 1)); }
     static constexpr int H = NY / 2;                 // complex length behind the real y transforms
     static constexpr int W4_ELEMS = NX * RS;         // float4
     static constexpr int S_ELEMS = NK;               // float2; S sits at the start of the dynamic shared memory
@@ -73,12 +77,13 @@ GX_HD float4 f4_from(pk::c2 v) {
 // ------------------------------------------------------------------------------------------------
 // a2: S[slot] (+)= sum_l coef[l] raw_l[slot] over the planes of one staging chunk, in place: plane 0 of the
 // first chunk lands on S itself, so a thread only ever overwrites slots it has just read.
-template <class C, class P4>
+template <class C, int NT = C::NT, class P4>
 GX_HD void rx_combine(int tid, P4 stage4, const float* coef, int l0, int nl, bool first) {
     // stage4: float4 view of the staging region; plane at slot index sl occupies [sl*NK2, (sl+1)*NK2)
+    constexpr int PER = (C::NK2 + NT - 1) / NT;
 #pragma unroll
-    for (int u = 0; u < C::PER; ++u) {
-        const int slot = u * C::NT + tid;
+    for (int u = 0; u < PER; ++u) {
+        const int slot = u * NT + tid;
         if (slot < C::NK2) {
             float4 acc = first ? make_float4(0.f, 0.f, 0.f, 0.f) : ld(stage4, slot);
             for (int l = 0; l < nl; ++l) {
@@ -132,9 +137,35 @@ GX_HD void rx_xi1_store(P4 W4, PT twx, int n2, int q, const pk::c2 (&v)[C::RX1])
             const float2 w = ld(twx, n2 * k1);
             o = pk::cmul_s(o, w.x, w.y);
         }
-        st(W4, (k1 * C::RX2 + n2) * C::RS + q, f4_from(o));
+        st(W4, C::widx(k1 * C::RX2 + n2, q), f4_from(o));
     }
 }
+// single-item form (fewer registers; the x workers of the pipelined kernel run it with their own thread count)
+template <class C, int NT, class P2, class P4, class PT>
+GX_HD void rx_x_inverse_pass1_single(int tid, P2 S, P4 W4, PT twx, float dkx, float dky) {
+    constexpr int NAKY = C::NAKY, R1 = C::RX1, R2 = C::RX2, NITEM = R2 * NAKY;
+    for (int t = tid; t < NITEM; t += NT) {
+        const int n2 = t / NAKY, q = t - n2 * NAKY;
+        pk::c2 v[R1];
+        rx_xi1_load<C>(S, n2, q, dkx, dky * (float)q, v);
+        pk::dft<R1, +1, C::ZMX>(v);
+        rx_xi1_store<C>(W4, twx, n2, q, v);
+    }
+}
+template <class C, int NT, class P4>
+GX_HD void rx_x_inverse_pass2_single(int tid, P4 W4) {
+    constexpr int NAKY = C::NAKY, R1 = C::RX1, R2 = C::RX2, NITEM = R1 * NAKY;
+    for (int t = tid; t < NITEM; t += NT) {
+        const int k1 = t / NAKY, q = t - k1 * NAKY;
+        pk::c2 v[R2];
+#pragma unroll
+        for (int n2 = 0; n2 < R2; ++n2) v[n2] = c2_from(ld(W4, C::widx(k1 * R2 + n2, q)));
+        pk::dft<R2, +1>(v);
+#pragma unroll
+        for (int k2 = 0; k2 < R2; ++k2) st(W4, C::widx(k1 * R2 + k2, q), f4_from(v[k2]));
+    }
+}
+
 template <class C, class P2, class P4, class PT>
 GX_HD void rx_x_inverse_pass1(int tid, P2 S, P4 W4, PT twx, float dkx, float dky) {
     constexpr int NAKY = C::NAKY, R1 = C::RX1, R2 = C::RX2, NT = C::NT, NITEM = R2 * NAKY;
@@ -165,7 +196,7 @@ GX_HD void rx_x_inverse_pass1(int tid, P2 S, P4 W4, PT twx, float dkx, float dky
 // Item (k1, q): DFT_R2 over n2; position k1*R2 + k2 <- x = k1 + R1*k2.  Two items per thread as above.
 template <class C, class P4>
 GX_HD void rx_x_inverse_pass2(int tid, P4 W4) {
-    constexpr int NAKY = C::NAKY, RS = C::RS, R1 = C::RX1, R2 = C::RX2, NT = C::NT, NITEM = R1 * NAKY;
+    constexpr int NAKY = C::NAKY, R1 = C::RX1, R2 = C::RX2, NT = C::NT, NITEM = R1 * NAKY;
     for (int t0 = tid; t0 < NITEM; t0 += 2 * NT) {
         const int t1 = t0 + NT;
         const bool has1 = t1 < NITEM;
@@ -175,24 +206,24 @@ GX_HD void rx_x_inverse_pass2(int tid, P4 W4) {
             pk::c2 va[R2], vb[R2];
 #pragma unroll
             for (int n2 = 0; n2 < R2; ++n2) {
-                va[n2] = c2_from(ld(W4, (k1a * R2 + n2) * RS + qa));
-                vb[n2] = c2_from(ld(W4, (k1b * R2 + n2) * RS + qb));
+                va[n2] = c2_from(ld(W4, C::widx(k1a * R2 + n2, qa)));
+                vb[n2] = c2_from(ld(W4, C::widx(k1b * R2 + n2, qb)));
             }
             pk::dft<R2, +1>(va);
             pk::dft<R2, +1>(vb);
 #pragma unroll
-            for (int k2 = 0; k2 < R2; ++k2) st(W4, (k1a * R2 + k2) * RS + qa, f4_from(va[k2]));
+            for (int k2 = 0; k2 < R2; ++k2) st(W4, C::widx(k1a * R2 + k2, qa), f4_from(va[k2]));
             if (has1) {
 #pragma unroll
-                for (int k2 = 0; k2 < R2; ++k2) st(W4, (k1b * R2 + k2) * RS + qb, f4_from(vb[k2]));
+                for (int k2 = 0; k2 < R2; ++k2) st(W4, C::widx(k1b * R2 + k2, qb), f4_from(vb[k2]));
             }
         } else {
             pk::c2 va[R2];
 #pragma unroll
-            for (int n2 = 0; n2 < R2; ++n2) va[n2] = c2_from(ld(W4, (k1a * R2 + n2) * RS + qa));
+            for (int n2 = 0; n2 < R2; ++n2) va[n2] = c2_from(ld(W4, C::widx(k1a * R2 + n2, qa)));
             pk::dft<R2, +1>(va);
 #pragma unroll
-            for (int k2 = 0; k2 < R2; ++k2) st(W4, (k1a * R2 + k2) * RS + qa, f4_from(va[k2]));
+            for (int k2 = 0; k2 < R2; ++k2) st(W4, C::widx(k1a * R2 + k2, qa), f4_from(va[k2]));
         }
     }
 }
@@ -200,14 +231,14 @@ GX_HD void rx_x_inverse_pass2(int tid, P4 W4) {
 // ------------------------------------------------------------------------------------------------
 // a6 (x part): forward x transform of the column pairs (lane 0 = ky 2p, lane 1 = ky 2p+1).
 // Item (a, p): DFT_R2 over b of W4[(a*R2 + b)][p], twiddle e^{-2 pi i a d / NX}, back in place.
-template <class C, class P4, class PT>
+template <class C, int NT = C::NT, class P4, class PT>
 GX_HD void rx_x_forward_pass1(int tid, P4 W4, PT twx) {
-    constexpr int NP = C::NP, RS = C::RS, R1 = C::RX1, R2 = C::RX2;
-    for (int t = tid; t < R1 * NP; t += C::NT) {
+    constexpr int NP = C::NP, R1 = C::RX1, R2 = C::RX2;
+    for (int t = tid; t < R1 * NP; t += NT) {
         const int a = t / NP, pp = t - a * NP;
         pk::c2 v[R2];
 #pragma unroll
-        for (int b = 0; b < R2; ++b) v[b] = c2_from(ld(W4, (a * R2 + b) * RS + pp));
+        for (int b = 0; b < R2; ++b) v[b] = c2_from(ld(W4, C::widx(a * R2 + b, pp)));
         pk::dft<R2, -1>(v);
 #pragma unroll
         for (int d = 0; d < R2; ++d) {
@@ -216,21 +247,21 @@ GX_HD void rx_x_forward_pass1(int tid, P4 W4, PT twx) {
                 const float2 w = ld(twx, a * d);
                 o = pk::cmul_s(o, w.x, -w.y);
             }
-            st(W4, (a * R2 + d) * RS + pp, f4_from(o));
+            st(W4, C::widx(a * R2 + d, pp), f4_from(o));
         }
     }
 }
 
 // Item (d, p): DFT_R1 over a; kept rows n = d + R2*cc (|kx| <= K: a7) times `scale` to the compact plane
 // out4 (float4 = two neighbouring ky of one kx row; NAKY even).
-template <class C, class P4, class PO>
+template <class C, int NT = C::NT, class P4, class PO>
 GX_HD void rx_x_forward_pass2(int tid, P4 W4, PO out4, float scale) {
-    constexpr int NX = C::NX, K = C::K, NAKX = C::NAKX, NP = C::NP, RS = C::RS, R1 = C::RX1, R2 = C::RX2;
-    for (int t = tid; t < R2 * NP; t += C::NT) {
+    constexpr int NX = C::NX, K = C::K, NAKX = C::NAKX, NP = C::NP, R1 = C::RX1, R2 = C::RX2;
+    for (int t = tid; t < R2 * NP; t += NT) {
         const int d = t / NP, pp = t - d * NP;
         pk::c2 v[R1];
 #pragma unroll
-        for (int a = 0; a < R1; ++a) v[a] = c2_from(ld(W4, (a * R2 + d) * RS + pp));
+        for (int a = 0; a < R1; ++a) v[a] = c2_from(ld(W4, C::widx(a * R2 + d, pp)));
         pk::dft<R1, -1>(v);
 #pragma unroll
         for (int cc = 0; cc < R1; ++cc) {
@@ -294,14 +325,14 @@ template <class T> GX_HD const void* addr_of(const T* p, int i) { return p + i; 
 template <class C, class P4>
 GX_HD void rx_row_load(P4 W4, int row, pk::c2 (&Cq)[C::NAKY]) {
 #pragma unroll
-    for (int q = 0; q < C::NAKY; ++q) Cq[q] = c2_from(ld(W4, row * C::RS + q));
+    for (int q = 0; q < C::NAKY; ++q) Cq[q] = c2_from(ld(W4, C::widx(row, q)));
 }
 
 // a4 (y part) + a5 + a6 (y part) + a7 (ky <= Q) for the rows of this thread.  dchi4[i*NX + row] holds
 // (d_x chi, d_y chi) at y = 2i and y = 2i+1 of the row.
 template <class C, class P4, class PD>
 GX_HD void rx_row_bracket(int tid, P4 W4, PD dchi4) {
-    constexpr int NX = C::NX, NY = C::NY, H = C::H, Q = C::Q, NP = C::NP, RS = C::RS;
+    constexpr int NX = C::NX, NY = C::NY, H = C::H, Q = C::Q, NP = C::NP;
     constexpr int A = 8, B = 4;                    // H = A*B: second stage in groups of B outputs i = k1 + A*k2
     static_assert(A * B == H, "split of the half-length transform");
     for (int row = tid; row < NX; row += C::NT) {
@@ -363,7 +394,7 @@ GX_HD void rx_row_bracket(int tid, P4 W4, PD dchi4) {
         }
 #pragma unroll
         for (int pp = 0; pp < NP; ++pp)
-            st(W4, row * RS + pp, make_float4(F[2 * pp].x, F[2 * pp + 1].x, F[2 * pp].y, F[2 * pp + 1].y));
+            st(W4, C::widx(row, pp), make_float4(F[2 * pp].x, F[2 * pp + 1].x, F[2 * pp].y, F[2 * pp + 1].y));
     }
 }
 
@@ -764,6 +795,231 @@ __global__ void __launch_bounds__(2 * C::NT, 1) nl_rx_persist_kernel(const NlPar
     }
     publish_pending();
     laguerre_items(true);
+}
+
+// ================================================================================================
+// Warp-specialised software pipeline (family "rxw"): ONE persistent CTA per SM, 512 threads,
+//     row workers  = warp groups 0-1 (192 of 256 threads used, 168 registers each after setmaxnreg.inc):
+//                    y direction + bracket of item k (a4 y part, a5, a6 y part), chi rows, a8 items;
+//     x workers    = warp groups 2-3 (256 threads, 88 registers after setmaxnreg.dec):
+//                    staging + Laguerre combine + inverse x passes of item k+1, forward x passes of item k-1.
+// Why (profiles/r02_rx_pipeline.md): with all warps walking the phases in lock step the FP32 pipe idles during
+// the TMA wait, the latency-bound x passes and every barrier (48 % busy, 12.9 k cycles per unit and SM); the
+// register file (168 registers for a 64-point row in one thread) allows no third lock-step group.  Shrinking
+// the registers of the warps that never run the row phase pays for 8 more warps, and the two kinds of work
+// overlap by construction: the row workers never wait for memory, the x workers hide their latencies behind
+// the row phase.  Two plane buffers W4[2] alternate between the stages; hand-over is by named barriers
+// (bar.arrive / bar.sync), the raw Laguerre planes of item k+1 are requested one stage ahead.
+//
+// Work list per CTA c: items c, c + grid, ... of [chi planes | bracket units]; chi items come first and never wait.
+template <int N> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
+__device__ __forceinline__ void nbar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void nbar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
+template <class C>
+struct RxwLayout {
+    static constexpr int NROW = C::NX;            // row workers in use (one per x row)
+    static constexpr int NXW = 256;               // x workers
+    static constexpr int NTHREADS = 512;
+    static constexpr int W4_BYTES = C::W4_ELEMS * 16;
+    static constexpr int CAPW_MAX = (232448 - 2 * W4_BYTES - C::NX * 8 - 2 * 16 * 23 * 4 - 64) / (C::NK * 8);
+    static constexpr int CAPW = CAPW_MAX > 8 ? 8 : CAPW_MAX;   // raw-plane slots of the staging area (slot 0 is S)
+    static constexpr int STAGE_BYTES = CAPW * C::NK * 8;
+    static constexpr int SMEM = 2 * W4_BYTES + STAGE_BYTES + C::NX * 8 + 2 * 16 * 23 * 4;
+    static_assert(NROW <= 256 && NROW % 32 == 0, "row workers live in warp groups 0-1");
+    static_assert(CAPW >= 2, "two plane buffers and the staging area do not fit in shared memory");
+};
+// named barriers: 1, 2 = W4[b] holds the inverse x transform (x workers arrive, row workers wait);
+// 3, 4 = W4[b] holds the forward data after the first forward x pass (row workers arrive, x workers wait);
+// 5 = x workers among themselves; 6 = row workers among themselves
+enum { RXW_BAR_INV = 1, RXW_BAR_FWD = 3, RXW_BAR_X = 5, RXW_BAR_ROW = 6 };
+
+__device__ __forceinline__ void mbar_expect_tx_noarrive(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.expect_tx.relaxed.cta.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+
+#ifdef GX_PHASE_TIMING
+#define GX_PHASE3(i) do { if ((threadIdx.x == 256 || threadIdx.x == 0) && cid < 256 && k < 16) gx_phase2_clk[(cid * 16 + k) * 12 + (i)] = gx_globaltimer(); } while (0)
+#else
+#define GX_PHASE3(i) do { } while (0)
+#endif
+template <class C>
+__global__ void __launch_bounds__(512, 1) nl_rx_pipeline_kernel(const NlParams p, unsigned* chi_flag, unsigned epoch) {
+    using L = RxwLayout<C>;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int NK = C::NK, NROW = L::NROW, NXW = L::NXW, NBOTH = NROW + NXW;
+    float4* W4b[2] = {reinterpret_cast<float4*>(smem_raw), reinterpret_cast<float4*>(smem_raw + L::W4_BYTES)};
+    unsigned char* stage = smem_raw + 2 * L::W4_BYTES;
+    float2* S = reinterpret_cast<float2*>(stage);
+    float4* stage4 = reinterpret_cast<float4*>(stage);
+    float2* twx = reinterpret_cast<float2*>(stage + L::STAGE_BYTES);
+    float* Tall = reinterpret_cast<float*>(twx + C::NX);        // T[j][l]
+    float* Ti = Tall + 16 * 23;                                 // -Tinv[l][j]
+    __shared__ unsigned long long stage_bar;
+    __shared__ int row_flag;
+
+    if (threadIdx.x == 0) mbar_init(&stage_bar, 1);
+    for (int i = threadIdx.x; i < C::NX; i += L::NTHREADS) twx[i] = __ldg(p.twx + i);
+    for (int i = threadIdx.x; i < p.Nl * p.J; i += L::NTHREADS) {
+        Tall[i] = __ldg(p.T + i);
+        Ti[i] = -__ldg(p.Tinv + i);                             // out = -N
+    }
+    __syncthreads();
+
+    const int n_chi = p.Ns * p.Nz * p.J, n_items = n_chi + n_chi * p.Nm;
+    const int G = gridDim.x, cid = blockIdx.x;
+    const size_t lstride = (size_t)p.Nz * NK;
+
+    if (threadIdx.x >= 256) {
+        // ======================================================================== x workers
+        reg_dealloc<88>();
+        const int tid = threadIdx.x - 256;
+        unsigned bar_parity = 0;
+        const int nl0 = min(L::CAPW, p.Nl);                              // planes of the first staging chunk
+        auto plane_src = [&](int unit, int l) {
+            const RxUnit u = rx_decode(unit, p);
+            return p.g + ((size_t)(u.s * p.Nm + u.m) * p.Nl * p.Nz + u.z) * NK + (size_t)l * lstride;
+        };
+        // first chunk in two steps: planes 1.. land in slots 1.. (free once the combine is done), plane 0 lands on S
+        // (free once the first inverse x pass has read it); the arrive of step B completes the mbarrier phase
+        auto request_upper = [&](int unit) {                            // one thread
+            if (nl0 > 1) {
+                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                mbar_expect_tx_noarrive(&stage_bar, (unsigned)((nl0 - 1) * NK * sizeof(float2)));
+                for (int l = 1; l < nl0; ++l) bulk_g2s(S + (size_t)l * NK, plane_src(unit, l), NK * sizeof(float2), &stage_bar);
+            }
+        };
+        auto request_plane0 = [&](int unit) {                           // one thread
+            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+            mbar_expect_tx(&stage_bar, (unsigned)(NK * sizeof(float2)));
+            bulk_g2s(S, plane_src(unit, 0), NK * sizeof(float2), &stage_bar);
+        };
+        bool staged = false;
+        int k = 0;
+        for (int item = cid; item < n_items + G; item += G, ++k) {
+            const int b = k & 1;
+            const int next = item + G;
+            const bool next_bracket = next < n_items && next >= n_chi;
+            GX_PHASE3(0);
+            if (item < n_items) {
+                // ---- produce item k into W4[b]: compact plane S, then the inverse x passes
+                if (item < n_chi) {
+                    const int z = (item / p.J) % p.Nz;
+                    const float2* __restrict__ phi = p.phi + (size_t)z * NK;
+                    const float* __restrict__ M = p.M + (size_t)item * NK;
+                    for (int i = tid; i < NK; i += NXW) {
+                        const float2 f = __ldg(phi + i);
+                        const float mm = __ldg(M + i);
+                        S[i] = make_float2(f.x * mm, f.y * mm);
+                    }
+                    nbar_sync(RXW_BAR_X, NXW);
+                } else {
+                    const int unit = item - n_chi;
+                    const RxUnit u = rx_decode(unit, p);
+                    if (!staged && tid == 0) { request_upper(unit); request_plane0(unit); }
+                    staged = false;
+                    for (int l0 = 0; l0 < p.Nl;) {
+                        const bool first = l0 == 0;
+                        const int nl = first ? nl0 : min(L::CAPW - 1, p.Nl - l0);
+                        if (!first && tid == 0) {
+                            asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+                            mbar_expect_tx(&stage_bar, (unsigned)(nl * NK * sizeof(float2)));
+                            for (int l = 0; l < nl; ++l) bulk_g2s(S + (size_t)(l + 1) * NK, plane_src(unit, l0 + l), NK * sizeof(float2), &stage_bar);
+                        }
+                        mbar_wait(&stage_bar, bar_parity);
+                        bar_parity ^= 1u;
+                        GX_PHASE3(5);
+                        rx_combine<C, NXW>(tid, stage4, Tall + u.j * p.Nl, l0, nl, first);
+                        nbar_sync(RXW_BAR_X, NXW);                   // chunk consumed / S complete
+                        l0 += nl;
+                    }
+                }
+                if (next_bracket && tid == 0) request_upper(next - n_chi);      // slots 1.. are dead from here on
+                GX_PHASE3(1);
+                rx_x_inverse_pass1_single<C, NXW>(tid, (const float2*)S, W4b[b], (const float2*)twx, p.dkx, p.dky);
+                nbar_sync(RXW_BAR_X, NXW);
+                if (next_bracket) {                                              // S is dead from here on
+                    if (tid == 0) request_plane0(next - n_chi);
+                    staged = true;
+                }
+                rx_x_inverse_pass2_single<C, NXW>(tid, W4b[b]);
+                __threadfence_block();
+                nbar_arrive(RXW_BAR_INV + b, NBOTH);                 // W4[b] ready for the row workers
+            }
+            GX_PHASE3(2);
+            // ---- retire item k-1 from W4[b^1]: second forward x pass of a bracket unit, then publish its node plane
+            if (k >= 1) {
+                const int prev = item - G;
+                nbar_sync(RXW_BAR_FWD + (b ^ 1), NBOTH);             // rows + first forward x pass of item k-1 done
+                GX_PHASE3(3);
+                if (prev >= n_chi) {
+                    const int unit = prev - n_chi;
+                    rx_x_forward_pass2<C, NXW>(tid, (const float4*)W4b[b ^ 1], reinterpret_cast<float4*>(p.bhat + (size_t)unit * NK), p.scale);
+                    nbar_sync(RXW_BAR_X, NXW);                       // node-plane stores precede the fence below (cumulative)
+                    if (tid == NXW - 1) {
+                        const RxUnit u = rx_decode(unit, p);
+                        __threadfence();                             // release: stores -> barrier -> fence -> atomic
+                        atomicAdd(p.count + (u.s * p.Nm + u.m) * p.Nz + u.z, 1u);
+                    }
+                }
+                GX_PHASE3(4);
+            }
+        }
+    } else {
+        // ======================================================================== row workers
+        reg_alloc<168>();
+        const int tid = threadIdx.x;
+        if (tid >= NROW) return;                                     // spare warps of warp group 1
+        // a8 items: (s,m,z) number i belongs to CTA G-1 - (i mod G); polled after every item, blocking at the end
+        const int n_smz = p.Ns * p.Nm * p.Nz;
+        int lag_item = G - 1 - cid;
+        auto laguerre_items = [&](bool block) {
+            while (lag_item < n_smz) {
+                if (tid == 0) {
+                    unsigned c = ld_acquire_u32(p.count + lag_item);
+                    while (block && c != (unsigned)p.J) { __nanosleep(200); c = ld_acquire_u32(p.count + lag_item); }
+                    row_flag = (c == (unsigned)p.J);
+                }
+                nbar_sync(RXW_BAR_ROW, NROW);
+                const int ready = row_flag;
+                nbar_sync(RXW_BAR_ROW, NROW);
+                if (!ready) break;
+                const int z = lag_item % p.Nz, m = (lag_item / p.Nz) % p.Nm, sp = lag_item / (p.Nz * p.Nm);
+                const float4* bh4 = reinterpret_cast<const float4*>(p.bhat + ((size_t)((sp * p.Nz + z) * p.J) * p.Nm + m) * NK);
+                float4* out4 = reinterpret_cast<float4*>(p.out + (((size_t)(sp * p.Nm + m) * p.Nl) * p.Nz + z) * NK);
+                rx_laguerre_inverse<C>(tid, CgPtr{bh4}, p.Nm * C::NK2, out4, (int)(lstride / 2), Ti, p.Nl, p.J);
+                if (tid == 0) p.count[lag_item] = 0u;               // nobody touches this counter again before the next call
+                lag_item += G;
+            }
+        };
+        int k = 0;
+        for (int item = cid; item < n_items; item += G, ++k) {
+            const int b = k & 1;
+            GX_PHASE3(6);
+            nbar_sync(RXW_BAR_INV + b, NBOTH);                       // inverse x transform of item k is in W4[b]
+            GX_PHASE3(7);
+            if (item < n_chi) {
+                rx_row_chi<C>(tid, (const float4*)W4b[b], reinterpret_cast<float4*>(p.dchi) + (size_t)item * C::H * C::NX);
+                nbar_sync(RXW_BAR_ROW, NROW);                        // every thread's stores precede thread 0's release
+                if (tid == 0) { __threadfence(); st_release_u32(chi_flag + item, epoch); }
+            } else {
+                const RxUnit u = rx_decode(item - n_chi, p);
+                if (tid == 0) while (ld_acquire_u32(chi_flag + u.szj) != epoch) __nanosleep(100);
+                nbar_sync(RXW_BAR_ROW, NROW);
+                GX_PHASE3(8);
+                rx_row_bracket<C>(tid, W4b[b], reinterpret_cast<const float4*>(p.dchi) + (size_t)u.szj * C::H * C::NX);
+                nbar_sync(RXW_BAR_ROW, NROW);
+                rx_x_forward_pass1<C>(tid, W4b[b], (const float2*)twx);      // a6 (x part), first pass: fits the row workers' slack
+            }
+            __threadfence_block();
+            nbar_arrive(RXW_BAR_FWD + b, NBOTH);                     // W4[b] handed back to the x workers
+            GX_PHASE3(9);
+            laguerre_items(false);
+            GX_PHASE3(10);
+        }
+        laguerre_items(true);
+    }
 }
 #endif  // __CUDACC__
 
