@@ -146,18 +146,21 @@ def run_reference(args):
         return 0
     cfg = I.named_config(args.config)
     geo = I.geometry_arrays(cfg)
-    steps = max(1, min(args.steps, 3))
-    for _ in range(min(args.warmup, 1)):
-        oracle_sample(cfg, geo, budget_s=2.0)
+    # every step is a bounded sample of the workload; the per-step budget shrinks with --steps so that the whole
+    # run (warm-up included) stays within about two minutes
+    steps, warm = max(1, args.steps), max(0, args.warmup)
+    budget = max(0.25, min(10.0, 90.0 / (steps + warm)))
+    for _ in range(warm):
+        oracle_sample(cfg, geo, budget_s=budget)
     vals, secs, sample = [], 0.0, ""
     for _ in range(steps):
-        v, sample, dt = oracle_sample(cfg, geo, budget_s=10.0)
+        v, sample, dt = oracle_sample(cfg, geo, budget_s=budget)
         vals.append(v)
         secs += dt
     value = float(np.mean(vals))
     cores = host_threads()
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-            "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": 1e3 / value, "higher_is_better": True,
+            "steps": steps, "warmup": warm, "ms_per_step": 1e3 / value, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": workload_name(cfg), "note": "fp64 CPU oracle on host cores; bounded sample per step"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
@@ -215,6 +218,26 @@ def cufft_composition(torch, cfg, grid, g, phi, ours, steps=20):
     return steps / (e0.elapsed_time(e1) * 1e-3), err
 
 
+# ------------------------------------------------------------------------------- measured FP32 peak
+def fp32_ubench(B, sm_mhz, n_sm, full=False):
+    """FP32 pipe micro-benchmark of the library (gx_ubench_fp32): lane operations per clock and SM for the scalar
+    and packed add / mul / fma, at 2 x 512 threads per SM (and more shapes with --ubench)."""
+    out = {}
+    shapes = [(512, 2)] + ([(256, 2), (192, 2), (1024, 1), (384, 1)] if full else [])
+    for kind, name in enumerate(B.UBENCH_KINDS):
+        for nt, bps in shapes:
+            best = 0.0
+            try:
+                for _ in range(3):
+                    ms, ops = B.gx_ubench_fp32(kind, nt, bps, 4096)
+                    best = max(best, ops / (ms * 1e-3))
+            except B.GxError:
+                continue                                  # launch shape not possible for this kernel (registers)
+            key = name if (nt, bps) == (512, 2) else f"{name} @{bps}x{nt}"
+            out[key] = {"lane_ops_per_s": best, "lane_ops_per_clk_per_sm": best / (sm_mhz * 1e6) / n_sm}
+    return out
+
+
 # ------------------------------------------------------------------------------- GPU leg
 def run_gpu(args):
     import torch
@@ -227,29 +250,38 @@ def run_gpu(args):
     dev = torch.device("cuda", local_rank)
     cfg = I.named_config(args.config)
     geo = I.geometry_arrays(cfg)
-    m0, m1, Nm_global = D.hermite_block(cfg.Nm, rank, world)      # weak scaling: one Hermite block per rank
+    # weak scaling: ONE seeded state with Nm*world Hermite moments, rank r owns the block [m0, m1) (the paper's
+    # own decomposition); phi is replicated: every rank solves quasineutrality from the m = 0 slab
+    m0, m1, Nm_global = D.hermite_block(cfg.Nm, rank, world)
+    cfg_global = I.Config(**{**cfg.__dict__, "Nm": Nm_global})
     grid = B.Grid(cfg, geo)
     flops = grid.query(B.GX_Q_NL_FLOPS)
     alg_bytes = grid.query(B.GX_Q_NL_BYTES)
     launches_per_call = grid.query(B.GX_Q_LAUNCHES_PER_NL)
 
-    # seeded state of this rank's Hermite block; phi from the library's own field solve (product path)
-    cfg_rank = I.Config(**{**cfg.__dict__, "seed": cfg.seed + 1000 * rank})
+    # this rank's Hermite block of the global seeded state; phi from the library's own field solve (product path)
+    # on the global m = 0 slab (a one-moment handle: the field solve reads m = 0 only)
     g_elems = int(np.prod(cfg.g_shape))
     set_bytes = 2 * g_elems * 8 + int(np.prod(cfg.phi_shape)) * 8
     nsets = max(2, int(np.ceil(4.2 * L2_BYTES / set_bytes)))
     nsets = min(nsets, max(2, int(40e9 // set_bytes)))
-    G0 = I.make_state(cfg_rank, geo)
+    G0 = I.make_state(cfg_global, geo, hermite_block=(m0, m1))
     g_host = torch.from_numpy(G0)
+    cfg_m0 = I.Config(**{**cfg.__dict__, "Nm": 1})
+    grid_m0 = B.Grid(cfg_m0, geo)
+    g_m0 = torch.from_numpy(I.make_state(cfg_global, geo, hermite_block=(0, 1))).to(dev)
     gs, phis, outs = [], [], []
     for k in range(nsets):
         g = g_host.to(dev)
+        scale_k = 1.0 + 0.01 * k            # distinct contents per set, same spectrum
         if k:
-            g.mul_(1.0 + 0.01 * k)          # distinct contents per set, same spectrum
+            g.mul_(scale_k)
         phi = torch.empty(cfg.phi_shape, dtype=torch.complex64, device=dev)
-        grid.field_solve(g, phi)
+        grid_m0.field_solve(g_m0, phi)
+        phi.mul_(scale_k)                   # the field solve is linear in g
         gs.append(g); phis.append(phi); outs.append(torch.empty_like(g))
     torch.cuda.synchronize()
+    grid_m0.close()
 
     def step(i):
         k = i % nsets
@@ -361,8 +393,19 @@ def run_gpu(args):
             traffic = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get(cfg.name, {}).get("bracket_kernel")
         except Exception:
             pass
+        ub = fp32_ubench(B, sm_max, n_sm, full=args.ubench)
+        peak_measured = 2.0 * ub["fma.rn.f32"]["lane_ops_per_s"] / 1e12          # FMA = 2 flops per lane operation
+        traffic_call = None
+        try:
+            traffic_call = json.load(open(os.path.join(ROOT, "profiles", "ncu_traffic.json"))).get(cfg.name, {}).get("call")
+        except Exception:
+            pass
         roofline = {"bound": "alu", "kernel": "bracket kernel of the %s family" % B.FAMILY_NAMES.get(grid.query(B.GX_Q_KERNEL_FAMILY), "?"), "achieved": achieved, "peak": peak_tflops,
                     "unit": "TFLOP/s", "frac": achieved / peak_tflops, "traffic": traffic,
+                    "peak_measured": peak_measured, "frac_of_measured": achieved / peak_measured,
+                    "peak_measured_source": "gx_ubench_fp32: fma.rn.f32, 16 chains per thread, 2 x 512 threads per SM, this run",
+                    "fp32_pipe_lane_ops_per_clk_per_sm": {k: round(v["lane_ops_per_clk_per_sm"], 2) for k, v in ub.items()},
+                    "traffic_per_call": traffic_call,
                     "peak_source": f"{n_sm} SMs x 128 FP32 lanes x 2 x {sm_max:.0f} MHz (max SM clock, MEASURED_PEAKS.json)",
                     "kernel_us": {"chi_planes": kern_us[0], "bracket": kern_us[1], "laguerre_inverse": kern_us[2]},
                     "kernel_share_of_step": kern_us[1] / max(sum(kern_us), 1e-9),
@@ -376,7 +419,7 @@ def run_gpu(args):
                 "warmup": args.warmup, "ms_per_step": 1e3 * sec_max / args.steps, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
                 "config": {"workload": workload_name(cfg), "hermite_moments_global": Nm_global,
-                           "parallelism": f"hermite-block x{world}, no collective",
+                           "parallelism": f"hermite-block x{world} of one seeded state, phi replicated, no collective",
                            "l2": f"inputs rotate through {nsets} buffer sets ({nsets * set_bytes / 1e6:.0f} MB > 126 MB L2)",
                            "grid_point_moments_per_s": value * cfg.grid_point_moments,
                            "phi": "gx_field_solve on device (Boltzmann electrons)" if cfg.Ns == 1 else "gx_field_solve on device"},
@@ -407,10 +450,25 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="omit the oracle timing (ncu passes)")
     ap.add_argument("--skip-reference-point", action="store_true", help="omit the cuFFT+cuBLAS composition")
+    ap.add_argument("--ubench", action="store_true", help="FP32 pipe micro-benchmark at more launch shapes (roofline.fp32_pipe_...)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
-    return run_reference(args) if args.impl == "reference" else run_gpu(args)
+    if args.impl == "reference":
+        return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # no launcher: start one process per GPU ourselves (same command the driver uses)
+        import subprocess
+        import torch
+        have = torch.cuda.device_count()
+        if have < args.gpus:
+            raise SystemExit(f"bench.py: --gpus {args.gpus} but only {have} CUDA device(s) are visible")
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+               "--master-addr", "127.0.0.1", "--master-port", str(29500 + os.getpid() % 2000), os.path.abspath(__file__)] + sys.argv[1:]
+        return subprocess.call(cmd)
+    if int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} does not match WORLD_SIZE={os.environ.get('WORLD_SIZE', '1')}")
+    return run_gpu(args)
 
 
 if __name__ == "__main__":

@@ -22,7 +22,11 @@
  * OWNERSHIP: g, phi, out are caller-owned DEVICE pointers (16-byte aligned; out must not alias g);
  *   the library keeps no reference after the call returns.  The handle owns all tables and the
  *   workspace.  Geometry / species arrays are HOST pointers, copied during the call.
+ *   Misaligned device pointers and partially overlapping g / out ranges are rejected with GX_ERR_ARG.
  * ASYNC: compute calls enqueue on the given cudaStream_t (passed as void*) and do not synchronise.
+ * CONCURRENCY: a handle owns ONE workspace (chi planes, node planes, arrival counters, phi of gx_rhs, RK buffers):
+ *   it is single-thread and single-stream -- all compute calls on a handle must be ordered on one stream (or
+ *   ordered by the caller with events).  Use one handle per stream for concurrent evaluations.
  * ERRORS: every call returns 0 (GX_OK) or a negative code; no exception crosses the ABI;
  *   gx_last_error() returns a message for the last failure on that handle.
  * There is NO CPU fallback: without a CUDA device gx_grid_create fails with GX_ERR_CUDA.
@@ -57,7 +61,7 @@ enum {
 };
 
 /* Kernel families of the nonlinear path; GX_KERNELS=scalar|pair|persist|row|rowp forces one. */
-enum { GX_FAMILY_SCALAR = 0, GX_FAMILY_PAIR = 1, GX_FAMILY_PERSIST = 2, GX_FAMILY_ROW = 3, GX_FAMILY_ROWP = 4, GX_FAMILY_RX = 5, GX_FAMILY_RXP = 6, GX_FAMILY_RXW = 7 };
+enum { GX_FAMILY_SCALAR = 0, GX_FAMILY_ROW = 3, GX_FAMILY_RX = 5, GX_FAMILY_RXP = 6, GX_FAMILY_RXW = 7 };   /* 1, 2, 4: families removed in round 2 */
 
 /* Create a handle for real-space grid Nx x Ny, Nz field-line points, Nl Laguerre and Nm Hermite
  * moments, Ns species.  Nx, Ny must be even, >= 4, and factor as R1*R2 with R1,R2 in
@@ -150,6 +154,14 @@ int gx_profile_set(gx_grid* g, int enabled);
 int gx_profile_get(gx_grid* g, double* ms, long long* calls);
 
 const char* gx_last_error(gx_grid* g);
+
+/* FP32 pipe micro-benchmark on the current device (no handle): `iters` rounds of 16 independent dependency
+ * chains per thread of one instruction kind -- 0 add.f32, 1 mul.f32, 2 fma.rn.f32, 3 add.f32x2, 4 mul.f32x2,
+ * 5 fma.rn.f32x2 -- on (SM count * blocks_per_sm) blocks of threads_per_block threads.  Writes the kernel time
+ * (CUDA events, one warm-up launch before) to *ms and the number of lane operations executed to *lane_ops (a
+ * packed instruction counts two, an FMA counts one: flops = 2 * lane_ops for kinds 2 and 5).  bench.py derives
+ * roofline.peak_measured from it ("the bench should also run a tiny FMA-peak kernel"). */
+int gx_ubench_fp32(int kind, int threads_per_block, int blocks_per_sm, int iters, double* ms, double* lane_ops);
 
 #ifdef __cplusplus
 }

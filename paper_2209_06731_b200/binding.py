@@ -18,12 +18,12 @@ LIB_PATH = os.environ.get("GX_LIBRARY_PATH") or os.path.join(_HERE, "libgx.so")
 GX_OK, GX_ERR_ARG, GX_ERR_STATE, GX_ERR_UNSUPPORTED, GX_ERR_CUDA, GX_ERR_ALLOC = 0, -1, -2, -3, -4, -5
 (GX_Q_NAKX, GX_Q_NAKY, GX_Q_NJ, GX_Q_G_ELEMS, GX_Q_PHI_ELEMS, GX_Q_WORKSPACE_BYTES,
  GX_Q_LAUNCHES_PER_NL, GX_Q_LAUNCHES_PER_RHS, GX_Q_NL_FLOPS, GX_Q_NL_BYTES, GX_Q_KERNEL_FAMILY) = range(11)
-FAMILY_NAMES = {0: "scalar", 1: "pair", 2: "persist", 3: "row", 4: "rowp", 5: "rx", 6: "rxp", 7: "rxw"}
+FAMILY_NAMES = {0: "scalar", 3: "row", 5: "rx", 6: "rxp", 7: "rxw"}
 
 EXPORTED = ["gx_grid_create", "gx_grid_destroy", "gx_box_set", "gx_species_set", "gx_adiabatic_set",
             "gx_dissipation_set", "gx_boundary_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_host",
             "gx_field_solve", "gx_rhs", "gx_linear_rhs", "gx_ssprk3_step", "gx_query", "gx_export_maps",
-            "gx_export_tables", "gx_profile_set", "gx_profile_get", "gx_last_error"]
+            "gx_export_tables", "gx_profile_set", "gx_profile_get", "gx_last_error", "gx_ubench_fp32"]
 
 _lib = None
 
@@ -65,6 +65,7 @@ def load():
     lib.gx_profile_get.argtypes = [vp, dp, C.POINTER(C.c_longlong)]
     lib.gx_last_error.argtypes = [vp]
     lib.gx_last_error.restype = C.c_char_p
+    lib.gx_ubench_fp32.argtypes = [i, i, i, i, dp, dp]
     for name in EXPORTED:
         if name != "gx_last_error":
             getattr(lib, name).restype = i
@@ -190,6 +191,16 @@ def gx_profile_get(h):
     return [ms[0], ms[1], ms[2]], n.value
 
 
+UBENCH_KINDS = ["add.f32", "mul.f32", "fma.rn.f32", "add.f32x2", "mul.f32x2", "fma.rn.f32x2"]
+
+
+def gx_ubench_fp32(kind, threads_per_block=512, blocks_per_sm=2, iters=4096):
+    """-> (milliseconds, lane operations) of the FP32 pipe micro-benchmark (include/gx.h)."""
+    ms, ops = C.c_double(), C.c_double()
+    _check(None, load().gx_ubench_fp32(kind, threads_per_block, blocks_per_sm, iters, C.byref(ms), C.byref(ops)))
+    return ms.value, ops.value
+
+
 # ---- convenience wrapper (marshalling only) -------------------------------------------------------
 class Grid:
     """Owns a gx_grid handle configured from an ``inputs.Config``; methods take torch CUDA tensors
@@ -225,28 +236,38 @@ class Grid:
         import torch
         return torch.cuda.current_stream().cuda_stream
 
+    def _chk(self, t, what, host=False):
+        """Marshalling checks: dtype, contiguity, device and element count (GX_Q_G_ELEMS / GX_Q_PHI_ELEMS)."""
+        import torch
+        n = gx_query(self.h, GX_Q_G_ELEMS if what == "g" else GX_Q_PHI_ELEMS)
+        if t.dtype != torch.complex64 or not t.is_contiguous() or t.numel() != n or (t.is_cuda == host):
+            raise ValueError(f"{what}: expected a contiguous complex64 {'host' if host else 'CUDA'} tensor of {n} elements, "
+                             f"got {t.dtype} {tuple(t.shape)} on {t.device}")
+        return t.data_ptr()
+
     def nonlinear_rhs(self, g, phi, out):
-        gx_nonlinear_rhs(self.h, g.data_ptr(), phi.data_ptr(), out.data_ptr(), self._stream())
+        gx_nonlinear_rhs(self.h, self._chk(g, "g"), self._chk(phi, "phi"), self._chk(out, "g"), self._stream())
         return out
 
     def nonlinear_rhs_host(self, g_host, phi_host, out_host):
-        gx_nonlinear_rhs_host(self.h, g_host.data_ptr(), phi_host.data_ptr(), out_host.data_ptr(), self._stream())
+        gx_nonlinear_rhs_host(self.h, self._chk(g_host, "g", True), self._chk(phi_host, "phi", True),
+                              self._chk(out_host, "g", True), self._stream())
         return out_host
 
     def field_solve(self, g, phi):
-        gx_field_solve(self.h, g.data_ptr(), phi.data_ptr(), self._stream())
+        gx_field_solve(self.h, self._chk(g, "g"), self._chk(phi, "phi"), self._stream())
         return phi
 
     def rhs(self, g, out):
-        gx_rhs(self.h, g.data_ptr(), out.data_ptr(), self._stream())
+        gx_rhs(self.h, self._chk(g, "g"), self._chk(out, "g"), self._stream())
         return out
 
     def linear_rhs(self, g, phi, out):
-        gx_linear_rhs(self.h, g.data_ptr(), phi.data_ptr(), out.data_ptr(), self._stream())
+        gx_linear_rhs(self.h, self._chk(g, "g"), self._chk(phi, "phi"), self._chk(out, "g"), self._stream())
         return out
 
     def ssprk3_step(self, g, dt):
-        gx_ssprk3_step(self.h, g.data_ptr(), dt, self._stream())
+        gx_ssprk3_step(self.h, self._chk(g, "g"), dt, self._stream())
         return g
 
     def export_maps(self):

@@ -6,16 +6,14 @@
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
+#include <cstdint>
 #include <cstring>
 #include <string>
 #include <vector>
 
 #include "../../include/gx.h"
 #include "linear_kernels.cuh"
-#include "nl_kernels.cuh"
-#include "nl_pair_kernels.cuh"
-#include "nl_row_kernels.cuh"
-#include "nl_rx_kernels.cuh"
+#include "kernel_sets.h"
 
 namespace {
 
@@ -26,364 +24,24 @@ struct Species {
     bool set = false;
 };
 
-// per-(Nx,Ny) kernel launchers
-struct KernelSet {
-    int Nx, Ny;
-    int smem_bytes;
-    int max_nl;          // 0: any Nl; else the set needs Nl <= max_nl (all Laguerre planes staged at once)
-    int family;          // GX_FAMILY_* of include/gx.h
-    cudaError_t (*launch_chi)(const NlParams&, int units, cudaStream_t);
-    cudaError_t (*launch_bracket)(const NlParams&, int units, cudaStream_t);
-    bool fused_laguerre = false;   // the bracket kernel writes `out` itself (a8 fused): no third launch
-    // one persistent kernel for the whole call (chi planes + bracket units + a8); launch_chi/bracket unused then
-    cudaError_t (*launch_call)(const NlParams&, unsigned* chi_flag, unsigned epoch, int n_items, cudaStream_t) = nullptr;
-};
+using gxhost::KernelSet;
+using gxhost::launch_pdl;
 
-template <class C> cudaError_t launch_chi_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    gx::chi_planes_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
-    return cudaGetLastError();
-}
-// Launch with the programmatic-stream-serialization attribute (PDL): the grid may begin before the
-// previous kernel in the stream has finished; the kernel itself waits (griddepcontrol.wait) before it
-// reads that kernel's output.
-template <class... Args, class... Act>
-cudaError_t launch_pdl(void (*kernel)(Args...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Act... args) {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
-    cudaLaunchAttribute at[1];
-    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    at[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = at; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, kernel, args...);
-}
-template <class C> cudaError_t launch_bracket_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::bracket_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    return launch_pdl(gx::bracket_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
-}
-template <class C> cudaError_t launch_chi_pair_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_pair_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    gx::chi_planes_pair_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
-    return cudaGetLastError();
-}
-template <class C> cudaError_t launch_bracket_pair_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::bracket_pair_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    return launch_pdl(gx::bracket_pair_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
-}
-int sm_count() {
-    static int n = 0;
-    if (!n) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) n = 148;
-    }
-    return n;
-}
-template <class C> cudaError_t launch_bracket_persist_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::bracket_persist_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    const int grid = units < sm_count() ? units : sm_count();
-    return launch_pdl(gx::bracket_persist_kernel<C>, dim3(grid), dim3(C::NT), C::SMEM_BYTES, st, p, units);
-}
-template <class CB, class CC> constexpr KernelSet make_persist_set() {
-    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
-                  "chi and bracket kernels must share the transform radices (same permuted real-space order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, CB::MAXL, GX_FAMILY_PERSIST, &launch_chi_pair_t<CC>, &launch_bracket_persist_t<CB>};
-}
-template <class C> cudaError_t launch_chi_row_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_row_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    gx::chi_planes_row_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
-    return cudaGetLastError();
-}
-template <class C> cudaError_t launch_bracket_row_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::bracket_row_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    return launch_pdl(gx::bracket_row_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
-}
-template <class CB, class CC> constexpr KernelSet make_row_set() {
-    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1,
-                  "chi and bracket kernels must share the x radices (same permuted x order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_ROW, &launch_chi_row_t<CC>, &launch_bracket_row_t<CB>};
-}
-template <class C> cudaError_t launch_chi_rowp_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_rowp_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    gx::chi_planes_rowp_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
-    return cudaGetLastError();
-}
-template <class C> cudaError_t launch_bracket_rowp_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::bracket_rowp_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    return launch_pdl(gx::bracket_rowp_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
-}
-template <class CB, class CC> constexpr KernelSet make_rowp_set() {
-    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1, "same permuted x order");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_ROWP, &launch_chi_rowp_t<CC>, &launch_bracket_rowp_t<CB>};
-}
-template <class CB, class CC> constexpr KernelSet make_pair_set() {
-    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
-                  "chi and bracket kernels must share the transform radices (same permuted real-space order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_PAIR, &launch_chi_pair_t<CC>, &launch_bracket_pair_t<CB>};
-}
-template <class CB, class CC> constexpr KernelSet make_set() {
-    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::RY1 == CC::RY1,
-                  "chi and bracket kernels must share the transform radices (same permuted real-space order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_SCALAR, &launch_chi_t<CC>, &launch_bracket_t<CB>};
-}
-
-#ifndef GX_BR_NT
-#define GX_BR_NT 448
-#endif
-#ifndef GX_BR_MINB
-#define GX_BR_MINB 2
-#endif
-#ifndef GX_CHI_NT
-#define GX_CHI_NT 512
-#endif
-#ifndef GX_BR_RB
-#define GX_BR_RB 64
-#endif
-//                  NX   NY  RX1 RX2 RY1 RY2  RB   NT MINB STAGE     (B = bracket kernel, C = chi kernel)
-using B16x16   = gx::PlaneCfg<16, 16, 4, 4, 4, 4, 16, 64, 1, true>;
-using B64x64   = gx::PlaneCfg<64, 64, 8, 8, 8, 8, 64, 256, 2, true>;
-using B128x64  = gx::PlaneCfg<128, 64, 16, 8, 8, 8, 64, GX_BR_NT, GX_BR_MINB, true>;
-using C128x64  = gx::PlaneCfg<128, 64, 16, 8, 8, 8, 64, GX_CHI_NT, 1, true>;
-using B192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, GX_BR_RB, GX_BR_NT, GX_BR_MINB, true>;
-using C192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, 64, GX_CHI_NT, 1, true>;
-using B256x64  = gx::PlaneCfg<256, 64, 16, 16, 8, 8, 64, 256, 1, true>;
-#ifndef GX_BIG_NT
-#define GX_BIG_NT 384
-#endif
-using B256x96  = gx::PlaneCfg<256, 96, 16, 16, 8, 12, 64, GX_BIG_NT, 1, true>;
-using B192x192 = gx::PlaneCfg<192, 192, 16, 12, 12, 16, 16, GX_BIG_NT, 1, false>;
-#ifndef GX_W7X_RB
-#define GX_W7X_RB 16
-#endif
-#ifndef GX_W7X_NT
-#define GX_W7X_NT 256
-#endif
-using B64x192  = gx::PlaneCfg<64, 192, 8, 8, 12, 16, GX_W7X_RB, GX_W7X_NT, (GX_W7X_RB <= 16 ? 2 : 1), true>;   // RB 16: 92 KB, two CTAs per SM
-
-const KernelSet kKernelSets[] = {
-    make_set<B16x16, B16x16>(),   make_set<B64x64, B64x64>(),     make_set<B128x64, C128x64>(),
-    make_set<B192x64, C192x64>(), make_set<B256x64, B256x64>(),   make_set<B256x96, B256x96>(),
-    make_set<B192x192, B192x192>(), make_set<B64x192, B64x192>(),
-};
-
-// packed-FP32 family (nl_pair_kernels.cuh): preferred when an instantiation exists
-#ifndef GX_PB_NT
-#define GX_PB_NT 256
-#endif
-#ifndef GX_PC_NT
-#define GX_PC_NT 256
-#endif
-//                   NX   NY  RX1 RX2 RY1 RY2  RB   NT MINB
-using P16x16   = gx::PairCfg<16, 16, 4, 4, 4, 4, 16, 64, 1>;
-using P64x64   = gx::PairCfg<64, 64, 8, 8, 8, 8, 64, 128, 2>;
-using P128x64  = gx::PairCfg<128, 64, 16, 8, 8, 8, 64, GX_PB_NT, 2>;
-using P192x64  = gx::PairCfg<192, 64, 16, 12, 8, 8, 64, GX_PB_NT, 2>;
-using PC192x64 = gx::PairCfg<192, 64, 16, 12, 8, 8, 64, GX_PC_NT, 1>;
-using P256x96  = gx::PairCfg<256, 96, 16, 16, 8, 12, 32, 256, 1>;
-using P64x192  = gx::PairCfg<64, 192, 8, 8, 12, 16, 32, 128, 1>;
-
-// row family (nl_row_kernels.cuh): whole y direction of an x row in one thread's registers; NY = 64 only
-#ifndef GX_ROW_NT
-#define GX_ROW_NT 192
-#endif
-#ifndef GX_ROW_MINB
-#define GX_ROW_MINB 2
-#endif
-using R64x64   = gx::RowCfg<64, 64, 8, 8, 64, 6>;
-using R128x64  = gx::RowCfg<128, 64, 16, 8, 128, 3>;
-using R192x64  = gx::RowCfg<192, 64, 16, 12, GX_ROW_NT, GX_ROW_MINB>;
-#ifndef GX_ROWCHI_NT
-#define GX_ROWCHI_NT 384
-#endif
-using RC192x64 = gx::RowCfg<192, 64, 16, 12, GX_ROWCHI_NT, 1>;   // chi planes: < 1 wave, more threads for the x passes
-using RP192x64  = gx::RowPairCfg<192, 64, 16, 12, GX_ROW_NT, GX_ROW_MINB>;
-using RPC192x64 = gx::RowPairCfg<192, 64, 16, 12, GX_ROWCHI_NT, 1>;
-using RP128x64  = gx::RowPairCfg<128, 64, 16, 8, 128, 2>;
-using RP64x64   = gx::RowPairCfg<64, 64, 8, 8, 64, 2>;
-const KernelSet kRowPairSets[] = {
-    make_rowp_set<RP64x64, RP64x64>(), make_rowp_set<RP128x64, RP128x64>(), make_rowp_set<RP192x64, RPC192x64>(),
-};
-// rx family (nl_rx_kernels.cuh): packed-FP32 x passes, row y direction, fused inverse Laguerre; NY = 64
-template <class C> cudaError_t launch_chi_rx_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::chi_planes_rx_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    gx::chi_planes_rx_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
-    return cudaGetLastError();
-}
-template <class C> cudaError_t launch_bracket_rx_t(const NlParams& p, int units, cudaStream_t st) {
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::bracket_rx_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             C::SMEM_BYTES);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    return launch_pdl(gx::bracket_rx_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
-}
-template <class CB, class CC> constexpr KernelSet make_rx_set() {
-    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1, "same permuted x order");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, 0, GX_FAMILY_RX, &launch_chi_rx_t<CC>, &launch_bracket_rx_t<CB>, true};
-}
-template <class C> cudaError_t launch_rxp_t(const NlParams& p, unsigned* chi_flag, unsigned epoch, int n_items, cudaStream_t st) {
-    constexpr int SMEM = 2 * C::STAGE_BYTES + C::NX * 8 + 2 * 16 * 23 * 4;
-    static_assert(SMEM <= 232448, "two plane buffers do not fit in shared memory");
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::nl_rx_persist_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    const int grid = std::min(sm_count(), (n_items + 1) / 2);
-    gx::nl_rx_persist_kernel<C><<<grid, 2 * C::NT, SMEM, st>>>(p, chi_flag, epoch);
-    return cudaGetLastError();
-}
-template <class C> cudaError_t launch_rxw_t(const NlParams& p, unsigned* chi_flag, unsigned epoch, int n_items, cudaStream_t st) {
-    using L = gx::RxwLayout<C>;
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(gx::nl_rx_pipeline_kernel<C>, cudaFuncAttributeMaxDynamicSharedMemorySize, L::SMEM);
-        if (e != cudaSuccess) return e;
-        attr = true;
-    }
-    const int grid = std::min(sm_count(), n_items);
-    gx::nl_rx_pipeline_kernel<C><<<grid, L::NTHREADS, L::SMEM, st>>>(p, chi_flag, epoch);
-    return cudaGetLastError();
-}
-template <class C> constexpr KernelSet make_rxw_set() {
-    return KernelSet{C::NX, C::NY, gx::RxwLayout<C>::SMEM, 0, GX_FAMILY_RXW, nullptr, nullptr, true, &launch_rxw_t<C>};
-}
-template <class C> constexpr KernelSet make_rxp_set() {
-    return KernelSet{C::NX, C::NY, 2 * C::STAGE_BYTES, 0, GX_FAMILY_RXP, nullptr, nullptr, true, &launch_rxp_t<C>};
-}
-#ifndef GX_RX_R1
-#define GX_RX_R1 12
-#endif
-using X64x64   = gx::RxCfg<64, 64, 8, 8, 64, 6>;
-using X128x64  = gx::RxCfg<128, 64, 8, 16, 128, 3>;
-using X192x64  = gx::RxCfg<192, 64, GX_RX_R1, 192 / GX_RX_R1, 192, 2>;
-using X256x64  = gx::RxCfg<256, 64, 16, 16, 256, 1>;
-const KernelSet kRxSets[] = {
-    make_rx_set<X64x64, X64x64>(), make_rx_set<X128x64, X128x64>(), make_rx_set<X192x64, X192x64>(),
-    make_rx_set<X256x64, X256x64>(),
-};
-
-const KernelSet kRxwSets[] = {
-    make_rxw_set<X64x64>(), make_rxw_set<X128x64>(), make_rxw_set<X192x64>(),
-};
-const KernelSet kRxpSets[] = {
-    make_rxp_set<X64x64>(), make_rxp_set<X128x64>(), make_rxp_set<X192x64>(),
-};
-
-using R256x64  = gx::RowCfg<256, 64, 16, 16, 256, 1>;
-const KernelSet kRowSets[] = {
-    make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, RC192x64>(),
-    make_row_set<R256x64, R256x64>(),
-};
-
-#ifndef GX_PS_NW
-#define GX_PS_NW 12
-#endif
-using S192x64  = gx::PersistCfg<192, 64, 16, 12, 8, 8, GX_PS_NW, 4>;
-const KernelSet kPersistSets[] = {
-    make_persist_set<S192x64, PC192x64>(),
-};
-
-const KernelSet kPairSets[] = {
-    make_pair_set<P16x16, P16x16>(),   make_pair_set<P64x64, P64x64>(),   make_pair_set<P128x64, P128x64>(),
-    make_pair_set<P192x64, PC192x64>(), make_pair_set<P256x96, P256x96>(), make_pair_set<P64x192, P64x192>(),
-};
-
-// Four kernel families share the C-ABI ("Kernel families"):
-//   row     (nl_row_kernels.cuh)   y direction of an x row in one thread's registers (NY = 64)  -- default where instantiated
-//   scalar  (nl_kernels.cuh)       block-synchronous two-pass transforms, scalar FP32            -- default otherwise
-//   pair    (nl_pair_kernels.cuh)  block-synchronous, packed FADD2/FFMA2                         -- GX_KERNELS=pair
-//   persist (nl_pair_kernels.cuh)  persistent, warp-asynchronous, packed                         -- GX_KERNELS=persist
+// Kernel families behind the one C-ABI ("Kernel families"; profiles/r02_rx_families.md):
+//   row     (nl_row_kernels.cuh)   y direction of an x row in one thread's registers (NY = 64)   -- default where instantiated
+//   scalar  (nl_kernels.cuh)       block-synchronous two-pass transforms, scalar FP32             -- default otherwise
+//   rx      (nl_rx_kernels.cuh)    packed-FP32 x passes, packed C2R rows, a8 fused                -- GX_KERNELS=rx
+//   rxp     (nl_rx_kernels.cuh)    rx phases in one persistent kernel, two groups per SM          -- GX_KERNELS=rxp
+//   rxw     (nl_rx_kernels.cuh)    warp-specialised pipeline (row warps + x warps)                -- GX_KERNELS=rxw
 // GX_KERNELS (read at gx_grid_create) forces a family; one without an instantiation for the grid falls through.
-const KernelSet* find_set(int Nx, int Ny, int Nl) {
+const KernelSet* find_set(int Nx, int Ny) {
     const char* fam = std::getenv("GX_KERNELS");
-    if (fam && std::strcmp(fam, "rowp") == 0)
-        for (const auto& k : kRowPairSets)
-            if (k.Nx == Nx && k.Ny == Ny) return &k;
-    if (fam && std::strcmp(fam, "rxw") == 0)
-        for (const auto& k : kRxwSets)
-            if (k.Nx == Nx && k.Ny == Ny) return &k;
-    if (fam && std::strcmp(fam, "rxp") == 0)
-        for (const auto& k : kRxpSets)
-            if (k.Nx == Nx && k.Ny == Ny) return &k;
-    if (fam && std::strcmp(fam, "rx") == 0)
-        for (const auto& k : kRxSets)
-            if (k.Nx == Nx && k.Ny == Ny) return &k;
-    if (!fam || std::strcmp(fam, "row") == 0)
-        for (const auto& k : kRowSets)
-            if (k.Nx == Nx && k.Ny == Ny) return &k;
-    if (fam && std::strcmp(fam, "persist") == 0)
-        for (const auto& k : kPersistSets)
-            if (k.Nx == Nx && k.Ny == Ny && Nl <= k.max_nl) return &k;
-    if (fam && (std::strcmp(fam, "pair") == 0 || std::strcmp(fam, "persist") == 0))
-        for (const auto& k : kPairSets)
-            if (k.Nx == Nx && k.Ny == Ny) return &k;
-    for (const auto& k : kKernelSets)
-        if (k.Nx == Nx && k.Ny == Ny) return &k;
-    return nullptr;
+    const KernelSet* k = nullptr;
+    if (fam && std::strcmp(fam, "rxw") == 0 && (k = gxhost::find_rx(Nx, Ny, GX_FAMILY_RXW))) return k;
+    if (fam && std::strcmp(fam, "rxp") == 0 && (k = gxhost::find_rx(Nx, Ny, GX_FAMILY_RXP))) return k;
+    if (fam && std::strcmp(fam, "rx") == 0 && (k = gxhost::find_rx(Nx, Ny, GX_FAMILY_RX))) return k;
+    if ((!fam || std::strcmp(fam, "row") == 0) && (k = gxhost::find_row(Nx, Ny))) return k;
+    return gxhost::find_scalar(Nx, Ny);
 }
 
 // ---------------------------------------------------------------------------- Gauss-Laguerre
@@ -463,7 +121,7 @@ struct gx_grid {
     gx::LinTables lin;                                                  // linear-term tables
     float2* dphi_rhs = nullptr;                                         // phi of gx_rhs
     float2 *drk_y = nullptr, *drk_k = nullptr;                          // SSP-RK3 stage and slope buffers
-    size_t bytes = 0;
+    size_t bytes = 0, lin_bytes = 0;
     bool profile = false;
     std::vector<cudaEvent_t> ev_pool;          // 4 events per profiled call
     size_t ev_used = 0;
@@ -471,6 +129,12 @@ struct gx_grid {
 };
 
 namespace {
+
+bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+bool overlap(const void* a, const void* b, size_t bytes) {
+    const uintptr_t x = reinterpret_cast<uintptr_t>(a), y = reinterpret_cast<uintptr_t>(b);
+    return x < y + bytes && y < x + bytes;
+}
 
 int fail(gx_grid* g, int code, const std::string& msg) {
     if (g) g->err = msg;
@@ -553,9 +217,10 @@ int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out
     g->J = (3 * Nl - 1) / 2;
     g->sp.resize(Ns);
     g->adiabatic = (Ns == 1);
-    g->ks = find_set(Nx, Ny, Nl);
+    g->ks = find_set(Nx, Ny);
     *out = g;                       // returned even on failure below so that gx_last_error works
     if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
+    GX_CUDA(g, g->ks->prepare());      // per device and per handle: no process-wide cache of function attributes
 
     gauss_laguerre(g->J, g->xj, g->wj);
     g->hT.resize((size_t)g->J * Nl);
@@ -724,7 +389,8 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
         size_t bytes = 0;
         if (!gx::lin_tables_build(in, g->lin, bytes, msg))
             return fail(g, msg.find("quantised") != std::string::npos ? GX_ERR_ARG : GX_ERR_CUDA, msg);
-        g->bytes += bytes;
+        g->bytes += bytes - g->lin_bytes;          // a rebuilt table replaces the old one
+        g->lin_bytes = bytes;
         if (!g->dphi_rhs) {
             int rc = dev_alloc(g, &g->dphi_rhs, (size_t)Nz * g->nk);
             if (rc) return rc;
@@ -737,7 +403,10 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
 int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream) {
     if (!g) return GX_ERR_ARG;
     if (!g_dev || !phi_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: null pointer");
-    if (g_dev == out_dev) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: out must not alias g");
+    const size_t gbytes = (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk * sizeof(float2);
+    if (overlap(g_dev, out_dev, gbytes)) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: out must not alias g");
+    if (misaligned(g_dev) || misaligned(phi_dev) || misaligned(out_dev))
+        return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: device pointers must be 16-byte aligned");
     if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
     if (!g->geo_set) return fail(g, GX_ERR_STATE, "gx_nonlinear_rhs: geometry not set");
     cudaStream_t st = (cudaStream_t)cuda_stream;
@@ -838,7 +507,10 @@ int gx_field_solve(gx_grid* g, const void* g_dev, void* phi_dev, void* cuda_stre
 int gx_linear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream) {
     if (!g) return GX_ERR_ARG;
     if (!g_dev || !phi_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_linear_rhs: null pointer");
-    if (g_dev == out_dev) return fail(g, GX_ERR_ARG, "gx_linear_rhs: out must not alias g");
+    if (overlap(g_dev, out_dev, (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk * sizeof(float2)))
+        return fail(g, GX_ERR_ARG, "gx_linear_rhs: out must not alias g");
+    if (misaligned(g_dev) || misaligned(phi_dev) || misaligned(out_dev))
+        return fail(g, GX_ERR_ARG, "gx_linear_rhs: device pointers must be 16-byte aligned");
     if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_linear_rhs: full geometry not set");
     cudaError_t e = gx::lin_rhs(g->lin, (const float2*)g_dev, (const float2*)phi_dev, (float2*)out_dev,
                                 /*accumulate=*/false, (cudaStream_t)cuda_stream);
@@ -849,7 +521,9 @@ int gx_linear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_
 int gx_rhs(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream) {
     if (!g) return GX_ERR_ARG;
     if (!g_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_rhs: null pointer");
-    if (g_dev == out_dev) return fail(g, GX_ERR_ARG, "gx_rhs: out must not alias g");
+    if (overlap(g_dev, out_dev, (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk * sizeof(float2)))
+        return fail(g, GX_ERR_ARG, "gx_rhs: out must not alias g");
+    if (misaligned(g_dev) || misaligned(out_dev)) return fail(g, GX_ERR_ARG, "gx_rhs: device pointers must be 16-byte aligned");
     if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_rhs: full geometry not set");
     int rc;
     if ((rc = gx_field_solve(g, g_dev, g->dphi_rhs, cuda_stream))) return rc;
@@ -938,15 +612,6 @@ int gx_export_tables(gx_grid* g, float* T, float* Tinv, float* M) {
     }
     return GX_OK;
 }
-
-#ifdef GX_PHASE_TIMING
-int gx_debug_phase2_clocks(long long* out) {
-    return cudaMemcpyFromSymbol(out, gx::gx_phase2_clk, sizeof(long long) * 512 * 8 * 12) == cudaSuccess ? 0 : -1;
-}
-int gx_debug_phase_clocks(long long* out) {
-    return cudaMemcpyFromSymbol(out, gx::gx_phase_clk, sizeof(long long) * 64 * 32) == cudaSuccess ? 0 : -1;
-}
-#endif
 
 const char* gx_last_error(gx_grid* g) { return g ? g->err.c_str() : "null handle"; }
 

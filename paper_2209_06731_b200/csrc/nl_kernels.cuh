@@ -35,7 +35,7 @@ namespace gx {
 // Optional phase timing (development builds only, -DGX_PHASE_TIMING): thread 0 of the first CTAs records
 // clock64() at phase boundaries; read back with gx_debug_phase_clocks().
 #ifdef GX_PHASE_TIMING
-__device__ long long gx_phase_clk[64 * 32];
+static __device__ long long gx_phase_clk[64 * 32];   // one copy per translation unit (development builds only)
 #define GX_PHASE(i) do { if (threadIdx.x == 0 && blockIdx.x < 64) gx_phase_clk[blockIdx.x * 32 + (i)] = clock64(); } while (0)
 #else
 #define GX_PHASE(i) do { } while (0)
@@ -457,7 +457,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
         x_inverse_global_rw<C>(W, twx, p.dkx, p.dky, tmp);
     }
 
-    const float2* __restrict__ dchi = p.dchi + (size_t)szj * NX * NY;
+    const float2* dchi = p.dchi + (size_t)szj * NX * NY;   // written by the overlapping chi grid: no __restrict__/ld.nc
     pdl_wait();                     // chi planes of this call are complete and visible from here on
     for (int bt = 0; bt < C::NBATCH; ++bt) {
         // ---- a4 (y part): rows p and p+NX/2 of the batch

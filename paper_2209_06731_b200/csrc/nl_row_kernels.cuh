@@ -17,7 +17,6 @@
 // see nl_kernels.cuh).  Workspace dchi for this family: float2 (d_x chi, d_y chi) at [y][x position].
 #pragma once
 #include "nl_kernels.cuh"
-#include "nl_pair_kernels.cuh"
 
 namespace gx {
 
@@ -148,18 +147,18 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
     x_inverse<C, false>(W, twx, p.dkx, p.dky, S);
     GX_PHASE(2);
 
-    const float2* __restrict__ dchi = p.dchi + (size_t)szj * NX * NY;
+    const float2* dchi = p.dchi + (size_t)szj * NX * NY;
     pdl_wait();                     // chi planes of this call are complete and visible from here on
     GX_PHASE(3);
     // ---- a4 (y part) + a5 + a6 (y part) + a7 (ky), one x row per thread, all in registers
     for (int row = threadIdx.x; row < NX; row += C::NT) {
         float2* __restrict__ Wr = W + row * C::NCOL;
-        const float2* __restrict__ dc = dchi + row;
+        const float2* dc = dchi + row;     // written by the chi grid that overlaps this one (PDL): coherent loads after pdl_wait
         // chi pairs of the first output group are requested before the transform starts, those of group
         // k1+1 while group k1 is transformed: the L2 latency of dchi hides behind the butterflies
         float2 d[8], dn[8];
 #pragma unroll
-        for (int k2 = 0; k2 < 8; ++k2) d[k2] = __ldg(dc + (8 * k2) * NX);
+        for (int k2 = 0; k2 < 8; ++k2) d[k2] = dc[(8 * k2) * NX];
 #pragma unroll
         for (int k2 = 0; k2 < 8; ++k2) {       // groups 1 and 2 towards L1 (no registers held)
             asm volatile("prefetch.global.L1 [%0];" ::"l"(dc + (1 + 8 * k2) * NX));
@@ -181,7 +180,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
         for (int k1 = 0; k1 < 8; ++k1) {
             if (k1 < 7) {
 #pragma unroll
-                for (int k2 = 0; k2 < 8; ++k2) dn[k2] = __ldg(dc + (k1 + 1 + 8 * k2) * NX);
+                for (int k2 = 0; k2 < 8; ++k2) dn[k2] = dc[(k1 + 1 + 8 * k2) * NX];
             }
             if (k1 < 5) {
 #pragma unroll
@@ -205,183 +204,6 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
     x_forward<C>(W, twx, p.bhat + (size_t)unit * NK, p.scale);
 
     // ---- publish (see bracket_kernel)
-    __syncthreads();
-    GX_PHASE(5);
-    if (threadIdx.x == 0) { __threadfence(); atomicAdd(p.count + (s * p.Nm + m) * p.Nz + z, 1u); }
-}
-
-// ================================================================================================
-// "rowp": the row family with the x passes of the packed-FP32 family (nl_pair_kernels.cuh).  The r01c
-// capture of bracket_row_kernel shows its main phases issue-bound (stall "not selected" on top), and the x
-// passes hold half of its instructions; carrying two ky columns per thread through FADD2/FFMA2 removes about
-// a third of them.  W is the planar 32-bit layout of the packed family; a row thread reads its 2*NAKY-1
-// inputs and writes its NAKY outputs at compile-time slots (lanes over rows, odd row stride: conflict-free).
-template <int NX_, int NY_, int RX1_, int RX2_, int NT_, int MINB_>
-struct RowPairCfg {
-    static constexpr int NX = NX_, NY = NY_, RX1 = RX1_, RX2 = RX2_, NT = NT_, MINB = MINB_;
-    static constexpr int K = (NX - 1) / 3, Q = (NY - 1) / 3;
-    static constexpr int NAKX = 2 * K + 1, NAKY = Q + 1, NK = NAKX * NAKY;
-    static constexpr int NP = NAKY / 2, NPAIR = 2 * NP, NSLOT = 2 * NPAIR, RS = NSLOT + 1;
-    static constexpr int W_WORDS = ((2 * NX * RS + 3) / 4) * 4;
-    static constexpr int S_MIN = 8 * NK > W_WORDS ? 8 * NK - W_WORDS : 0;          // W + S hold 4 raw planes
-    static constexpr int S_WORDS = ((2 * NK > S_MIN ? 2 * NK : S_MIN) + 3) / 4 * 4;
-    static constexpr int SMEM_BYTES = (W_WORDS + S_WORDS) * 4 + NX * 8;
-    static constexpr unsigned zero_mask(int R1, int R2, int N, int KK) {
-        unsigned m = 0;
-        for (int n1 = 0; n1 < R1; ++n1)
-            if (!(n1 * R2 <= KK || n1 * R2 + R2 - 1 >= N - KK)) m |= 1u << n1;
-        return m;
-    }
-    static constexpr unsigned ZMX = zero_mask(RX1, RX2, NX, K);
-    static constexpr zm_t zero_mask_y() {
-        zm_t m = 0;
-        for (int n = 0; n < NY; ++n)
-            if (n > Q && n < NY - Q) m |= 1ull << n;
-        return m;
-    }
-    static constexpr zm_t ZMY = zero_mask_y();
-    // slot of y index n in a planar W row (inverse data) and of kept ky = k (forward data)
-    __host__ __device__ static constexpr int slot_in(int n) {
-        return n <= Q ? ((n & 1) ? NPAIR : 0) + n / 2 : (((NY - n) & 1) ? NPAIR : 0) + NP + (NY - n) / 2;
-    }
-    __host__ __device__ static constexpr int slot_out(int k) { return ((k & 1) ? NP : 0) + k / 2; }
-    static_assert(NY == 64 && NAKY % 2 == 0, "single-thread 64-point y transform, ky pairs");
-    static_assert(RX1 * RX2 == NX, "radix split");
-    static_assert(SMEM_BYTES <= 232448, "plane does not fit in shared memory");
-};
-
-template <class C>
-__device__ __forceinline__ void rowp_load(const float* __restrict__ Wr, float2 (&v)[64]) {
-    constexpr int IM = C::NX * C::RS;
-#pragma unroll
-    for (int n = 0; n < 64; ++n) {
-        if (n <= C::Q || n >= C::NY - C::Q) v[n] = make_float2(Wr[C::slot_in(n)], Wr[IM + C::slot_in(n)]);
-        else v[n] = make_float2(0.f, 0.f);
-    }
-}
-
-template <class C>
-__global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_rowp_kernel(const NlParams p) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float* W = reinterpret_cast<float*>(smem_raw);
-    float4* S = reinterpret_cast<float4*>(W + C::W_WORDS);
-    float2* twx = reinterpret_cast<float2*>(W + C::W_WORDS + C::S_WORDS);
-    constexpr int NK2 = C::NK / 2;
-    const int unit = blockIdx.x;                 // (s*Nz + z)*J + j
-    const int z = (unit / p.J) % p.Nz;
-    const float4* __restrict__ phi = reinterpret_cast<const float4*>(p.phi + (size_t)z * C::NK);
-    const float2* __restrict__ M = reinterpret_cast<const float2*>(p.M + (size_t)unit * C::NK);
-    pdl_launch_dependents();
-    for (int i = threadIdx.x; i < C::NX; i += C::NT) twx[i] = p.twx[i];
-    for (int i = threadIdx.x; i < NK2; i += C::NT) {
-        const float4 f = __ldg(phi + i);
-        const float2 m = __ldg(M + i);
-        S[i] = make_float4(f.x * m.x, f.z * m.y, f.y * m.x, f.w * m.y);
-    }
-    __syncthreads();
-    px_inverse<C>(W, twx, p.dkx, p.dky, S);
-    float2* __restrict__ dchi = p.dchi + (size_t)unit * C::NX * C::NY;
-    for (int row = threadIdx.x; row < C::NX; row += C::NT) {
-        float2 v[64];
-        rowp_load<C>(W + row * C::RS, v);
-        dft<64, +1, C::ZMY>(v);
-#pragma unroll
-        for (int y = 0; y < 64; ++y) dchi[y * C::NX + row] = v[y];
-    }
-}
-
-template <class C>
-__global__ void __launch_bounds__(C::NT, C::MINB) bracket_rowp_kernel(const NlParams p) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float* W = reinterpret_cast<float*>(smem_raw);
-    float4* S = reinterpret_cast<float4*>(W + C::W_WORDS);
-    float2* twx = reinterpret_cast<float2*>(W + C::W_WORDS + C::S_WORDS);
-    constexpr int NX = C::NX, NY = C::NY, NK = C::NK, IM = NX * C::RS;
-
-    const int unit = blockIdx.x;                 // ((s*Nz + z)*J + j)*Nm + m
-    const int m = unit % p.Nm;
-    const int szj = unit / p.Nm;
-    const int j = szj % p.J;
-    const int z = (szj / p.J) % p.Nz;
-    const int s = szj / (p.J * p.Nz);
-    const size_t lstride = (size_t)p.Nz * NK;
-    const float2* __restrict__ g0 = p.g + ((size_t)(s * p.Nm + m) * p.Nl * p.Nz + z) * NK;
-
-    __shared__ unsigned long long stage_bar;
-    __shared__ float Tsh[16];
-    unsigned bar_parity = 0;
-    GX_PHASE(0);
-    if (threadIdx.x == 0) mbar_init(&stage_bar, 1);
-    if (threadIdx.x < p.Nl) Tsh[threadIdx.x] = __ldg(p.T + j * p.Nl + threadIdx.x);
-    __syncthreads();
-    pdl_launch_dependents();
-    for (int i = threadIdx.x; i < NX; i += C::NT) twx[i] = p.twx[i];
-    pstage_combine_tma<C>(W, S, &stage_bar, bar_parity, g0, lstride, Tsh, p.Nl);     // a2
-    __syncthreads();
-    GX_PHASE(1);
-    px_inverse<C>(W, twx, p.dkx, p.dky, S);                                          // a3 + a4 (x part)
-    GX_PHASE(2);
-
-    const float2* __restrict__ dchi = p.dchi + (size_t)szj * NX * NY;
-    pdl_wait();                     // chi planes of this call are complete and visible from here on
-    GX_PHASE(3);
-    for (int row = threadIdx.x; row < NX; row += C::NT) {
-        float* __restrict__ Wr = W + row * C::RS;
-        const float2* __restrict__ dc = dchi + row;
-        float2 d[8], dn[8];
-#pragma unroll
-        for (int k2 = 0; k2 < 8; ++k2) d[k2] = __ldg(dc + (8 * k2) * NX);
-#pragma unroll
-        for (int k2 = 0; k2 < 8; ++k2) {
-            asm volatile("prefetch.global.L1 [%0];" ::"l"(dc + (1 + 8 * k2) * NX));
-            asm volatile("prefetch.global.L1 [%0];" ::"l"(dc + (2 + 8 * k2) * NX));
-        }
-        float2 y[64];
-        {
-            float2 v[64];
-            rowp_load<C>(Wr, v);
-            dft_split_col<64, 8, 8, +1, C::ZMY, 0>(v, y);
-        }
-        float b[64];
-#pragma unroll
-        for (int k1 = 0; k1 < 8; ++k1) {
-            if (k1 < 7) {
-#pragma unroll
-                for (int k2 = 0; k2 < 8; ++k2) dn[k2] = __ldg(dc + (k1 + 1 + 8 * k2) * NX);
-            }
-            if (k1 < 5) {
-#pragma unroll
-                for (int k2 = 0; k2 < 8; ++k2) asm volatile("prefetch.global.L1 [%0];" ::"l"(dc + (k1 + 3 + 8 * k2) * NX));
-            }
-            float2 u[8];
-#pragma unroll
-            for (int n2 = 0; n2 < 8; ++n2) u[n2] = y[k1 * 8 + n2];
-            Dft<8, +1, sub_mask_second<8, 8, C::ZMY>()>::run(u);
-#pragma unroll
-            for (int k2 = 0; k2 < 8; ++k2) {
-                b[k1 + 8 * k2] = fmaf(d[k2].y, u[k2].x, -d[k2].x * u[k2].y);
-                d[k2] = dn[k2];
-            }
-        }
-        // 64-point real forward transform (see row_forward_real), outputs to the planar forward slots
-        float2 zc[32];
-#pragma unroll
-        for (int i = 0; i < 32; ++i) zc[i] = make_float2(b[2 * i], b[2 * i + 1]);
-        dft<32, -1>(zc);
-#pragma unroll
-        for (int k = 0; k <= C::Q; ++k) {
-            const float2 a = zc[k], c = zc[(32 - k) % 32];
-            const float2 e = make_float2(0.5f * (a.x + c.x), 0.5f * (a.y - c.y));
-            const float2 o = make_float2(0.5f * (a.y + c.y), 0.5f * (c.x - a.x));
-            const float2 x = cadd(e, twiddle<64, -1>(o, k));
-            Wr[C::slot_out(k)] = x.x;
-            Wr[IM + C::slot_out(k)] = x.y;
-        }
-    }
-    __syncthreads();
-    GX_PHASE(4);
-    px_forward<C>(W, twx, p.bhat + (size_t)unit * NK, p.scale);                      // a6 (x part) + a7
-
     __syncthreads();
     GX_PHASE(5);
     if (threadIdx.x == 0) { __threadfence(); atomicAdd(p.count + (s * p.Nm + m) * p.Nz + z, 1u); }

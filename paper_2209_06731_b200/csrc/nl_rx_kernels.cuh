@@ -623,7 +623,7 @@ __device__ __forceinline__ void st_release_u32(unsigned* p, unsigned v) {
 
 #ifdef GX_PHASE_TIMING
 // development builds: per group and per processed item, clock64() at phase boundaries and %globaltimer at the start
-__device__ long long gx_phase2_clk[512 * 8 * 12];
+static __device__ long long gx_phase2_clk[512 * 8 * 12];
 __device__ __forceinline__ long long gx_globaltimer() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 #define GX_PHASE2(i) do { if (tid == 0 && gid < 512 && round < 8) gx_phase2_clk[(gid * 8 + round) * 12 + (i)] = ((i) == 0 ? gx_globaltimer() : clock64()); } while (0)
 #else

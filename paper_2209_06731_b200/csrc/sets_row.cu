@@ -1,0 +1,43 @@
+// sets_row.cu -- instantiations and launchers of the row family (nl_row_kernels.cuh).
+#include "kernel_sets.h"
+#include "nl_row_kernels.cuh"
+
+namespace gxhost {
+namespace {
+// ---- row family (nl_row_kernels.cuh): whole y direction of an x row in one thread's registers; NY = 64
+template <class CB, class CC> cudaError_t prepare_row() {
+    cudaError_t e = set_smem(gx::chi_planes_row_kernel<CC>, CC::SMEM_BYTES);
+    return e != cudaSuccess ? e : set_smem(gx::bracket_row_kernel<CB>, CB::SMEM_BYTES);
+}
+template <class C> cudaError_t launch_chi_row_t(const NlParams& p, int units, cudaStream_t st) {
+    gx::chi_planes_row_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
+    return cudaGetLastError();
+}
+template <class C> cudaError_t launch_bracket_row_t(const NlParams& p, int units, cudaStream_t st) {
+    return launch_pdl(gx::bracket_row_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
+}
+template <class CB, class CC> constexpr KernelSet make_row_set() {
+    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1,
+                  "chi and bracket kernels must share the x radices (same permuted x order)");
+    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, GX_FAMILY_ROW, &prepare_row<CB, CC>, &launch_chi_row_t<CC>,
+                     &launch_bracket_row_t<CB>, false, nullptr};
+}
+using R64x64   = gx::RowCfg<64, 64, 8, 8, 64, 6>;
+using R128x64  = gx::RowCfg<128, 64, 16, 8, 128, 3>;
+using R192x64  = gx::RowCfg<192, 64, 16, 12, 192, 2>;
+using RC192x64 = gx::RowCfg<192, 64, 16, 12, 384, 1>;   // chi planes: < 1 wave, more threads for the x passes
+using R256x64  = gx::RowCfg<256, 64, 16, 16, 256, 1>;
+const KernelSet kRowSets[] = {
+    make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, RC192x64>(),
+    make_row_set<R256x64, R256x64>(),
+};
+
+}  // namespace
+const KernelSet* find_row(int Nx, int Ny) { return find_in(kRowSets, Nx, Ny); }
+}  // namespace gxhost
+
+#ifdef GX_PHASE_TIMING
+extern "C" int gx_debug_phase_clocks(long long* out) {
+    return cudaMemcpyFromSymbol(out, gx::gx_phase_clk, sizeof(long long) * 64 * 32) == cudaSuccess ? 0 : -1;
+}
+#endif

@@ -262,29 +262,34 @@ def hermitian_fix_ky0(a: np.ndarray) -> None:
     a[..., 0, 0] = 0.0
 
 
-def make_state(cfg: Config, geo: dict | None = None, planes=None) -> np.ndarray:
+def make_state(cfg: Config, geo: dict | None = None, planes=None, hermite_block=None) -> np.ndarray:
     """Seeded g of shape cfg.g_shape, complex64 (generated in fp64, rounded once).
 
     ``planes``: optional iterable of (s, m) pairs; if given only those (s,m) slabs are filled
     (others are zero) -- lets the large configurations be sampled without 2x600 MB of fp64.
+    ``hermite_block``: optional (m0, m1): return only the slab g[:, m0:m1] of the SAME global state (the
+    counter-based generator makes any slice reproducible) -- one rank's share in the multi-GPU bench.
     """
     geo = geo or geometry_arrays(cfg)
     env = _envelope(cfg, geo)                       # [z][kx][ky]
     Ns, Nm, Nl, Nz, nakx, naky = cfg.g_shape
-    g = np.zeros(cfg.g_shape, dtype=np.complex64)
+    m0, m1 = (0, Nm) if hermite_block is None else hermite_block
+    if not (0 <= m0 < m1 <= Nm):
+        raise ValueError("hermite_block out of range")
+    g = np.zeros((Ns, m1 - m0, Nl, Nz, nakx, naky), dtype=np.complex64)
     per_l = Nz * nakx * naky
     want = None if planes is None else set(planes)
     for s in range(Ns):
-        for m in range(Nm):
+        for m in range(m0, m1):
             if want is not None and (s, m) not in want:
                 continue
             for l in range(Nl):
-                flat0 = ((s * Nm + m) * Nl + l) * per_l      # complex element counter
+                flat0 = ((s * Nm + m) * Nl + l) * per_l      # complex element counter of the global layout
                 n = counter_normals(cfg.seed, 2 * flat0, 2 * per_l)
                 v = (n[0::2] + 1j * n[1::2]).reshape(Nz, nakx, naky)
                 v *= env * (cfg.decay ** (-(l + m))) * cfg.species[s].amp
                 hermitian_fix_ky0(v)
-                g[s, m, l] = v.astype(np.complex64)
+                g[s, m - m0, l] = v.astype(np.complex64)
     return g
 
 

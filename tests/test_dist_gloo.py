@@ -24,6 +24,33 @@ def test_hermite_blocks_partition():
     assert all(b[2] == Nm * world for b in blocks)
 
 
+def test_rank_blocks_are_slices_of_one_seeded_state():
+    """bench.py --gpus N: rank r owns the Hermite block [m0, m1) of ONE global seeded state (weak scaling: Nm per
+    rank fixed); the blocks of all ranks tile the single-process state bit for bit."""
+    import numpy as np
+    from paper_2209_06731_b200 import dist as D, inputs as I
+    world = 2
+    cfg = I.Config("t", 16, 16, 2, 2, 3, [I.Species()], seed=11)
+    blocks = [D.hermite_block(cfg.Nm, r, world) for r in range(world)]
+    cfg_global = I.Config(**{**cfg.__dict__, "Nm": blocks[0][2]})
+    whole = I.make_state(cfg_global)
+    for (m0, m1, _) in blocks:
+        part = I.make_state(cfg_global, hermite_block=(m0, m1))
+        assert part.shape[1] == cfg.Nm and np.array_equal(part, whole[:, m0:m1])
+    # the m = 0 slab every rank uses for the replicated field solve is the global one
+    assert np.array_equal(I.make_state(cfg_global, hermite_block=(0, 1)), whole[:, 0:1])
+
+
+def test_bench_refuses_more_gpus_than_visible():
+    import subprocess
+    env = dict(os.environ)
+    env.pop("WORLD_SIZE", None)
+    env["CUDA_VISIBLE_DEVICES"] = ""
+    res = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "3", "--warmup", "3"],
+                         env=env, capture_output=True, text=True, timeout=300)
+    assert res.returncode != 0 and "--gpus 2" in (res.stderr + res.stdout)
+
+
 def test_two_rank_gloo_aggregate():
     script = textwrap.dedent("""
         import sys
