@@ -96,6 +96,13 @@ int gx_boundary_set(gx_grid* g, int linked);
  * hyper-collisions nu_hyp m^p, p = Nm/2, strength f_hyp (Eq. 4.27-4.28). Defaults 0.05, 4, 1. */
 int gx_dissipation_set(gx_grid* g, double D_hyper, int n_hyper, double f_hyp);
 
+/* Wave-absorbing layer at the ends of every (extended) z domain, Eq. 4.30:
+ * dG_{l,m}/dt -= d(z_hat) H_{l,m} for ky != 0, d = A [1 - 2 z_hat^2/(1 + z_hat^4)] for |z_hat| < 1, z_hat the
+ * distance from either end of the domain in units of width_fraction * L_z (the paper uses 1/8 and A = 0.1/dt).
+ * With gx_boundary_set(0) every mode is its own domain of length 2 pi.  A = 0 (default) switches the layer off.
+ * Call before gx_geometry_set. */
+int gx_damping_set(gx_grid* g, double A, double width_fraction);
+
 /* Per-z geometry coefficients (HOST arrays of length Nz, P:677-694 Eq. E4-E11) and the constant
  * gradpar = b.grad z.  bmag, gds2, gds21, gds22 define k_perp^2 and b_s and hence the
  * gyroaverage table M[s][z][j][kx][ky] = J0(sqrt(2 x_j b_s)) built here in fp64; the drift,
@@ -110,8 +117,10 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
 int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev,
                      void* cuda_stream);
 
-/* Same call with HOST buffers (pinned for full speed): copies g and phi to internal device buffers,
- * runs gx_nonlinear_rhs, copies out back, and synchronises the stream before returning. */
+/* Same call with HOST buffers (pinned for full speed).  The evaluation is diagonal in the Hermite index, so it
+ * is pipelined over blocks of moments on three streams: the host-to-device copy of block b+1 and the
+ * device-to-host copy of block b-1 overlap the kernels of block b (chi planes computed once).  Ordered after
+ * the work already queued on `cuda_stream`; synchronises before returning. */
 int gx_nonlinear_rhs_host(gx_grid* g, const void* g_host, const void* phi_host, void* out_host,
                           void* cuda_stream);
 

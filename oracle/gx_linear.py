@@ -29,8 +29,10 @@ Readings of silent / garbled points (rows L1-L8):
       modes kx_0 + n dk (n integer, inside the dealiased set) of one ky form ONE periodic extended domain of
       L 2 pi, on which mode n holds the segment theta = z - 2 pi n of the ballooning function; the z operators
       are spectral on that domain (k = j/L, Nyquist dropped in the derivative).  dk is a whole number
-      jtwist*q of kx grid steps because Lx/Ly = jtwist/(2 pi |shat|).  No end-damping layer
-      (Eq. 4.30 is optional, P:333).
+      jtwist*q of kx grid steps because Lx/Ly = jtwist/(2 pi |shat|).
+  L9  end-damping layer Eq. 4.30, optional (``damping=dict(A=..., width_frac=1/8)``): distance
+      measured from BOTH ends of each extended domain, z_width = L_z/8 with L_z the length of that domain, acts
+      on H, non-zonal modes only; A is a free parameter (the paper uses 0.1/dt).
   L3  w_d^gradB = (ky gbdrift + kx gbdrift0/shat)/2, w_d^kappa = (ky cvdrift + kx cvdrift0/shat)/2
       (P:229 with Eq. E9-E11: the arrays carry a factor 2 and gbdrift0 a factor shat).
   L4  i w_* = i ky; 1/L_n = fprim, 1/L_T = tprim.
@@ -195,9 +197,39 @@ def jtwist_of(dkx, dky, shat):
     return int(round(j))
 
 
+def end_damping_profile(Nz, Nx, Ny, A, width_frac=0.125, boundary="periodic", jtwist=None):
+    """d[z][kx][ky] of the wave-absorbing layer, Eq. 4.30: d(zh) = A [1 - 2 zh^2/(1 + zh^4)] for
+    |zh| < 1, zh = (theta - theta_end)/z_width the distance from either end of the extended z domain in units
+    of z_width = width_frac * L_z (L_z/8), L_z = 2 pi L the length of the extended domain of L linked
+    modes; zero elsewhere and for the zonal modes ky = 0.  Mode n of a chain holds theta = z - 2 pi n (reading L2),
+    so the domain runs from theta_lo = -pi - 2 pi (L-1) to theta_hi = pi; boundary="periodic": every mode is
+    its own domain (L = 1).  The end theta_hi itself is not a grid point (periodic grid z_i = -pi + 2 pi i/Nz)."""
+    nakx, naky = O.dealiased_counts(Nx, Ny)
+    z = -math.pi + 2.0 * math.pi * np.arange(Nz) / Nz
+    d = np.zeros((Nz, nakx, naky))
+    if boundary == "periodic":
+        chains = [(q, [i]) for q in range(naky) for i in range(nakx)]
+    else:
+        chains = twist_shift_chains(Nx, Ny, jtwist)
+    for q, rows in chains:
+        if q == 0:
+            continue
+        L = len(rows)
+        Lz = 2.0 * math.pi * L
+        w = width_frac * Lz
+        th_lo, th_hi = -math.pi - 2.0 * math.pi * (L - 1), math.pi
+        for n, i in enumerate(rows):
+            theta = z - 2.0 * math.pi * n
+            for dist in (theta - th_lo, th_hi - theta):
+                zh = dist / w
+                inside = zh < 1.0
+                d[inside, i, q] += A * (1.0 - 2.0 * zh[inside] ** 2 / (1.0 + zh[inside] ** 4))
+    return d
+
+
 def linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper=0.05, n_hyper=4, f_hyp=1.0,
                terms=("stream", "mirror", "drift", "drive", "coll", "hypervisc", "hypercoll"),
-               boundary="periodic"):
+               boundary="periodic", damping=None):
     """dG/dt from every term of Eq. 4.9 except the nonlinear one (see module header).  fp64.
     G [s][m][l][z][kx][ky], Phi [z][kx][ky]; geo holds the per-z arrays of P:677-694 plus gradpar.
     ``terms`` selects contributions (the pins test them one at a time)."""
@@ -213,6 +245,9 @@ def linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper=0.05, n_hyp
     iky = 1j * ky[None, None, :]
     kp2max = float(np.max(kp2))
     out = np.zeros_like(G)
+    dend = None
+    if damping is not None and damping.get("A", 0.0) != 0.0:                           # Eq. 4.30 (optional)
+        dend = end_damping_profile(Nz, Nx, Ny, damping["A"], damping.get("width_frac", 0.125), boundary, jtw)
     dpar = lambda f: apply_z_operator(f, "d", gradpar, Nx, Ny, boundary, jtw)          # grad_par
     kpar = lambda f: apply_z_operator(f, "a", gradpar, Nx, Ny, boundary, jtw)          # |k_par|
     for s, sp in enumerate(species):
@@ -272,17 +307,20 @@ def linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper=0.05, n_hyp
                     r -= D_hyper * (kp2 / kp2max) ** n_hyper * G[s, m, l]
                 if "hypercoll" in terms and f_hyp != 0.0 and m > 2:
                     r -= nuhyp_fac * float(m) ** p_hyp * kpar(G[s, m, l])
+                if dend is not None:
+                    r -= dend * Hlm(l, m)                                   # Eq. 4.30: acts on H, ky != 0 only
                 out[s, m, l] = r
     return out
 
 
 # ============================================================================ full RHS and time step
 def rhs(G, Nx, Ny, dkx, dky, shat, geo, species, tau_fac=1.0, adiabatic=None, D_hyper=0.05, n_hyper=4,
-        f_hyp=1.0, nonlinear=True, planes=None, boundary="periodic"):
+        f_hyp=1.0, nonlinear=True, planes=None, boundary="periodic", damping=None):
     """gx_rhs: Phi from quasineutrality, then -N + linear terms (Eq. 4.9)."""
     adiabatic = (len(species) == 1) if adiabatic is None else adiabatic
     Phi = O.field_solve(G, Nx, Ny, dkx, dky, shat, geo, species, tau_fac=tau_fac, adiabatic=adiabatic)
-    out = linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper, n_hyper, f_hyp, boundary=boundary)
+    out = linear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, D_hyper, n_hyper, f_hyp, boundary=boundary,
+                     damping=damping)
     if nonlinear:
         out = out + O.nonlinear_rhs(G, Phi, Nx, Ny, dkx, dky, shat, geo, species, method="dft", planes=planes)
     return out

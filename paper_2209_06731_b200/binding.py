@@ -21,7 +21,7 @@ GX_OK, GX_ERR_ARG, GX_ERR_STATE, GX_ERR_UNSUPPORTED, GX_ERR_CUDA, GX_ERR_ALLOC =
 FAMILY_NAMES = {0: "scalar", 3: "row", 5: "rx", 6: "rxp", 7: "rxw"}
 
 EXPORTED = ["gx_grid_create", "gx_grid_destroy", "gx_box_set", "gx_species_set", "gx_adiabatic_set",
-            "gx_dissipation_set", "gx_boundary_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_host",
+            "gx_dissipation_set", "gx_boundary_set", "gx_damping_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_host",
             "gx_field_solve", "gx_rhs", "gx_linear_rhs", "gx_ssprk3_step", "gx_query", "gx_export_maps",
             "gx_export_tables", "gx_profile_set", "gx_profile_get", "gx_last_error", "gx_ubench_fp32"]
 
@@ -51,6 +51,7 @@ def load():
     lib.gx_adiabatic_set.argtypes = [vp, i, d]
     lib.gx_dissipation_set.argtypes = [vp, d, i, d]
     lib.gx_boundary_set.argtypes = [vp, i]
+    lib.gx_damping_set.argtypes = [vp, d, d]
     lib.gx_geometry_set.argtypes = [vp] + [dp] * 10 + [d]
     lib.gx_nonlinear_rhs.argtypes = [vp, vp, vp, vp, vp]
     lib.gx_nonlinear_rhs_host.argtypes = [vp, vp, vp, vp, vp]
@@ -113,6 +114,10 @@ def gx_adiabatic_set(h, enabled, tau_fac=1.0):
 
 def gx_boundary_set(h, linked):
     _check(h, load().gx_boundary_set(h, int(linked)))
+
+
+def gx_damping_set(h, A, width_fraction=0.125):
+    _check(h, load().gx_damping_set(h, A, width_fraction))
 
 
 def gx_dissipation_set(h, D_hyper, n_hyper, f_hyp):
@@ -206,7 +211,7 @@ class Grid:
     """Owns a gx_grid handle configured from an ``inputs.Config``; methods take torch CUDA tensors
     (complex64, contiguous) and pass their data pointers and the current stream to the C-ABI."""
 
-    def __init__(self, cfg, geo=None, linked=False):
+    def __init__(self, cfg, geo=None, linked=False, damping=None):
         from . import inputs as I
         self.cfg = cfg
         self.geo = geo or I.geometry_arrays(cfg)
@@ -216,6 +221,8 @@ class Grid:
             gx_species_set(self.h, s, sp.Z, sp.mass, sp.temp, sp.dens, sp.tprim, sp.fprim, sp.nu_ss)
         gx_adiabatic_set(self.h, cfg.Ns == 1, cfg.tau_fac)
         gx_boundary_set(self.h, linked)
+        if damping:
+            gx_damping_set(self.h, damping["A"], damping.get("width_frac", 0.125))
         g = self.geo
         gx_geometry_set(self.h, g["bmag"], g["gds2"], g["gds21"], g["gds22"], g["gbdrift"], g["gbdrift0"],
                         g["cvdrift"], g["cvdrift0"], g["bgrad"], g["jacobian"], g["gradpar"])

@@ -104,6 +104,7 @@ struct gx_grid {
     double tau_fac = 1.0;
     double D_hyper = 0.05, f_hyp = 1.0;
     int n_hyper = 4;
+    double damp_A = 0.0, damp_width = 0.125;    // end-damping layer Eq. 4.30 (off by default)
     std::vector<Species> sp;
     std::vector<double> bmag, gds2, gds21, gds22, gbdrift, gbdrift0, cvdrift, cvdrift0, bgrad, jacobian;
     bool have_lin_geo = false;
@@ -117,7 +118,13 @@ struct gx_grid {
     unsigned* dcount = nullptr;
     unsigned* dchi_flag = nullptr;              // [s][z][j] epoch of the last call that produced the chi plane (persistent family)
     unsigned calls = 0;                         // number of gx_nonlinear_rhs calls issued (counter epoch)
-    float2 *dgbuf = nullptr, *dphibuf = nullptr, *doutbuf = nullptr;   // for the *_host entry point
+    float2 *dgbuf = nullptr, *dphibuf = nullptr, *doutbuf = nullptr;   // for the *_host entry point: Hermite-block buffers each way
+    unsigned* dcount_blk = nullptr;             // arrival counters of the block-wise evaluations of the *_host entry point
+    cudaStream_t st_in = nullptr, st_out = nullptr, st_cmp = nullptr;
+    cudaEvent_t ev_user = nullptr;
+    cudaGraphExec_t host_graph = nullptr;       // captured pipeline of the *_host entry point for the pointers below
+    const void *hg_g = nullptr, *hg_phi = nullptr, *hg_out = nullptr;
+    std::vector<cudaEvent_t> ev_host;
     gx::LinTables lin;                                                  // linear-term tables
     float2* dphi_rhs = nullptr;                                         // phi of gx_rhs
     float2 *drk_y = nullptr, *drk_k = nullptr;                          // SSP-RK3 stage and slope buffers
@@ -130,6 +137,7 @@ struct gx_grid {
 
 namespace {
 
+constexpr int kHostBufs = 3;       // Hermite-block buffers each way of gx_nonlinear_rhs_host
 bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
 bool overlap(const void* a, const void* b, size_t bytes) {
     const uintptr_t x = reinterpret_cast<uintptr_t>(a), y = reinterpret_cast<uintptr_t>(b);
@@ -269,6 +277,13 @@ int gx_grid_destroy(gx_grid* g) {
     cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dcount); cudaFree(g->dchi_flag); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
     cudaFree(g->dphi_rhs); cudaFree(g->drk_y); cudaFree(g->drk_k);
     for (auto e : g->ev_pool) cudaEventDestroy(e);
+    for (auto e : g->ev_host) cudaEventDestroy(e);
+    if (g->host_graph) cudaGraphExecDestroy(g->host_graph);
+    if (g->st_in) cudaStreamDestroy(g->st_in);
+    if (g->st_cmp) cudaStreamDestroy(g->st_cmp);
+    if (g->ev_user) cudaEventDestroy(g->ev_user);
+    if (g->st_out) cudaStreamDestroy(g->st_out);
+    cudaFree(g->dcount_blk);
     gx::lin_tables_free(g->lin);
     delete g;
     return GX_OK;
@@ -315,6 +330,14 @@ int gx_dissipation_set(gx_grid* g, double D_hyper, int n_hyper, double f_hyp) {
     if (!g) return GX_ERR_ARG;
     if (D_hyper < 0 || n_hyper < 0 || f_hyp < 0) return fail(g, GX_ERR_ARG, "negative dissipation parameter");
     g->D_hyper = D_hyper; g->n_hyper = n_hyper; g->f_hyp = f_hyp;
+    g->geo_set = false;
+    return GX_OK;
+}
+
+int gx_damping_set(gx_grid* g, double A, double width_fraction) {
+    if (!g) return GX_ERR_ARG;
+    if (A < 0 || !(width_fraction > 0) || width_fraction > 0.5) return fail(g, GX_ERR_ARG, "gx_damping_set: A >= 0, 0 < width_fraction <= 1/2");
+    g->damp_A = A; g->damp_width = width_fraction;
     g->geo_set = false;
     return GX_OK;
 }
@@ -383,6 +406,7 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
         in.adiabatic = g->adiabatic; in.tau_fac = g->tau_fac;
         in.D_hyper = g->D_hyper; in.n_hyper = g->n_hyper; in.f_hyp = g->f_hyp;
         in.linked = g->linked;
+        in.damp_A = g->damp_A; in.damp_width = g->damp_width;
         for (const auto& sp : g->sp)
             in.species.push_back({sp.Z, sp.mass, sp.temp, sp.dens, sp.tprim, sp.fprim, sp.nu});
         std::string msg;
@@ -396,51 +420,44 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
             if (rc) return rc;
         }
     }
+    if (g->host_graph) { cudaGraphExecDestroy(g->host_graph); g->host_graph = nullptr; }   // table pointers may have changed
     g->geo_set = true;
     return GX_OK;
 }
 
-int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream) {
-    if (!g) return GX_ERR_ARG;
-    if (!g_dev || !phi_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: null pointer");
-    const size_t gbytes = (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk * sizeof(float2);
-    if (overlap(g_dev, out_dev, gbytes)) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: out must not alias g");
-    if (misaligned(g_dev) || misaligned(phi_dev) || misaligned(out_dev))
-        return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: device pointers must be 16-byte aligned");
-    if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
-    if (!g->geo_set) return fail(g, GX_ERR_STATE, "gx_nonlinear_rhs: geometry not set");
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    const NlParams p = make_params(g, g_dev, phi_dev, out_dev);
+}  // extern "C"
+
+namespace {
+// Enqueues the kernels of one evaluation for Nm_eff Hermite moments (p.Nm = Nm_eff; the arrays behind p.g / p.out
+// hold exactly those moments).  do_chi = false reuses the chi planes already in the workspace (same phi).
+// count / calls: arrival counters of the separate inverse-Laguerre kernel and their epoch.
+int nl_enqueue(gx_grid* g, NlParams p, int Nm_eff, bool do_chi, unsigned* count, unsigned* calls, cudaStream_t st,
+               cudaEvent_t* ev) {
+    // calls == nullptr: the counters are zeroed by a memset node before the kernels and the target is J itself
+    // (no epoch in the kernel arguments: the sequence can be captured in a CUDA graph and replayed)
+    p.Nm = Nm_eff;
+    p.count = count;
     const int szj = g->Ns * g->Nz * g->J;
-    cudaEvent_t* ev = nullptr;
-    if (g->profile) {
-        if (g->ev_used + 4 > g->ev_pool.size()) {
-            const size_t old = g->ev_pool.size();
-            g->ev_pool.resize(old + 4 * 256);
-            for (size_t i = old; i < g->ev_pool.size(); ++i) GX_CUDA(g, cudaEventCreate(&g->ev_pool[i]));
-        }
-        ev = &g->ev_pool[g->ev_used];
-        g->ev_used += 4;
-        GX_CUDA(g, cudaEventRecord(ev[0], st));
-    }
+    if (!calls && !g->ks->fused_laguerre)
+        GX_CUDA(g, cudaMemsetAsync(count, 0, (size_t)g->Ns * Nm_eff * g->Nz * sizeof(unsigned), st));
     if (g->ks->launch_call) {
         g->calls += 1;
         if (ev) GX_CUDA(g, cudaEventRecord(ev[1], st));
-        GX_CUDA(g, g->ks->launch_call(p, g->dchi_flag, g->calls, szj + szj * g->Nm, st));
+        GX_CUDA(g, g->ks->launch_call(p, g->dchi_flag, g->calls, szj + szj * Nm_eff, st));
         if (ev) { GX_CUDA(g, cudaEventRecord(ev[2], st)); GX_CUDA(g, cudaEventRecord(ev[3], st)); }
         return GX_OK;
     }
-    GX_CUDA(g, g->ks->launch_chi(p, szj, st));
+    if (do_chi) GX_CUDA(g, g->ks->launch_chi(p, szj, st));
     if (ev) GX_CUDA(g, cudaEventRecord(ev[1], st));
-    GX_CUDA(g, g->ks->launch_bracket(p, szj * g->Nm, st));
+    GX_CUDA(g, g->ks->launch_bracket(p, szj * Nm_eff, st));
     if (ev) GX_CUDA(g, cudaEventRecord(ev[2], st));
     if (!g->ks->fused_laguerre) {
         const int vec = (g->nk % 2 == 0) ? 2 : 1;
         const int nkv = (int)(g->nk / vec);
-        dim3 grid((unsigned)((nkv + 255) / 256), (unsigned)(g->Ns * g->Nm * g->Nz));
+        dim3 grid((unsigned)((nkv + 255) / 256), (unsigned)(g->Ns * Nm_eff * g->Nz));
         const int nk = (int)g->nk;
-        g->calls += 1;
-        const unsigned target = g->calls * (unsigned)g->J;
+        unsigned target = (unsigned)g->J;
+        if (calls) { *calls += 1; target = *calls * (unsigned)g->J; }
         cudaError_t e;
 #define GX_LAGINV(L, J)                                                                                        \
     e = (vec == 2) ? launch_pdl(gx::laguerre_inverse_kernel<L, J, 2>, grid, dim3(256), 0, st, p, nk, target)  \
@@ -453,6 +470,34 @@ int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* o
     }
     if (ev) GX_CUDA(g, cudaEventRecord(ev[3], st));
     return GX_OK;
+}
+}  // namespace
+
+extern "C" {
+
+int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_dev || !phi_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: null pointer");
+    const size_t gbytes = (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk * sizeof(float2);
+    if (overlap(g_dev, out_dev, gbytes)) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: out must not alias g");
+    if (misaligned(g_dev) || misaligned(phi_dev) || misaligned(out_dev))
+        return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs: device pointers must be 16-byte aligned");
+    if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
+    if (!g->geo_set) return fail(g, GX_ERR_STATE, "gx_nonlinear_rhs: geometry not set");
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const NlParams p = make_params(g, g_dev, phi_dev, out_dev);
+    cudaEvent_t* ev = nullptr;
+    if (g->profile) {
+        if (g->ev_used + 4 > g->ev_pool.size()) {
+            const size_t old = g->ev_pool.size();
+            g->ev_pool.resize(old + 4 * 256);
+            for (size_t i = old; i < g->ev_pool.size(); ++i) GX_CUDA(g, cudaEventCreate(&g->ev_pool[i]));
+        }
+        ev = &g->ev_pool[g->ev_used];
+        g->ev_used += 4;
+        GX_CUDA(g, cudaEventRecord(ev[0], st));
+    }
+    return nl_enqueue(g, p, g->Nm, true, g->dcount, &g->calls, st, ev);
 }
 
 int gx_profile_set(gx_grid* g, int enabled) {
@@ -479,19 +524,107 @@ int gx_profile_get(gx_grid* g, double* ms, long long* calls) {
 int gx_nonlinear_rhs_host(gx_grid* g, const void* g_host, const void* phi_host, void* out_host, void* cuda_stream) {
     if (!g) return GX_ERR_ARG;
     if (!g_host || !phi_host || !out_host) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs_host: null pointer");
-    const size_t ng = (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk, np = (size_t)g->Nz * g->nk;
+    if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
+    if (!g->geo_set) return fail(g, GX_ERR_STATE, "gx_nonlinear_rhs_host: geometry not set");
+    const size_t per_m = (size_t)g->Nl * g->Nz * g->nk, np = (size_t)g->Nz * g->nk;
+    // Hermite blocks: the term is diagonal in m, so block b of every species is an independent sub-problem that
+    // shares the chi planes.  Three streams: H2D of block b+1 and D2H of block b-1 overlap the kernels of block b
+    // (the PCIe link is full duplex); three block buffers each way.
+    const bool pipelined = g->ks->launch_call == nullptr && g->Nm > 1;
+    int want = 4;       // about four blocks: each is one launch-latency-bound wave of kernels (GX_HOST_BLOCKS overrides)
+    if (const char* e = std::getenv("GX_HOST_BLOCKS")) want = std::max(1, std::atoi(e));
+    const int mb = pipelined ? std::max(1, (g->Nm + want - 1) / want) : g->Nm;      // moments per block
+    const int nb = (g->Nm + mb - 1) / mb;
+    const size_t blk = (size_t)g->Ns * mb * per_m;
     int rc;
     if (!g->dgbuf) {
-        if ((rc = dev_alloc(g, &g->dgbuf, ng))) return rc;
-        if ((rc = dev_alloc(g, &g->doutbuf, ng))) return rc;
+        if ((rc = dev_alloc(g, &g->dgbuf, kHostBufs * blk))) return rc;
+        if ((rc = dev_alloc(g, &g->doutbuf, kHostBufs * blk))) return rc;
         if ((rc = dev_alloc(g, &g->dphibuf, np))) return rc;
+        if ((rc = dev_alloc(g, &g->dcount_blk, (size_t)g->Ns * mb * g->Nz))) return rc;
+        GX_CUDA(g, cudaMemset(g->dcount_blk, 0, (size_t)g->Ns * mb * g->Nz * sizeof(unsigned)));
+        GX_CUDA(g, cudaStreamCreateWithFlags(&g->st_cmp, cudaStreamNonBlocking));
+        GX_CUDA(g, cudaEventCreateWithFlags(&g->ev_user, cudaEventDisableTiming));
+        GX_CUDA(g, cudaStreamCreateWithFlags(&g->st_in, cudaStreamNonBlocking));
+        GX_CUDA(g, cudaStreamCreateWithFlags(&g->st_out, cudaStreamNonBlocking));
+        g->ev_host.resize(3 * 64 + 2);
+        for (auto& e : g->ev_host) GX_CUDA(g, cudaEventCreateWithFlags(&e, std::getenv("GX_HOST_TRACE") ? cudaEventDefault : cudaEventDisableTiming));
     }
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    GX_CUDA(g, cudaMemcpyAsync(g->dgbuf, g_host, ng * sizeof(float2), cudaMemcpyHostToDevice, st));
-    GX_CUDA(g, cudaMemcpyAsync(g->dphibuf, phi_host, np * sizeof(float2), cudaMemcpyHostToDevice, st));
-    if ((rc = gx_nonlinear_rhs(g, g->dgbuf, g->dphibuf, g->doutbuf, cuda_stream))) return rc;
-    GX_CUDA(g, cudaMemcpyAsync(out_host, g->doutbuf, ng * sizeof(float2), cudaMemcpyDeviceToHost, st));
+    if (nb > 64) return fail(g, GX_ERR_UNSUPPORTED, "gx_nonlinear_rhs_host: more than 64 Hermite blocks");
+    // all work runs on three internal streams (the caller's stream may be the legacy default stream, which cannot
+    // be captured); it is ordered after the work already queued on the caller's stream, and the call synchronises
+    cudaStream_t ust = (cudaStream_t)cuda_stream, st = g->st_cmp, sin = g->st_in, sout = g->st_out;
+    GX_CUDA(g, cudaEventRecord(g->ev_user, ust));
+    GX_CUDA(g, cudaStreamWaitEvent(st, g->ev_user, 0));
+    // The whole pipeline (about a hundred copies, launches and event edges) is captured once per set of host
+    // pointers into a CUDA graph and replayed: one launch per call instead of a hundred driver calls.
+    const bool use_graph = pipelined && std::getenv("GX_HOST_NO_GRAPH") == nullptr;
+    if (use_graph && g->host_graph && g->hg_g == g_host && g->hg_phi == phi_host && g->hg_out == out_host) {
+        GX_CUDA(g, cudaGraphLaunch(g->host_graph, st));
+        GX_CUDA(g, cudaStreamSynchronize(st));
+        return GX_OK;
+    }
+    if (use_graph) {
+        if (g->host_graph) { cudaGraphExecDestroy(g->host_graph); g->host_graph = nullptr; }
+        GX_CUDA(g, cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+    }
+    const float2* gh = (const float2*)g_host;
+    float2* oh = (float2*)out_host;
+    cudaEvent_t* e_in = g->ev_host.data();          // block copied in
+    cudaEvent_t* e_cmp = e_in + 64;                 // block computed
+    cudaEvent_t* e_out = e_cmp + 64;                // block copied out
+    cudaEvent_t e_start = g->ev_host[3 * 64], e_phi = g->ev_host[3 * 64 + 1];
+    GX_CUDA(g, cudaEventRecord(e_start, st));       // work already queued on the caller's stream comes first
+    GX_CUDA(g, cudaStreamWaitEvent(sin, e_start, 0));
+    GX_CUDA(g, cudaStreamWaitEvent(sout, e_start, 0));
+    GX_CUDA(g, cudaMemcpyAsync(g->dphibuf, phi_host, np * sizeof(float2), cudaMemcpyHostToDevice, sin));
+    GX_CUDA(g, cudaEventRecord(e_phi, sin));
+    GX_CUDA(g, cudaStreamWaitEvent(st, e_phi, 0));
+    for (int b = 0; b < nb; ++b) {
+        const int m0 = b * mb, nm = std::min(mb, g->Nm - m0);
+        float2* dg = g->dgbuf + (size_t)(b % kHostBufs) * blk;
+        float2* dout = g->doutbuf + (size_t)(b % kHostBufs) * blk;
+        if (b >= kHostBufs) GX_CUDA(g, cudaStreamWaitEvent(sin, e_cmp[b - kHostBufs], 0));       // block buffer free again
+        for (int s = 0; s < g->Ns; ++s)
+            GX_CUDA(g, cudaMemcpyAsync(dg + (size_t)s * nm * per_m, gh + ((size_t)s * g->Nm + m0) * per_m,
+                                       (size_t)nm * per_m * sizeof(float2), cudaMemcpyHostToDevice, sin));
+        GX_CUDA(g, cudaEventRecord(e_in[b], sin));
+        GX_CUDA(g, cudaStreamWaitEvent(st, e_in[b], 0));
+        if (b >= kHostBufs) GX_CUDA(g, cudaStreamWaitEvent(st, e_out[b - kHostBufs], 0));        // its result has left the device
+        const NlParams p = make_params(g, dg, g->dphibuf, dout);
+        if (pipelined) rc = nl_enqueue(g, p, nm, b == 0, g->dcount_blk, nullptr, st, nullptr);
+        else rc = nl_enqueue(g, p, nm, true, g->dcount, &g->calls, st, nullptr);
+        if (rc) {
+            if (use_graph) { cudaGraph_t dead = nullptr; cudaStreamEndCapture(st, &dead); if (dead) cudaGraphDestroy(dead); }
+            return rc;
+        }
+        GX_CUDA(g, cudaEventRecord(e_cmp[b], st));
+        GX_CUDA(g, cudaStreamWaitEvent(sout, e_cmp[b], 0));
+        for (int s = 0; s < g->Ns; ++s)
+            GX_CUDA(g, cudaMemcpyAsync(oh + ((size_t)s * g->Nm + m0) * per_m, dout + (size_t)s * nm * per_m,
+                                       (size_t)nm * per_m * sizeof(float2), cudaMemcpyDeviceToHost, sout));
+        GX_CUDA(g, cudaEventRecord(e_out[b], sout));
+    }
+    GX_CUDA(g, cudaStreamWaitEvent(st, e_out[nb - 1], 0));
+    if (use_graph) {
+        cudaGraph_t graph = nullptr;
+        GX_CUDA(g, cudaStreamEndCapture(st, &graph));
+        cudaError_t e = cudaGraphInstantiate(&g->host_graph, graph, 0);
+        cudaGraphDestroy(graph);
+        if (e != cudaSuccess) return cuda_fail(g, e, "cudaGraphInstantiate");
+        g->hg_g = g_host; g->hg_phi = phi_host; g->hg_out = out_host;
+        GX_CUDA(g, cudaGraphLaunch(g->host_graph, st));
+    }
     GX_CUDA(g, cudaStreamSynchronize(st));
+    if (std::getenv("GX_HOST_TRACE") && !use_graph) {      // development aid: stage completion times of this call
+        for (int b = 0; b < nb; ++b) {
+            float a = 0, c = 0, d = 0;
+            cudaEventElapsedTime(&a, e_start, e_in[b]);
+            cudaEventElapsedTime(&c, e_start, e_cmp[b]);
+            cudaEventElapsedTime(&d, e_start, e_out[b]);
+            std::fprintf(stderr, "gx host pipeline: block %d in %.0f us, computed %.0f us, out %.0f us\n", b, a * 1e3, c * 1e3, d * 1e3);
+        }
+    }
     return GX_OK;
 }
 

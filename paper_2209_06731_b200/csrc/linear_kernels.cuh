@@ -25,6 +25,7 @@ struct LinHostInput {
     double tau_fac, D_hyper, f_hyp;
     int n_hyper;
     bool linked = false;       // twist-and-shift linked z operators (Eq. 4.29) instead of periodic per mode
+    double damp_A = 0.0, damp_width = 0.125;   // wave-absorbing end layer, Eq. 4.30 (A = 0: off)
     std::vector<LinSpecies> species;
 };
 
@@ -42,6 +43,7 @@ struct LinTables {
     float* Az = nullptr;       // [Nz] circulant column of |gradpar| * spectral |k_z|
     float* omd = nullptr;      // [2][z][k]  omega_d^kappa, omega_d^gradB
     float* hypv = nullptr;     // [z][k] D (kperp2/kperp2max)^n
+    float* dend = nullptr;     // [z][k] end-damping profile d(z_hat) of Eq. 4.30 (nullptr: layer off)
     float* bgrad = nullptr;    // [z]
     float qn[kMaxSpecies] = {0}, zt[kMaxSpecies] = {0}, vt[kMaxSpecies] = {0}, tz[kMaxSpecies] = {0};
     float tprim[kMaxSpecies] = {0}, fprim[kMaxSpecies] = {0}, nu[kMaxSpecies] = {0}, nuhyp[kMaxSpecies] = {0};
@@ -68,7 +70,7 @@ constexpr int kLinLaunchesRhs = 3;
 
 inline void lin_tables_free(LinTables& t) {
     cudaFree(t.Jl); cudaFree(t.invD); cudaFree(t.fsfac); cudaFree(t.wz); cudaFree(t.bs);
-    cudaFree(t.Dz); cudaFree(t.Az); cudaFree(t.omd); cudaFree(t.hypv); cudaFree(t.bgrad);
+    cudaFree(t.Dz); cudaFree(t.Az); cudaFree(t.omd); cudaFree(t.hypv); cudaFree(t.dend); cudaFree(t.bgrad);
     cudaFree(t.mpow); cudaFree(t.mom);
     cudaFree(t.chain_off); cudaFree(t.chain_mode); cudaFree(t.ext_off); cudaFree(t.ext_d); cudaFree(t.ext_a); cudaFree(t.zwork);
     t = LinTables();
@@ -244,6 +246,40 @@ inline bool lin_tables_build(const LinHostInput& in, LinTables& t, size_t& bytes
             !lin_upload(&t.ext_off, eoff, bytes, msg) || !lin_upload(&t.ext_d, ed, bytes, msg) ||
             !lin_upload(&t.ext_a, ea, bytes, msg))
             return false;
+    }
+    // ---- wave-absorbing layer at the ends of every extended z domain, Eq. 4.30: d = A [1 - 2 zh^2/(1 + zh^4)]
+    // for |zh| < 1, zh = distance from either end / (damp_width * L_z), L_z = 2 pi L; ky = 0 untouched (reading L9)
+    if (t.dend) { cudaFree(t.dend); t.dend = nullptr; }
+    if (in.damp_A != 0.0) {
+        std::vector<float> dend((size_t)Nz * nk, 0.f);
+        const double jt = 2.0 * M_PI * in.shat * in.dky / in.dkx;
+        const int jtw = in.linked ? (int)std::lround(jt) : 0;
+        for (int q = 1; q < naky; ++q) {
+            const int step = jtw * q;
+            for (int pidx = -K; pidx <= K; ++pidx) {
+                std::vector<int> members;
+                if (step == 0) members.push_back(pidx);
+                else {
+                    if (std::abs(pidx - step) <= K) continue;
+                    for (int pp = pidx; std::abs(pp) <= K; pp += step) members.push_back(pp);
+                }
+                const int L = (int)members.size();
+                const double w = in.damp_width * 2.0 * M_PI * L, lo = -M_PI - 2.0 * M_PI * (L - 1), hi = M_PI;
+                for (int n = 0; n < L; ++n) {
+                    const int row = members[n] >= 0 ? members[n] : members[n] + nakx;
+                    for (int z = 0; z < Nz; ++z) {
+                        const double theta = -M_PI + 2.0 * M_PI * z / Nz - 2.0 * M_PI * n;
+                        double d = 0.0;
+                        for (double dist : {theta - lo, hi - theta}) {
+                            const double zh = dist / w;
+                            if (zh < 1.0) d += in.damp_A * (1.0 - 2.0 * zh * zh / (1.0 + zh * zh * zh * zh));
+                        }
+                        dend[((size_t)z * nakx + row) * naky + q] = (float)d;
+                    }
+                }
+            }
+        }
+        if (!lin_upload(&t.dend, dend, bytes, msg)) return false;
     }
     if (!lin_upload(&t.Jl, Jl, bytes, msg) || !lin_upload(&t.bs, bs, bytes, msg) ||
         !lin_upload(&t.invD, invD, bytes, msg) || !lin_upload(&t.fsfac, fsfac, bytes, msg) ||
@@ -541,6 +577,12 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
             r.x -= hv * gg.x;
             r.y -= hv * gg.y;
         }
+        // wave-absorbing end layer (Eq. 4.30): - d(z_hat) H_{l,m}, non-zonal modes
+        if (t.dend) {
+            const float dd = t.dend[(size_t)z * t.nk + k];
+            r.x -= dd * h00.x;
+            r.y -= dd * h00.y;
+        }
         }
         float2* __restrict__ o = out + ((unsigned)((s * t.Nm + m) * t.Nl + l) * (unsigned)(t.Nz * t.nk) + (unsigned)(z * t.nk + k));
         if (ACC || DERIV_ONLY) { const float2 prev = *o; r.x += prev.x; r.y += prev.y; }
@@ -600,6 +642,7 @@ __global__ void __launch_bounds__(256) lin_point_kernel(LinTables t, const float
     const float bg = -vt * t.bgrad[z];
     const float wk = tz * t.omd[zk], wb = tz * t.omd[pl + zk];
     const float hv = t.hypv[zk];
+    const float dd = t.dend ? t.dend[zk] : 0.f;
     const float ky = t.dky * (float)(k % t.naky);
     const float b = t.bs[(unsigned)s * pl + zk];
     const float sb = sqrtf(fmaxf(b, 0.f));
@@ -651,6 +694,9 @@ __global__ void __launch_bounds__(256) lin_point_kernel(LinTables t, const float
             // hyper-viscosity
             r.x -= hv * graw[l].x;
             r.y -= hv * graw[l].y;
+            // wave-absorbing end layer (Eq. 4.30)
+            r.x -= dd * c0.x;
+            r.y -= dd * c0.y;
             float2* __restrict__ o = out + ((unsigned)((s * t.Nm + m) * t.Nl + l) * pl + zk);
             if (ACC) { const float2 prev = *o; r.x += prev.x; r.y += prev.y; }
             *o = r;

@@ -454,3 +454,57 @@ def test_linked_rhs_differs_only_through_the_z_operators():
     assert np.allclose(L.linear_rhs(G, Phi, boundary="linked", terms=local, **kw),
                        L.linear_rhs(G, Phi, boundary="periodic", terms=local, **kw), atol=0)
     assert np.allclose(a[..., 0], b[..., 0], atol=1e-12) and not np.allclose(a[..., 1:], b[..., 1:], atol=1e-3)
+
+
+# ---------------------------------------------------------------------------- end-damping layer (Eq. 4.30)
+def test_end_damping_profile_hand_values_and_structure():
+    """d(zh) = A [1 - 2 zh^2/(1 + zh^4)], |zh| < 1, distance from either end of the extended domain in units of
+    L_z/8; ky = 0 untouched.  Periodic domains (L = 1), Nz = 16: z_width = 2 pi/8 = two grid steps."""
+    A, Nz = 0.7, 16
+    d = L.end_damping_profile(Nz, NX, NY, A, 0.125, "periodic")
+    f = lambda zh: A * (1 - 2 * zh ** 2 / (1 + zh ** 4))
+    expect = np.zeros(Nz)
+    expect[0] = f(0.0)             # z_0 = -pi is the lower end itself: d = A
+    expect[1] = f(0.5)             # one step = half a width from the lower end: A (1 - 0.5/1.0625)
+    expect[15] = f(0.5)            # one step below the upper end (theta = pi is not a grid point)
+    assert abs(f(0.5) - A * (1 - 0.5 / 1.0625)) < 1e-15 and abs(f(1.0)) < 1e-15
+    for i in range(NAKX):
+        for q in range(1, NAKY):
+            assert np.allclose(d[:, i, q], expect, atol=1e-15)
+    assert np.all(d[:, :, 0] == 0)                     # zonal modes are not filtered (P:335)
+    # linked domains: only the two end segments of a chain are damped, symmetrically, and the width grows with L
+    jt = 2
+    dl = L.end_damping_profile(Nz, NX, NY, A, 0.125, "linked", jt)
+    z = -math.pi + 2 * math.pi * np.arange(Nz) / Nz
+    for q, rows in L.twist_shift_chains(NX, NY, jt):
+        if q == 0:
+            continue
+        Lc = len(rows)
+        theta = np.concatenate([z - 2 * math.pi * n for n in range(Lc - 1, -1, -1)])       # increasing ballooning angle
+        prof = np.concatenate([dl[:, rows[n], q] for n in range(Lc - 1, -1, -1)])
+        lo, hi, w = -math.pi - 2 * math.pi * (Lc - 1), math.pi, 2 * math.pi * Lc / 8
+        ref = np.where(theta - lo < w, f((theta - lo) / w), 0.0) + np.where(hi - theta < w, f((hi - theta) / w), 0.0)
+        assert np.allclose(prof, ref, atol=1e-14)
+        assert np.all(prof >= 0) and prof[0] == A and np.all(prof[(theta - lo >= w) & (hi - theta >= w)] == 0)
+        # reflection symmetry about the middle of the extended domain (the end point theta_hi is off-grid by one step)
+        assert np.allclose(prof[1:], prof[1:][::-1], atol=1e-14)
+
+
+def test_end_damping_acts_on_H_for_nonzonal_modes_only():
+    Nz = 8
+    geo, z = _geo(Nz)
+    sp = dict(Z=2.0, mass=1.0, temp=0.5, dens=1.0, tprim=0, fprim=0, nu_ss=0)
+    G = _rand((1, 3, 2, Nz, NAKX, NAKY), 53)
+    Phi = _rand((Nz, NAKX, NAKY), 54)
+    dmp = dict(A=0.3, width_frac=0.25)
+    r = L.linear_rhs(G, Phi, NX, NY, DKX, DKY, SHAT, geo, [sp], terms=(), damping=dmp)
+    d = L.end_damping_profile(Nz, NX, NY, 0.3, 0.25)
+    kx, ky = DKX * O.kx_index(NX), DKY * O.ky_index(NY)
+    b = O.kperp2(kx, ky, geo["gds2"], geo["gds21"], geo["gds22"], SHAT) * (0.5 * 1.0 / 4.0) / geo["bmag"][:, None, None] ** 2
+    for l in range(2):
+        Jl = (-b / 2) ** l / math.factorial(l) * np.exp(-b / 2)
+        assert np.allclose(r[0, 0, l], -d * (G[0, 0, l] + (2.0 / 0.5) * Jl * Phi), atol=1e-13)     # m = 0: H = G + (Z/tau) J_l Phi
+        assert np.allclose(r[0, 2, l], -d * G[0, 2, l], atol=1e-13)
+    assert np.all(r[..., 0] == 0) and np.max(np.abs(r[..., 1:])) > 0.01
+    # without the option nothing changes
+    assert np.all(L.linear_rhs(G, Phi, NX, NY, DKX, DKY, SHAT, geo, [sp], terms=()) == 0)

@@ -236,9 +236,12 @@ def test_zero_input_and_error_paths(torch_cuda):
     B.gx_grid_destroy(h)
 
 
-def test_host_entry_point_matches_device_entry_point(torch_cuda):
+@pytest.mark.parametrize("name", ["tiny", "kinetic"])
+def test_host_entry_point_matches_device_entry_point(torch_cuda, name):
+    """gx_nonlinear_rhs_host pipelines Hermite blocks over three streams (two species: strided block copies);
+    the result must be bit-identical to the one-shot device call, also when called twice in a row."""
     torch = torch_cuda
-    cfg = I.named_config("tiny")
+    cfg = I.named_config(name)
     geo = I.geometry_arrays(cfg)
     G = I.make_state(cfg, geo)
     Phi = _oracle_phi(cfg, geo, G)
@@ -248,6 +251,10 @@ def test_host_entry_point_matches_device_entry_point(torch_cuda):
     oh = torch.empty_like(gh).pin_memory()
     grid.nonlinear_rhs_host(gh, ph, oh)
     assert np.array_equal(oh.numpy(), out_dev)
+    oh.zero_()
+    grid.nonlinear_rhs_host(gh, ph, oh)
+    assert np.array_equal(oh.numpy(), out_dev)
+    assert np.array_equal(_gpu_nl(torch, grid, G, Phi), out_dev)      # and the device entry point still works after it
     grid.close()
 
 
@@ -506,3 +513,31 @@ def test_linked_boundary_needs_a_quantised_box(torch_cuda):
                           geo["cvdrift"], geo["cvdrift0"], geo["bgrad"], geo["jacobian"], geo["gradpar"])
     assert e.value.code == B.GX_ERR_ARG
     B.gx_grid_destroy(h)
+
+
+@pytest.mark.parametrize("name,linked", [("tiny", False), ("tiny", True), ("cyclone", True), ("hires", False)])
+def test_linear_rhs_parity_with_end_damping(torch_cuda, name, linked):
+    """Eq. 4.30: the wave-absorbing end layer on periodic and on linked extended domains
+    (split pointwise kernel for Nl <= 4, generic kernel for hires with Nl = 8)."""
+    torch = torch_cuda
+    from paper_2209_06731_b200 import binding
+    cfg = I.named_config(name)
+    if name == "hires":
+        cfg = I.Config(cfg.name, cfg.Nx, cfg.Ny, 8, cfg.Nl, 4, cfg.species, decay=cfg.decay, seed=cfg.seed)
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    dmp = dict(A=0.8, width_frac=0.125)
+    grid = binding.Grid(cfg, geo, linked=linked, damping=dmp)
+    g, phi = torch.from_numpy(G).cuda(), torch.from_numpy(Phi).cuda()
+    out = torch.full_like(g, float("nan"))
+    grid.linear_rhs(g, phi, out)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    bc = "linked" if linked else "periodic"
+    ref = OL.linear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, boundary=bc, damping=dmp)
+    off = OL.linear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, boundary=bc)
+    assert np.all(np.isfinite(out))
+    assert O.relative_max_error(out, ref) <= TOL
+    assert O.relative_max_error(off, ref) > 20 * TOL           # the layer is visible at this tolerance
+    grid.close()
