@@ -417,6 +417,137 @@ def test_series_gyroaverage_variant_within_truncation_bound(tiny):
     assert np.all(np.abs(exact - series) <= tail + 1e-13)
     assert np.max(np.abs(exact - series)) > 1e-4          # and the bound is not vacuous
 
+# ------------------------------------------------------------------ electromagnetic brackets (row f4)
+def test_em_gyro_tables_project_to_the_paper_printed_coefficients():
+    """Eq. 4.6: the Laguerre projections of the three gyroaveraged potentials of Eq. 4.5 are J_l (Phi),
+    J_l (A_par) and J_l + J_{l-1} (dB_par/B): int psi_l(t) [2 t J1(sqrt(2tb))/sqrt(2tb)] e^-t dt = J_l + J_{l-1}.
+    Library Gauss-Laguerre nodes (numpy), closed form of Eq. 4.7 typed here."""
+    xr, wr = np.polynomial.laguerre.laggauss(60)
+    for b in (0.0, 0.3, 1.7):
+        bb = np.full((1, 1, 1), b)
+        MB = O.gyro_table_bpar(bb, xr)[0, :, 0, 0]
+        M0 = O.gyro_table(bb, xr)[0, :, 0, 0]
+        for l in range(5):
+            lag = (-1.0) ** l * special.eval_laguerre(l, xr)
+            jl = _jflr_by_hand(l, b)
+            jlm = _jflr_by_hand(l - 1, b) if l > 0 else 0.0
+            assert abs(np.sum(wr * lag * MB) - (jl + jlm)) < 1e-10, (b, l)
+            assert abs(np.sum(wr * lag * M0) - jl) < 1e-10, (b, l)
+    # zero Larmor radius: 2 x J1(alpha)/alpha -> x (the factor mu B itself)
+    assert np.allclose(O.gyro_table_bpar(np.zeros((1, 1, 1)), xr)[0, :, 0, 0], xr)
+    assert np.allclose(O.gyro_table_bpar(np.full((1, 1, 1), 1e-20), xr)[0, :, 0, 0], xr)
+
+
+def test_em_reduces_to_electrostatic_term(tiny):
+    cfg, geo, G, Phi = tiny
+    zero = np.zeros_like(Phi)
+    a = O.nonlinear_rhs_em(G, Phi, zero, zero, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species)
+    assert O.relative_max_error(a, _nl(cfg, geo, G, Phi)) < 1e-14
+
+
+@pytest.mark.parametrize("method", ["conv_np", "dft"])
+def test_em_single_mode_closed_forms_at_finite_b(method):
+    """One Fourier mode p in A_par (then in dB_par/B), G non-zero only in l' = 0 and one mode q, J = 40 nodes:
+        A_par:  N_{l,m} = -v_ts L_l F{J0 A, sqrt(m+1) gt_{m+1} + sqrt(m) gt_{m-1}}  =>  with G only at m = 1:
+                out[l, m=0] = +v_ts J_l(b_p) X A_p g_q,  out[l, m=2] = +v_ts sqrt(2) J_l(b_p) X A_p g_q,  out[l, m=1] = 0
+        dB_par: out[l, m] = -(tau/Z) (J_l + J_{l-1})(b_p) X B_p g_q                      (Eq. 4.6 coefficient)
+    with X = p_x q_y - p_y q_x at k = p+q (and the mirrored coefficient at q-p), b_p by hand from P:85."""
+    Nx = Ny = 16
+    nakx, naky = O.dealiased_counts(Nx, Ny)
+    Nz, Nl, Nm = 2, 3, 3
+    dkx, dky, shat = 0.9, 0.7, 0.8
+    geo = dict(bmag=np.array([1.0, 1.6]), gds2=np.array([1.3, 0.9]), gds21=np.array([0.2, -0.4]), gds22=np.array([0.64, 1.1]))
+    Zs, ms, ts = -2.0, 3.0, 0.5
+    vt = math.sqrt(ts / ms)
+    sp = [dict(Z=Zs, mass=ms, temp=ts, dens=1.0)]
+    (pa, pb), (qa, qb) = (2, 1), (-1, 3)
+    fp = np.array([0.8 - 0.3j, -0.2 + 0.9j])
+    gq = np.array([-0.5 + 1.1j, 0.3 - 0.7j])
+    field = np.zeros((Nz, nakx, naky), complex)
+    G = np.zeros((1, Nm, Nl, Nz, nakx, naky), complex)
+    for z in range(Nz):
+        field[z] = _single_mode(nakx, naky, pa, pb, fp[z])
+        G[0, 1, 0, z] = _single_mode(nakx, naky, qa, qb, gq[z])
+    zero = np.zeros_like(field)
+    px, py, qx, qy = dkx * pa, dky * pb, dkx * qa, dky * qb
+    cross = px * qy - py * qx
+    i_sum, i_dif = (pa + qa) % nakx, (qa - pa) % nakx
+    bs = [(py * py * geo["gds2"][z] + 2 * px * py * geo["gds21"][z] / shat + px * px * geo["gds22"][z] / shat ** 2)
+          * ts * ms / (Zs ** 2 * geo["bmag"][z] ** 2) for z in range(Nz)]
+    kw = dict(method=method, J=40)
+    outA = O.nonlinear_rhs_em(G, zero, field, zero, Nx, Ny, dkx, dky, shat, geo, sp, **kw)
+    outB = O.nonlinear_rhs_em(G, zero, zero, field, Nx, Ny, dkx, dky, shat, geo, sp, **kw)
+    expA, expB = np.zeros_like(outA), np.zeros_like(outB)
+    for z in range(Nz):
+        for l in range(Nl):
+            jl = _jflr_by_hand(l, bs[z])
+            jb = jl + (_jflr_by_hand(l - 1, bs[z]) if l > 0 else 0.0)
+            for m, c in [(0, 1.0), (2, math.sqrt(2.0))]:
+                expA[0, m, l, z, i_sum, pb + qb] = +vt * c * jl * cross * fp[z] * gq[z]
+                expA[0, m, l, z, i_dif, qb - pb] = -vt * c * jl * cross * np.conj(fp[z]) * gq[z]
+            expB[0, 1, l, z, i_sum, pb + qb] = -(ts / Zs) * jb * cross * fp[z] * gq[z]
+            expB[0, 1, l, z, i_dif, qb - pb] = +(ts / Zs) * jb * cross * np.conj(fp[z]) * gq[z]
+    assert np.max(np.abs(outA - expA)) < 1e-9 * np.max(np.abs(expA))
+    assert np.max(np.abs(outB - expB)) < 1e-9 * np.max(np.abs(expB))
+    assert np.all(outA[0, 1] == 0)
+
+
+def test_em_apar_coupling_is_the_hermite_matrix_of_v_par(tiny):
+    """At zero Larmor radius the A_par bracket is out_m = +v_ts sum_m' <phi_m| v_par |phi_m'> C[A_par, G_m'] per l:
+    matrix elements by library Gauss-Hermite quadrature (the recurrence v phi_m = sqrt(m+1) phi_{m+1} + sqrt(m) phi_{m-1})."""
+    from numpy.polynomial import hermite_e as HE
+    cfg, geo, G, Phi = tiny
+    cold = [dict(Z=1.0, mass=1e-30, temp=4e-30, dens=1.0)]           # b = 0, v_ts = 2
+    A = I.random_phi(cfg, geo, seed_offset=31)
+    zero = np.zeros_like(A)
+    out = O.nonlinear_rhs_em(G, zero, A, zero, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cold, planes=[(0, m, 3) for m in range(cfg.Nm)])
+    xh, wh = HE.hermegauss(40)
+    wh = wh / math.sqrt(2 * math.pi)
+    phi_m = lambda m: HE.hermeval(xh, np.eye(m + 1)[m]) / math.sqrt(math.factorial(m))
+    X = np.array([[np.sum(wh * phi_m(a) * xh * phi_m(c)) for c in range(cfg.Nm)] for a in range(cfg.Nm)])
+    for l in range(cfg.Nl):
+        C = [O.bracket_convolution_c(A[3].astype(np.complex128), G[0, m, l, 3].astype(np.complex128), cfg.dkx, cfg.dky)
+             for m in range(cfg.Nm)]
+        for m in range(cfg.Nm):
+            ref = 2.0 * sum(X[m, mp] * C[mp] for mp in range(cfg.Nm))
+            assert np.max(np.abs(out[0, m, l, 3] - ref)) < 1e-12 * np.max(np.abs(ref))
+
+
+def test_em_field_solve_satisfies_the_field_equations_in_H():
+    """Eq. 4.20-4.22 with H rebuilt from Eq. 4.8, J_l typed here, two kinetic species, B != 1."""
+    cfg = I.named_config("kinetic")
+    small = I.Config("k2", 16, 16, 3, 3, 3, cfg.species, seed=9)
+    geo = I.geometry_arrays(small)
+    G = I.make_state(small, geo).astype(np.complex128)
+    beta = 0.02
+    Phi, Apar, Bpar = O.field_solve_em(G, beta, 16, 16, small.dkx, small.dky, small.shat, geo, small.species)
+    kx, ky = small.dkx * O.kx_index(16), small.dky * O.ky_index(16)
+    zz = geo["z"][:, None, None]
+    kp2 = (kx[None, :, None] - small.shat * zz * ky[None, None, :]) ** 2 + ky[None, None, :] ** 2
+    bm2 = geo["bmag"][:, None, None] ** 2
+    lhs_q, rhs_q, rhs_a, rhs_b = 0, 0, 0, 0
+    for s, sp in enumerate(small.species):
+        b = kp2 * sp.temp * sp.mass / (sp.Z ** 2 * bm2)
+        Jl = [(-b / 2) ** l / math.factorial(l) * np.exp(-b / 2) for l in range(3)]
+        Jb = [Jl[l] + (Jl[l - 1] if l else 0) for l in range(3)]
+        vt = math.sqrt(sp.temp / sp.mass)
+        H0 = [G[s, 0, l] + (sp.Z / sp.temp) * Jl[l] * Phi + Jb[l] * Bpar for l in range(3)]
+        H1 = [G[s, 1, l] - (sp.Z * vt / sp.temp) * Jl[l] * Apar for l in range(3)]
+        lhs_q = lhs_q + sp.Z ** 2 * sp.dens / sp.temp * Phi
+        rhs_q = rhs_q + sp.Z * sp.dens * sum(Jl[l] * H0[l] for l in range(3))
+        rhs_a = rhs_a + 0.5 * beta * sp.Z * sp.dens * vt * sum(Jl[l] * H1[l] for l in range(3))
+        rhs_b = rhs_b - 0.5 * beta / bm2 * sp.dens * sp.temp * sum(Jb[l] * H0[l] for l in range(3))
+    for res, scale in [(lhs_q - rhs_q, rhs_q), (kp2 * Apar - rhs_a, rhs_a), (Bpar - rhs_b, rhs_b)]:
+        res = res.copy()
+        res[:, 0, 0] = 0
+        assert np.max(np.abs(res)) < 1e-11 * np.max(np.abs(scale))
+    assert np.max(np.abs(Apar)) > 0 and np.max(np.abs(Bpar)) > 0
+    # beta -> 0: electrostatic two-species solve
+    P0, A0, B0 = O.field_solve_em(G, 0.0, 16, 16, small.dkx, small.dky, small.shat, geo, small.species)
+    assert np.all(A0 == 0) and np.all(B0 == 0)
+    assert np.allclose(P0, O.field_solve(G, 16, 16, small.dkx, small.dky, small.shat, geo, small.species, adiabatic=False), atol=1e-13)
+
+
 # ------------------------------------------------------------------ field solve
 def test_field_solve_satisfies_eq_6_1(tiny):
     cfg, geo, G, _ = tiny
