@@ -117,6 +117,21 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
 int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev,
                      void* cuda_stream);
 
+/* Electromagnetic form of the hot path (App. D Eq. D1 lines 1-4, with Eq. 4.5):
+ *   out = -N,  N_{l,m} = L_l F[ {J0 Phi + (tau/Z) 2 muB (J1/alpha) dB_par/B, gt_m} - v_ts {J0 A_par, sqrt(m+1) gt_{m+1} + sqrt(m) gt_{m-1}} ]
+ * apar_dev, bpar_dev: device fields A_par and dB_par/B in the layout of phi.  Evaluated as two passes of the
+ * electrostatic kernels (potential planes built in spectral space, Hermite-shifted state for the A_par pass) whose
+ * results are added; needs the full geometry (gx_geometry_set with all arrays); two state-sized work buffers are
+ * allocated on first use.  apar = bpar = 0 reproduces gx_nonlinear_rhs. */
+int gx_nonlinear_rhs_em(gx_grid* g, const void* g_dev, const void* phi_dev, const void* apar_dev, const void* bpar_dev,
+                        void* out_dev, void* cuda_stream);
+
+/* Field solve with electromagnetic fluctuations, Eq. 4.23-4.25, kinetic species only (no adiabatic
+ * closure), beta = beta_ref >= 0: per (z,k) the 2x2 system for (Phi, dB_par/B) and the parallel Ampere law for A_par;
+ * sums over l truncated at Nl; all three fields vanish at kx = ky = 0.  beta = 0 gives the two-species gx_field_solve. */
+int gx_field_solve_em(gx_grid* g, const void* g_dev, double beta, void* phi_dev, void* apar_dev, void* bpar_dev,
+                      void* cuda_stream);
+
 /* Same call with HOST buffers (pinned for full speed).  The evaluation is diagonal in the Hermite index, so it
  * is pipelined over blocks of moments on three streams: the host-to-device copy of block b+1 and the
  * device-to-host copy of block b-1 overlap the kernels of block b (chi planes computed once).  Ordered after

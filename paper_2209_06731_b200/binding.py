@@ -21,7 +21,7 @@ GX_OK, GX_ERR_ARG, GX_ERR_STATE, GX_ERR_UNSUPPORTED, GX_ERR_CUDA, GX_ERR_ALLOC =
 FAMILY_NAMES = {0: "scalar", 3: "row", 5: "rx", 6: "rxp", 7: "rxw"}
 
 EXPORTED = ["gx_grid_create", "gx_grid_destroy", "gx_box_set", "gx_species_set", "gx_adiabatic_set",
-            "gx_dissipation_set", "gx_boundary_set", "gx_damping_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_host",
+            "gx_dissipation_set", "gx_boundary_set", "gx_damping_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_em", "gx_field_solve_em", "gx_nonlinear_rhs_host",
             "gx_field_solve", "gx_rhs", "gx_linear_rhs", "gx_ssprk3_step", "gx_query", "gx_export_maps",
             "gx_export_tables", "gx_profile_set", "gx_profile_get", "gx_last_error", "gx_ubench_fp32"]
 
@@ -55,6 +55,8 @@ def load():
     lib.gx_geometry_set.argtypes = [vp] + [dp] * 10 + [d]
     lib.gx_nonlinear_rhs.argtypes = [vp, vp, vp, vp, vp]
     lib.gx_nonlinear_rhs_host.argtypes = [vp, vp, vp, vp, vp]
+    lib.gx_nonlinear_rhs_em.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+    lib.gx_field_solve_em.argtypes = [vp, vp, d, vp, vp, vp, vp]
     lib.gx_field_solve.argtypes = [vp, vp, vp, vp]
     lib.gx_rhs.argtypes = [vp, vp, vp, vp]
     lib.gx_linear_rhs.argtypes = [vp, vp, vp, vp, vp]
@@ -132,6 +134,14 @@ def gx_geometry_set(h, bmag, gds2, gds21, gds22, gbdrift=None, gbdrift0=None, cv
 
 def gx_nonlinear_rhs(h, g_ptr, phi_ptr, out_ptr, stream=0):
     _check(h, load().gx_nonlinear_rhs(h, g_ptr, phi_ptr, out_ptr, stream))
+
+
+def gx_nonlinear_rhs_em(h, g_ptr, phi_ptr, apar_ptr, bpar_ptr, out_ptr, stream=0):
+    _check(h, load().gx_nonlinear_rhs_em(h, g_ptr, phi_ptr, apar_ptr, bpar_ptr, out_ptr, stream))
+
+
+def gx_field_solve_em(h, g_ptr, beta, phi_ptr, apar_ptr, bpar_ptr, stream=0):
+    _check(h, load().gx_field_solve_em(h, g_ptr, float(beta), phi_ptr, apar_ptr, bpar_ptr, stream))
 
 
 def gx_nonlinear_rhs_host(h, g_ptr, phi_ptr, out_ptr, stream=0):
@@ -255,6 +265,16 @@ class Grid:
     def nonlinear_rhs(self, g, phi, out):
         gx_nonlinear_rhs(self.h, self._chk(g, "g"), self._chk(phi, "phi"), self._chk(out, "g"), self._stream())
         return out
+
+    def nonlinear_rhs_em(self, g, phi, apar, bpar, out):
+        gx_nonlinear_rhs_em(self.h, self._chk(g, "g"), self._chk(phi, "phi"), self._chk(apar, "phi"), self._chk(bpar, "phi"),
+                            self._chk(out, "g"), self._stream())
+        return out
+
+    def field_solve_em(self, g, beta, phi, apar, bpar):
+        gx_field_solve_em(self.h, self._chk(g, "g"), beta, self._chk(phi, "phi"), self._chk(apar, "phi"), self._chk(bpar, "phi"),
+                          self._stream())
+        return phi, apar, bpar
 
     def nonlinear_rhs_host(self, g_host, phi_host, out_host):
         gx_nonlinear_rhs_host(self.h, self._chk(g_host, "g", True), self._chk(phi_host, "phi", True),

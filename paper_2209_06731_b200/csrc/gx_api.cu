@@ -114,6 +114,10 @@ struct gx_grid {
     const KernelSet* ks = nullptr;
     // device
     float *dT = nullptr, *dTinv = nullptr, *dM = nullptr;
+    // electromagnetic brackets (gx_nonlinear_rhs_em): (tau/Z) 2 x_j J1(alpha)/alpha table, shared plane of ones, kperp2 and
+    // bmag^2 on the device, spectral chi planes, Hermite-shifted state and second result (allocated on first use)
+    float *dMB = nullptr, *dones = nullptr, *dkp2 = nullptr, *dbmag2 = nullptr;
+    float2 *dchis = nullptr, *dg_em = nullptr, *dout_em = nullptr;
     float2 *dtwx = nullptr, *dtwy = nullptr, *ddchi = nullptr, *dbhat = nullptr;
     unsigned* dcount = nullptr;
     unsigned* dchi_flag = nullptr;              // [s][z][j] epoch of the last call that produced the chi plane (persistent family)
@@ -273,7 +277,8 @@ int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out
 
 int gx_grid_destroy(gx_grid* g) {
     if (!g) return GX_ERR_ARG;
-    cudaFree(g->dT); cudaFree(g->dTinv); cudaFree(g->dM); cudaFree(g->dtwx); cudaFree(g->dtwy);
+    cudaFree(g->dT); cudaFree(g->dTinv); cudaFree(g->dM); cudaFree(g->dMB); cudaFree(g->dones); cudaFree(g->dkp2);
+    cudaFree(g->dbmag2); cudaFree(g->dchis); cudaFree(g->dg_em); cudaFree(g->dout_em); cudaFree(g->dtwx); cudaFree(g->dtwy);
     cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dcount); cudaFree(g->dchi_flag); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
     cudaFree(g->dphi_rhs); cudaFree(g->drk_y); cudaFree(g->drk_k);
     for (auto e : g->ev_pool) cudaEventDestroy(e);
@@ -395,6 +400,38 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
         }
     }
     GX_CUDA(g, cudaMemcpy(g->dM, M.data(), M.size() * sizeof(float), cudaMemcpyHostToDevice));
+    {   // electromagnetic tables (row f4): MB[s][z][j][k] = (tau/Z) 2 x_j J1(alpha)/alpha (Eq. 4.5), kperp2, bmag^2
+        std::vector<float> MB(M.size()), kf(kp2.size()), b2(Nz);
+        for (int s = 0; s < g->Ns; ++s) {
+            const Species& sp = g->sp[s];
+            const double rho2 = sp.temp * sp.mass / (sp.Z * sp.Z), tz = sp.temp / sp.Z;
+            for (int z = 0; z < Nz; ++z)
+                for (int j = 0; j < J; ++j) {
+                    float* Mp = MB.data() + (((size_t)s * Nz + z) * J + j) * g->nk;
+                    const double* kp = kp2.data() + (size_t)z * g->nk;
+                    for (long long k = 0; k < g->nk; ++k) {
+                        const double b = std::max(0.0, kp[k] * rho2 / (bmag[z] * bmag[z]));
+                        const double a = std::sqrt(2.0 * g->xj[j] * b);
+                        const double r = a > 1e-8 ? ::j1(a) / a : 0.5 - a * a / 16.0;
+                        Mp[k] = (float)(tz * 2.0 * g->xj[j] * r);
+                    }
+                }
+        }
+        for (size_t i = 0; i < kp2.size(); ++i) kf[i] = (float)kp2[i];
+        for (int z = 0; z < Nz; ++z) b2[z] = (float)(bmag[z] * bmag[z]);
+        int rc;
+        if (!g->dMB) {
+            if ((rc = dev_alloc(g, &g->dMB, MB.size()))) return rc;
+            if ((rc = dev_alloc(g, &g->dkp2, kf.size()))) return rc;
+            if ((rc = dev_alloc(g, &g->dbmag2, b2.size()))) return rc;
+            if ((rc = dev_alloc(g, &g->dones, (size_t)g->nk))) return rc;
+            std::vector<float> ones((size_t)g->nk, 1.f);
+            GX_CUDA(g, cudaMemcpy(g->dones, ones.data(), ones.size() * sizeof(float), cudaMemcpyHostToDevice));
+        }
+        GX_CUDA(g, cudaMemcpy(g->dMB, MB.data(), MB.size() * sizeof(float), cudaMemcpyHostToDevice));
+        GX_CUDA(g, cudaMemcpy(g->dkp2, kf.data(), kf.size() * sizeof(float), cudaMemcpyHostToDevice));
+        GX_CUDA(g, cudaMemcpy(g->dbmag2, b2.data(), b2.size() * sizeof(float), cudaMemcpyHostToDevice));
+    }
 
     if (g->have_lin_geo) {
         gx::LinHostInput in;
@@ -498,6 +535,66 @@ int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* o
         GX_CUDA(g, cudaEventRecord(ev[0], st));
     }
     return nl_enqueue(g, p, g->Nm, true, g->dcount, &g->calls, st, ev);
+}
+
+int gx_nonlinear_rhs_em(gx_grid* g, const void* g_dev, const void* phi_dev, const void* apar_dev, const void* bpar_dev,
+                        void* out_dev, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_dev || !phi_dev || !apar_dev || !bpar_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs_em: null pointer");
+    const size_t ng = (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk;
+    if (overlap(g_dev, out_dev, ng * sizeof(float2))) return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs_em: out must not alias g");
+    if (misaligned(g_dev) || misaligned(phi_dev) || misaligned(apar_dev) || misaligned(bpar_dev) || misaligned(out_dev))
+        return fail(g, GX_ERR_ARG, "gx_nonlinear_rhs_em: device pointers must be 16-byte aligned");
+    if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
+    if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_nonlinear_rhs_em: full geometry not set");
+    if (ng % 2) return fail(g, GX_ERR_UNSUPPORTED, "gx_nonlinear_rhs_em: odd number of coefficients");
+    const size_t szj = (size_t)g->Ns * g->Nz * g->J;
+    int rc;
+    if (!g->dchis) {
+        if ((rc = dev_alloc(g, &g->dchis, szj * g->nk))) return rc;
+        if ((rc = dev_alloc(g, &g->dg_em, ng))) return rc;
+        if ((rc = dev_alloc(g, &g->dout_em, ng))) return rc;
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const dim3 cgrid((unsigned)((g->nk + 255) / 256), (unsigned)szj);
+    // out = -L F{ J0 Phi + (tau/Z) 2 muB (J1/alpha) dB_par/B , gt_m }            (D1 lines 1 and 4)
+    gx::em_chi_spectral_kernel<<<cgrid, 256, 0, st>>>(g->dM, g->dMB, (const float2*)phi_dev, (const float2*)bpar_dev, g->dchis,
+                                                      (int)g->nk, g->Nz, g->J);
+    NlParams p = make_params(g, g_dev, g->dchis, out_dev);
+    p.M = g->dones; p.phi_by_unit = 1; p.M_shared = 1;
+    if ((rc = nl_enqueue(g, p, g->Nm, true, g->dcount, &g->calls, st, nullptr))) return rc;
+    // out += -L F{ J0 A_par , gt2_m },  G2_{l,m} = -v_ts ( sqrt(m+1) G_{l,m+1} + sqrt(m) G_{l,m-1} )   (D1 lines 2-3)
+    gx::em_chi_spectral_kernel<<<cgrid, 256, 0, st>>>(g->dM, nullptr, (const float2*)apar_dev, nullptr, g->dchis, (int)g->nk, g->Nz, g->J);
+    {
+        const unsigned pl = (unsigned)((size_t)g->Nl * g->Nz * g->nk);
+        gx::em_hermite_shift_kernel<<<dim3((pl + 255) / 256, (unsigned)(g->Ns * g->Nm)), 256, 0, st>>>(g->lin, (const float2*)g_dev, g->dg_em);
+    }
+    p = make_params(g, g->dg_em, g->dchis, g->dout_em);
+    p.M = g->dones; p.phi_by_unit = 1; p.M_shared = 1;
+    if ((rc = nl_enqueue(g, p, g->Nm, true, g->dcount, &g->calls, st, nullptr))) return rc;
+    gx::em_add_kernel<<<(unsigned)((ng / 2 + 255) / 256), 256, 0, st>>>((float4*)out_dev, (const float4*)g->dout_em, ng / 2);
+    GX_CUDA(g, cudaGetLastError());
+    return GX_OK;
+}
+
+int gx_field_solve_em(gx_grid* g, const void* g_dev, double beta, void* phi_dev, void* apar_dev, void* bpar_dev, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_dev || !phi_dev || !apar_dev || !bpar_dev || beta < 0) return fail(g, GX_ERR_ARG, "gx_field_solve_em: null pointer or beta < 0");
+    if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_field_solve_em: full geometry not set");
+    gx::EmSpecies e{};
+    for (int s = 0; s < g->Ns; ++s) {
+        const Species& sp = g->sp[s];
+        e.qn[s] = (float)(sp.Z * sp.dens);
+        e.z2nt[s] = (float)(sp.Z * sp.Z * sp.dens / sp.temp);
+        e.nt[s] = (float)(sp.dens * sp.temp);
+        e.z2nm[s] = (float)(sp.Z * sp.Z * sp.dens / sp.mass);
+        e.qnv[s] = (float)(sp.Z * sp.dens * std::sqrt(sp.temp / sp.mass));
+    }
+    dim3 grid((unsigned)((g->nk + 255) / 256), (unsigned)g->Nz);
+    gx::field_solve_em_kernel<<<grid, 256, 0, (cudaStream_t)cuda_stream>>>(g->lin, e, g->dkp2, g->dbmag2, (float)beta, (const float2*)g_dev,
+                                                                           (float2*)phi_dev, (float2*)apar_dev, (float2*)bpar_dev);
+    GX_CUDA(g, cudaGetLastError());
+    return GX_OK;
 }
 
 int gx_profile_set(gx_grid* g, int enabled) {

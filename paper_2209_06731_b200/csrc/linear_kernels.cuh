@@ -347,6 +347,91 @@ inline cudaError_t lin_field_solve(const LinTables& t, const float2* g, float2* 
 }
 
 // ------------------------------------------------------------------------------------------------
+// Electromagnetic field solve, Eq. 4.23-4.25: per (z,k) a 2x2 system for (Phi, dB_par/B)
+// and the decoupled parallel Ampere law for A_par; kinetic species only; fields vanish at kx = ky = 0.
+struct EmSpecies { float qn[kMaxSpecies], z2nt[kMaxSpecies], nt[kMaxSpecies], z2nm[kMaxSpecies], qnv[kMaxSpecies]; };
+__global__ void __launch_bounds__(256) field_solve_em_kernel(LinTables t, EmSpecies e, const float* __restrict__ kp2,
+                                                             const float* __restrict__ bmag2, float beta,
+                                                             const float2* __restrict__ g, float2* __restrict__ phi,
+                                                             float2* __restrict__ apar, float2* __restrict__ bpar) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int z = blockIdx.y;
+    if (k >= t.nk) return;
+    float a11 = 0.f, a12 = 0.f, a22 = 0.f, amp = 0.f;
+    float2 r1 = make_float2(0.f, 0.f), r2 = r1, ra = r1;
+    for (int s = 0; s < t.Ns; ++s) {
+        float sjj = 0.f, sjb = 0.f, sbb = 0.f, jprev = 0.f;
+        float2 n0 = make_float2(0.f, 0.f), nb = n0, n1 = n0;
+        for (int l = 0; l < t.Nl; ++l) {
+            const float j = t.Jl[(((size_t)s * t.Nl + l) * t.Nz + z) * t.nk + k], jb = j + jprev;
+            jprev = j;
+            sjj = fmaf(j, j, sjj); sjb = fmaf(j, jb, sjb); sbb = fmaf(jb, jb, sbb);
+            const float2 g0 = g[((((size_t)s * t.Nm + 0) * t.Nl + l) * t.Nz + z) * t.nk + k];
+            n0.x = fmaf(j, g0.x, n0.x); n0.y = fmaf(j, g0.y, n0.y);
+            nb.x = fmaf(jb, g0.x, nb.x); nb.y = fmaf(jb, g0.y, nb.y);
+            if (t.Nm > 1) {
+                const float2 g1 = g[((((size_t)s * t.Nm + 1) * t.Nl + l) * t.Nz + z) * t.nk + k];
+                n1.x = fmaf(j, g1.x, n1.x); n1.y = fmaf(j, g1.y, n1.y);
+            }
+        }
+        a11 += e.z2nt[s] * (1.f - sjj);
+        a12 += e.qn[s] * sjb;
+        a22 += e.nt[s] * sbb;
+        amp += e.z2nm[s] * sjj;
+        r1.x = fmaf(e.qn[s], n0.x, r1.x); r1.y = fmaf(e.qn[s], n0.y, r1.y);
+        r2.x = fmaf(e.nt[s], nb.x, r2.x); r2.y = fmaf(e.nt[s], nb.y, r2.y);
+        ra.x = fmaf(e.qnv[s], n1.x, ra.x); ra.y = fmaf(e.qnv[s], n1.y, ra.y);
+    }
+    const float h = 0.5f * beta / bmag2[z];
+    const float det = a11 * (1.f + h * a22) + a12 * h * a12;
+    const float idet = det != 0.f ? 1.f / det : 0.f;
+    const float c11 = (1.f + h * a22) * idet, c12 = -a12 * h * idet, c21 = -h * a12 * idet, c22 = -a11 * h * idet;
+    const float den = kp2[(size_t)z * t.nk + k] + 0.5f * beta * amp;
+    const float ia = den != 0.f ? 0.5f * beta / den : 0.f;
+    const size_t o = (size_t)z * t.nk + k;
+    const bool zero = k == 0;
+    phi[o] = zero ? make_float2(0.f, 0.f) : make_float2(c11 * r1.x + c12 * r2.x, c11 * r1.y + c12 * r2.y);
+    bpar[o] = zero ? make_float2(0.f, 0.f) : make_float2(c21 * r1.x + c22 * r2.x, c21 * r1.y + c22 * r2.y);
+    apar[o] = zero ? make_float2(0.f, 0.f) : make_float2(ia * ra.x, ia * ra.y);
+}
+
+// chi planes of the electromagnetic brackets in spectral form: chis[unit = (s,z,j)][k] = M fa + MB fb  (fb may be null)
+__global__ void __launch_bounds__(256) em_chi_spectral_kernel(const float* __restrict__ M, const float* __restrict__ MB,
+                                                              const float2* __restrict__ fa, const float2* __restrict__ fb,
+                                                              float2* __restrict__ chis, int nk, int Nz, int J) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int unit = blockIdx.y;
+    if (k >= nk) return;
+    const int z = (unit / J) % Nz;
+    const size_t i = (size_t)unit * nk + k;
+    const float2 a = fa[(size_t)z * nk + k];
+    float2 r = make_float2(M[i] * a.x, M[i] * a.y);
+    if (fb) {
+        const float2 b = fb[(size_t)z * nk + k];
+        r.x = fmaf(MB[i], b.x, r.x);
+        r.y = fmaf(MB[i], b.y, r.y);
+    }
+    chis[i] = r;
+}
+
+// g2_{l,m} = -v_ts ( sqrt(m+1) G_{l,m+1} + sqrt(m) G_{l,m-1} )  (Hermite recurrence of v_par; G outside 0 <= m < Nm is 0)
+__global__ void __launch_bounds__(256) em_hermite_shift_kernel(LinTables t, const float2* __restrict__ g, float2* __restrict__ g2) {
+    const unsigned pl = (unsigned)(t.Nl * t.Nz * t.nk);       // elements of one (s,m) slab
+    const unsigned i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= pl) return;
+    const int s = blockIdx.y / t.Nm, m = blockIdx.y % t.Nm;
+    const float up = -t.vt[s] * sqrtf((float)(m + 1)), dn = -t.vt[s] * sqrtf((float)m);
+    float2 r = make_float2(0.f, 0.f);
+    if (m + 1 < t.Nm) { const float2 a = g[(size_t)(s * t.Nm + m + 1) * pl + i]; r.x = up * a.x; r.y = up * a.y; }
+    if (m > 0) { const float2 a = g[(size_t)(s * t.Nm + m - 1) * pl + i]; r.x = fmaf(dn, a.x, r.x); r.y = fmaf(dn, a.y, r.y); }
+    g2[(size_t)(s * t.Nm + m) * pl + i] = r;
+}
+__global__ void __launch_bounds__(256) em_add_kernel(float4* __restrict__ out, const float4* __restrict__ add, size_t n4) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n4) { float4 a = out[i]; const float4 b = add[i]; a.x += b.x; a.y += b.y; a.z += b.z; a.w += b.w; out[i] = a; }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Linear terms of Eq. 4.9 for gx_linear_rhs / gx_rhs.
 // H_{l,m} = G_{l,m} + (Z/tau) J_l Phi delta_{m0} (Eq. 4.8) is formed on the fly; H, G, J vanish outside
 // 0 <= l < Nl, 0 <= m < Nm.

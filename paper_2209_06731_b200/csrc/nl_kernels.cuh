@@ -80,6 +80,9 @@ struct NlParams {
     const float2* twy;
     float dkx, dky, scale;
     int Nz, Nl, Nm, Ns, J;
+    // electromagnetic evaluations (gx_nonlinear_rhs_em) hand the chi kernels ready-made spectral planes
+    // chi_{s,z,j}(k): phi then holds one plane per unit (s,z,j) and M one shared plane of ones
+    int phi_by_unit, M_shared;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -361,8 +364,8 @@ __global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_kernel(const NlPara
     float2* twy = twx + C::NX;
     const int unit = blockIdx.x;                 // (s*Nz + z)*J + j
     const int z = (unit / p.J) % p.Nz;
-    const float2* __restrict__ phi = p.phi + (size_t)z * C::NK;
-    const float* __restrict__ M = p.M + (size_t)unit * C::NK;
+    const float2* __restrict__ phi = p.phi + (size_t)(p.phi_by_unit ? unit : z) * C::NK;
+    const float* __restrict__ M = p.M + (size_t)(p.M_shared ? 0 : unit) * C::NK;
     pdl_launch_dependents();        // the bracket kernel's prologue (a2-a4 x part) does not read dchi
     load_twiddles<C>(twx, twy, p);
     if constexpr (C::STAGE) {

@@ -91,8 +91,8 @@ __global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_row_kernel(const Nl
     float2* twx = S + C::S_ELEMS;
     const int unit = blockIdx.x;                 // (s*Nz + z)*J + j
     const int z = (unit / p.J) % p.Nz;
-    const float2* __restrict__ phi = p.phi + (size_t)z * C::NK;
-    const float* __restrict__ M = p.M + (size_t)unit * C::NK;
+    const float2* __restrict__ phi = p.phi + (size_t)(p.phi_by_unit ? unit : z) * C::NK;
+    const float* __restrict__ M = p.M + (size_t)(p.M_shared ? 0 : unit) * C::NK;
     pdl_launch_dependents();
     for (int i = threadIdx.x; i < C::NX; i += C::NT) twx[i] = p.twx[i];
     for (int i = threadIdx.x; i < C::NK; i += C::NT) {

@@ -487,8 +487,8 @@ __global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_rx_kernel(const NlP
     const int tid = threadIdx.x;
     const int unit = blockIdx.x;                 // (s*Nz + z)*J + j
     const int z = (unit / p.J) % p.Nz;
-    const float2* __restrict__ phi = p.phi + (size_t)z * C::NK;
-    const float* __restrict__ M = p.M + (size_t)unit * C::NK;
+    const float2* __restrict__ phi = p.phi + (size_t)(p.phi_by_unit ? unit : z) * C::NK;
+    const float* __restrict__ M = p.M + (size_t)(p.M_shared ? 0 : unit) * C::NK;
     pdl_launch_dependents();        // the bracket kernel's prologue (a2-a4 x part) does not read dchi
     for (int i = tid; i < C::NX; i += C::NT) twx[i] = p.twx[i];
     for (int i = tid; i < C::NK; i += C::NT) {
@@ -721,8 +721,8 @@ __global__ void __launch_bounds__(2 * C::NT, 1) nl_rx_persist_kernel(const NlPar
         if (item < n_chi) {
             // ---- a1 + a3 + a4 for the potential: chi plane (s,z,j)
             const int z = (item / p.J) % p.Nz;
-            const float2* __restrict__ phi = p.phi + (size_t)z * NK;
-            const float* __restrict__ M = p.M + (size_t)item * NK;
+            const float2* __restrict__ phi = p.phi + (size_t)(p.phi_by_unit ? item : z) * NK;
+            const float* __restrict__ M = p.M + (size_t)(p.M_shared ? 0 : item) * NK;
             for (int i = tid; i < NK; i += NT) {
                 const float2 f = __ldg(phi + i);
                 const float mm = __ldg(M + i);
@@ -906,8 +906,8 @@ __global__ void __launch_bounds__(512, 1) nl_rx_pipeline_kernel(const NlParams p
                 // ---- produce item k into W4[b]: compact plane S, then the inverse x passes
                 if (item < n_chi) {
                     const int z = (item / p.J) % p.Nz;
-                    const float2* __restrict__ phi = p.phi + (size_t)z * NK;
-                    const float* __restrict__ M = p.M + (size_t)item * NK;
+                    const float2* __restrict__ phi = p.phi + (size_t)(p.phi_by_unit ? item : z) * NK;
+                    const float* __restrict__ M = p.M + (size_t)(p.M_shared ? 0 : item) * NK;
                     for (int i = tid; i < NK; i += NXW) {
                         const float2 f = __ldg(phi + i);
                         const float mm = __ldg(M + i);

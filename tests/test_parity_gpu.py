@@ -541,3 +541,67 @@ def test_linear_rhs_parity_with_end_damping(torch_cuda, name, linked):
     assert O.relative_max_error(out, ref) <= TOL
     assert O.relative_max_error(off, ref) > 20 * TOL           # the layer is visible at this tolerance
     grid.close()
+
+
+# ------------------------------------------------------------------------------------------------
+# electromagnetic brackets and field solve
+@pytest.mark.parametrize("name", ["tiny", "kinetic"])
+def test_em_nonlinear_rhs_parity(torch_cuda, name):
+    """gx_nonlinear_rhs_em against the oracle's nonlinear_rhs_em (App. D Eq. D1 lines 1-4): every plane on tiny,
+    sampled planes at the kinetic size; each of the three potentials is visible on its own at the tolerance."""
+    torch = torch_cuda
+    cfg = I.named_config(name)
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    Apar = (0.7 * I.random_phi(cfg, geo, seed_offset=101)).astype(np.complex64)
+    Bpar = (0.4 * I.random_phi(cfg, geo, seed_offset=202)).astype(np.complex64)
+    grid = _grid(cfg, geo)
+    g = torch.from_numpy(G).cuda()
+    f = [torch.from_numpy(a).cuda() for a in (Phi, Apar, Bpar)]
+    out = torch.full_like(g, float("nan"))
+    grid.nonlinear_rhs_em(g, f[0], f[1], f[2], out)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    planes = None if name == "tiny" else [(0, 0, 0), (1, 0, 5), (1, 7, 31), (0, 4, 16), (1, 3, 9)]
+    kw = dict(method="dft", planes=planes)
+    ref = O.nonlinear_rhs_em(G, Phi, Apar, Bpar, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, **kw)
+    es = O.nonlinear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, **kw)
+    noA = O.nonlinear_rhs_em(G, Phi, 0 * Apar, Bpar, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, **kw)
+    sel = [(s, m, z) for s in range(cfg.Ns) for m in range(cfg.Nm) for z in range(cfg.Nz)] if planes is None else planes
+    assert np.all(np.isfinite(out))
+    for (s, m, z) in sel:
+        a, r = out[s, m, :, z], ref[s, m, :, z]
+        den = np.max(np.abs(r))
+        assert np.max(np.abs(a - r)) <= TOL * den, (s, m, z)
+    big = max(np.max(np.abs(ref[s, m, :, z])) for (s, m, z) in sel)
+    assert max(np.max(np.abs((es - ref)[s, m, :, z])) for (s, m, z) in sel) > 100 * TOL * big
+    assert max(np.max(np.abs((noA - ref)[s, m, :, z])) for (s, m, z) in sel) > 100 * TOL * big
+    assert max(np.max(np.abs((noA - es)[s, m, :, z])) for (s, m, z) in sel) > 100 * TOL * big
+    # zero vector potentials: the electrostatic entry point, bit for bit
+    zero = torch.zeros_like(f[0])
+    out0 = torch.full_like(g, float("nan"))
+    grid.nonlinear_rhs_em(g, f[0], zero, zero, out0)
+    torch.cuda.synchronize()
+    assert np.array_equal(out0.cpu().numpy(), _gpu_nl(torch, grid, G, Phi))
+    grid.close()
+
+
+def test_em_field_solve_parity(torch_cuda):
+    torch = torch_cuda
+    cfg = I.named_config("kinetic")
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo, planes=[(s, m) for s in range(cfg.Ns) for m in (0, 1)])
+    grid = _grid(cfg, geo)
+    g = torch.from_numpy(G).cuda()
+    f = [torch.empty(cfg.phi_shape, dtype=torch.complex64, device="cuda") for _ in range(3)]
+    for beta in (0.0, 0.01):
+        grid.field_solve_em(g, beta, f[0], f[1], f[2])
+        torch.cuda.synchronize()
+        ref = O.field_solve_em(G, beta, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species)
+        for a, r, nm in zip(f, ref, ("phi", "apar", "bpar")):
+            if np.max(np.abs(r)) == 0:
+                assert torch.all(a == 0), nm
+            else:
+                assert O.relative_max_error(a.cpu().numpy(), r) <= TOL, (beta, nm)
+    grid.close()
