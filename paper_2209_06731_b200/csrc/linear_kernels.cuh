@@ -8,6 +8,8 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include "dft_regs.cuh"
+
 #include <algorithm>
 #include <cmath>
 #include <string>
@@ -41,6 +43,8 @@ struct LinTables {
     float* bs = nullptr;       // [s][z][k]  b_s
     float* Dz = nullptr;       // [Nz] circulant column of gradpar * spectral d/dz:  D[z][z'] = Dz[(z - z') mod Nz]
     float* Az = nullptr;       // [Nz] circulant column of |gradpar| * spectral |k_z|
+    float2* twz = nullptr;     // [Nz] e^{+2 pi i t/Nz}: twiddles of the z FFT path (Nz = 64, 96, 128)
+    float gradpar = 0.f;
     float* omd = nullptr;      // [2][z][k]  omega_d^kappa, omega_d^gradB
     float* hypv = nullptr;     // [z][k] D (kperp2/kperp2max)^n
     float* dend = nullptr;     // [z][k] end-damping profile d(z_hat) of Eq. 4.30 (nullptr: layer off)
@@ -70,7 +74,7 @@ constexpr int kLinLaunchesRhs = 3;
 
 inline void lin_tables_free(LinTables& t) {
     cudaFree(t.Jl); cudaFree(t.invD); cudaFree(t.fsfac); cudaFree(t.wz); cudaFree(t.bs);
-    cudaFree(t.Dz); cudaFree(t.Az); cudaFree(t.omd); cudaFree(t.hypv); cudaFree(t.dend); cudaFree(t.bgrad);
+    cudaFree(t.Dz); cudaFree(t.Az); cudaFree(t.twz); cudaFree(t.omd); cudaFree(t.hypv); cudaFree(t.dend); cudaFree(t.bgrad);
     cudaFree(t.mpow); cudaFree(t.mom);
     cudaFree(t.chain_off); cudaFree(t.chain_mode); cudaFree(t.ext_off); cudaFree(t.ext_d); cudaFree(t.ext_a); cudaFree(t.zwork);
     t = LinTables();
@@ -168,6 +172,12 @@ inline bool lin_tables_build(const LinHostInput& in, LinTables& t, size_t& bytes
         }
         dzc[d] = (float)(in.gradpar * sd / Nz);
         azc[d] = (float)(std::abs(in.gradpar) * sa / Nz);
+    }
+    {
+        std::vector<float2> tw(Nz);
+        for (int i = 0; i < Nz; ++i) tw[i] = make_float2((float)std::cos(2.0 * M_PI * i / Nz), (float)std::sin(2.0 * M_PI * i / Nz));
+        if (!lin_upload(&t.twz, tw, bytes, msg)) return false;
+        t.gradpar = (float)in.gradpar;
     }
     const double p_hyp = 0.5 * in.Nm, m_max = std::max(in.Nm - 1, 1);
     for (int m = 0; m < in.Nm; ++m) mpow[m] = m > 2 ? (float)std::pow((double)m, p_hyp) : 0.f;
@@ -482,13 +492,84 @@ __global__ void __launch_bounds__(256) lin_moments_kernel(LinTables t, const flo
 constexpr int kLinTK = 32;      // k per block
 constexpr int kLinZG = 8;       // z groups per block
 
+// Spectral z operators by FFT (Eq. 4.10-4.11) for long field lines: for every column tk of the tile
+//     S1[z] <- F^-1[ -v_t gradpar (i k_z) F[S1] - hyp |gradpar| |k_z| F[S2] ](z)      (Nyquist dropped in the derivative)
+// with N = A*B two register-radix passes each way through shared memory: the forward transform is decimation in
+// time with digit-transposed output (position k1*B + k2 holds k = k1 + A*k2), the inverse the matching decimation
+// in frequency that reads that order and ends in natural order (same scheme as the x passes of nl_kernels.cuh).
+// S2 is preserved (the hyper-viscosity term reads G_{l,m} from it later); S3 is scratch for its transform.
+template <int A, int B>
+__device__ __forceinline__ void lin_zfft(float2* __restrict__ S1, const float2* __restrict__ S2, float2* __restrict__ S3,
+                                         const float2* __restrict__ tw, float vt_gp, float hyp_gp, bool with_hyp) {
+    constexpr int N = A * B, NT = kLinTK * kLinZG;
+    // forward pass 1: DFT_A over n1 of z = n1*B + n2, twiddle e^{-2 pi i n2 k1 / N}
+    for (int it = threadIdx.x; it < B * kLinTK; it += NT) {
+        const int n2 = it / kLinTK, c = it - n2 * kLinTK;
+        float2 v[A], u[A];
+#pragma unroll
+        for (int n1 = 0; n1 < A; ++n1) {
+            v[n1] = S1[(n1 * B + n2) * kLinTK + c];
+            u[n1] = with_hyp ? S2[(n1 * B + n2) * kLinTK + c] : make_float2(0.f, 0.f);
+        }
+        dft<A, -1>(v);
+        if (with_hyp) dft<A, -1>(u);
+#pragma unroll
+        for (int k1 = 0; k1 < A; ++k1) {
+            const float2 w = tw[(n2 * k1) % N];
+            S1[(k1 * B + n2) * kLinTK + c] = k1 == 0 ? v[0] : cmul_conj(v[k1], w);
+            if (with_hyp) S3[(k1 * B + n2) * kLinTK + c] = k1 == 0 ? u[0] : cmul_conj(u[k1], w);
+        }
+    }
+    __syncthreads();
+    // forward pass 2 + spectral factors + inverse pass 1 (DFT_B over the same B values: the register tile is reused)
+    for (int it = threadIdx.x; it < A * kLinTK; it += NT) {
+        const int k1 = it / kLinTK, c = it - k1 * kLinTK;
+        float2 v[B], u[B];
+#pragma unroll
+        for (int n2 = 0; n2 < B; ++n2) {
+            v[n2] = S1[(k1 * B + n2) * kLinTK + c];
+            u[n2] = with_hyp ? S3[(k1 * B + n2) * kLinTK + c] : make_float2(0.f, 0.f);
+        }
+        dft<B, -1>(v);
+        if (with_hyp) dft<B, -1>(u);
+#pragma unroll
+        for (int k2 = 0; k2 < B; ++k2) {
+            const int k = k1 + A * k2;                           // frequency of this value
+            const int kz = k <= N / 2 ? k : k - N;
+            const float fd = (N % 2 == 0 && k == N / 2) ? 0.f : -vt_gp * (float)kz * (1.f / N);   // -v_t gradpar i k_z / N
+            const float fa = -hyp_gp * fabsf((float)kz) * (1.f / N);
+            // (i fd) v + fa u
+            v[k2] = make_float2(-fd * v[k2].y + fa * u[k2].x, fd * v[k2].x + fa * u[k2].y);
+        }
+        // inverse pass 1: for a = k1, DFT_B(+) over b = k2 -> d, twiddle e^{+2 pi i a d / N}
+        dft<B, +1>(v);
+#pragma unroll
+        for (int d = 0; d < B; ++d)
+            S1[(k1 * B + d) * kLinTK + c] = d == 0 ? v[0] : cmul(v[d], tw[(k1 * d) % N]);
+    }
+    __syncthreads();
+    // inverse pass 2: for each d, DFT_A(+) over a -> cc; z = d + B*cc (natural order)
+    for (int it = threadIdx.x; it < B * kLinTK; it += NT) {
+        const int d = it / kLinTK, c = it - d * kLinTK;
+        float2 v[A];
+#pragma unroll
+        for (int a = 0; a < A; ++a) v[a] = S1[(a * B + d) * kLinTK + c];
+        dft<A, +1>(v);
+        // in place: the item's outputs z = d + B*cc occupy exactly the positions a*B + d it has just read
+#pragma unroll
+        for (int cc = 0; cc < A; ++cc) S1[(d + B * cc) * kLinTK + c] = v[cc];
+    }
+    __syncthreads();
+}
+
 // out[s,m,l,z,k] (+)= linear terms.  Block: one (s,m,l), a tile of kLinTK modes k, all z.  The spectral
 // parallel derivative / |k_par| are circulant Nz x Nz products on tiles staged in shared memory.
 // ZB = 4: each thread owns blocks of 4 consecutive z and register-blocks the circulant products (one staged
 // value and one new weight per term feed 8 FMAs); ZB = 1 when Nz is not a multiple of 4.
 // DERIV_ONLY: only the two z-operator terms (streaming, hyper-collisions), added to out; the pointwise terms
 // then come from lin_point_kernel.
-template <bool ACC, int ZB, bool DERIV_ONLY = false>
+// FA x FB > 0: the z operators by FFT (lin_zfft, Nz = FA*FB) instead of the O(Nz^2) circulant products.
+template <bool ACC, int ZB, bool DERIV_ONLY = false, int FA = 0, int FB = 0>
 __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, const float2* __restrict__ g,
                                                                  const float2* __restrict__ phi,
                                                                  float2* __restrict__ out, const bool skip_z) {
@@ -497,16 +578,25 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
     float2* S2 = S1 + (size_t)t.Nz * kLinTK;                     // [Nz][TK] G_{l,m} (hyper-collisions)
     float* dz = reinterpret_cast<float*>(S2 + (size_t)t.Nz * kLinTK);   // [2 Nz] column repeated: no wrap test
     float* az = dz + 2 * t.Nz;
+    float2* S3 = reinterpret_cast<float2*>(az + 2 * t.Nz);       // FFT path only: [Nz][TK] scratch
+    static_assert(FA == 0 || ZB == 1, "the FFT path writes one z per thread and step");
     const int tk = threadIdx.x % kLinTK, zg = threadIdx.x / kLinTK;
-    const int k = blockIdx.x * kLinTK + tk;
+    // (s,m) varies fastest over the grid: the blocks that read the slabs m-1, m, m+1 of one k tile run together and
+    // share them through L2 (the state of the large configurations is several times the L2 capacity)
+    const int k = blockIdx.z * kLinTK + tk;
     const int l = blockIdx.y;
-    const int s = blockIdx.z / t.Nm, m = blockIdx.z % t.Nm;
+    const int s = blockIdx.x / t.Nm, m = blockIdx.x % t.Nm;
     const bool live = k < t.nk;
     const float sm1 = sqrtf((float)(m + 1)), sm0 = sqrtf((float)m);
-    for (int i = threadIdx.x; i < 2 * t.Nz; i += blockDim.x) {
-        const int d = i < t.Nz ? i : i - t.Nz;
-        dz[i] = t.Dz[d];
-        az[i] = t.Az[d];
+    if constexpr (FA > 0) {
+        float2* tws = reinterpret_cast<float2*>(dz);              // [Nz] twiddles in place of the circulant columns
+        for (int i = threadIdx.x; i < t.Nz; i += blockDim.x) tws[i] = t.twz[i];
+    } else {
+        for (int i = threadIdx.x; i < 2 * t.Nz; i += blockDim.x) {
+            const int d = i < t.Nz ? i : i - t.Nz;
+            dz[i] = t.Dz[d];
+            az[i] = t.Az[d];
+        }
     }
     {
         // staging: 4 z at a time, every load issued before the first use (indices clamped, invalid masked)
@@ -542,6 +632,12 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
         }
     }
     __syncthreads();
+    if constexpr (FA > 0) {
+        // every thread of the block takes part (dead columns hold zeros)
+        if (!skip_z)
+            lin_zfft<FA, FB>(S1, S2, S3, reinterpret_cast<const float2*>(dz), t.vt[s] * t.gradpar,
+                             t.nuhyp[s] * t.mpow[m] * fabsf(t.gradpar), t.nuhyp[s] * t.mpow[m] != 0.f);
+    }
     if (!live) return;
     const float vt = t.vt[s], tz = t.tz[s], nu = t.nu[s];
     const float hyp = t.nuhyp[s] * t.mpow[m];
@@ -589,9 +685,11 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
                   }
               }
           };
-          if (!skip_z) {                        // linked boundary: the z operators come from lin_zlink_kernel
-              blocked(dz, S1 + tk, dpb);
-              if (hyp != 0.f) blocked(az, S2 + tk, apb);
+          if constexpr (FA == 0) {
+              if (!skip_z) {                    // linked boundary: the z operators come from lin_zlink_kernel
+                  blocked(dz, S1 + tk, dpb);
+                  if (hyp != 0.f) blocked(az, S2 + tk, apb);
+              }
           }
       }
 #pragma unroll
@@ -599,6 +697,9 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
         const int z = z0 + zi;
         const float2 dp = dpb[zi], ap = apb[zi];
         float2 r = make_float2(-vt * dp.x - hyp * ap.x, -vt * dp.y - hyp * ap.y);
+        if constexpr (FA > 0) {
+            if (!skip_z) r = S1[z * kLinTK + tk];               // both z-operator terms, already scaled (lin_zfft)
+        }
         if constexpr (!DERIV_ONLY) {
         const float2 h00 = lin_H(t, g, phi, s, l, m, z, k);
         // mirror force
@@ -683,9 +784,9 @@ template <int MAXL, bool ACC>
 __global__ void __launch_bounds__(256) lin_point_kernel(LinTables t, const float2* __restrict__ g,
                                                         const float2* __restrict__ phi, float2* __restrict__ out) {
     const unsigned pl = (unsigned)(t.Nz * t.nk);
-    const unsigned zk = blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned zk = blockIdx.y * blockDim.x + threadIdx.x;       // (s,m) fastest over the grid: m-2..m+2 share L2
     if (zk >= pl) return;
-    const int s = blockIdx.y / t.Nm, m = blockIdx.y % t.Nm;
+    const int s = blockIdx.x / t.Nm, m = blockIdx.x % t.Nm;
     const int z = zk / t.nk, k = zk - z * t.nk;
     const float zt = t.zt[s], vt = t.vt[s], tz = t.tz[s], nu = t.nu[s];
     const float2 f = phi[zk];
@@ -897,7 +998,41 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
         dim3 gm((t.nk + 255) / 256, t.Nz, t.Ns);
         lin_moments_kernel<<<gm, 256, 0, st>>>(t, g, phi);
     }
-    const size_t smem = (size_t)t.Nz * kLinTK * sizeof(float2) * 2 + 4 * (size_t)t.Nz * sizeof(float);
+    const int fa = (t.Nz == 64 || t.Nz == 96 || t.Nz == 128) ? 8 : 0;      // z FFT path: Nz = 8 x {8, 12, 16}
+    const size_t smem = (size_t)t.Nz * kLinTK * sizeof(float2) * (fa ? 3 : 2) + 4 * (size_t)t.Nz * sizeof(float);
+    if (fa && !t.linked) {
+        cudaError_t e = cudaSuccess;
+        dim3 gridf(t.Ns * t.Nm, t.Nl, (t.nk + kLinTK - 1) / kLinTK);
+        const bool splitf = t.Nl <= 6;        // pointwise terms with the stencil in registers, z operators added on top
+        if (splitf) {
+            dim3 gp(t.Ns * t.Nm, (unsigned)(((size_t)t.Nz * t.nk + 255) / 256));
+            if (t.Nl <= 4) {
+                if (accumulate) lin_point_kernel<4, true><<<gp, 256, 0, st>>>(t, g, phi, out);
+                else lin_point_kernel<4, false><<<gp, 256, 0, st>>>(t, g, phi, out);
+            } else {
+                if (accumulate) lin_point_kernel<6, true><<<gp, 256, 0, st>>>(t, g, phi, out);
+                else lin_point_kernel<6, false><<<gp, 256, 0, st>>>(t, g, phi, out);
+            }
+        }
+#define GX_ZFFT(FB)                                                                                                        \
+    do {                                                                                                                   \
+        if (splitf) {                                                                                                      \
+            e = cudaFuncSetAttribute(lin_rhs_kernel<true, 1, true, 8, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+            if (e == cudaSuccess) lin_rhs_kernel<true, 1, true, 8, FB><<<gridf, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false);  \
+        } else if (accumulate) {                                                                                           \
+            e = cudaFuncSetAttribute(lin_rhs_kernel<true, 1, false, 8, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+            if (e == cudaSuccess) lin_rhs_kernel<true, 1, false, 8, FB><<<gridf, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false); \
+        } else {                                                                                                           \
+            e = cudaFuncSetAttribute(lin_rhs_kernel<false, 1, false, 8, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
+            if (e == cudaSuccess) lin_rhs_kernel<false, 1, false, 8, FB><<<gridf, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false); \
+        }                                                                                                                  \
+    } while (0)
+        if (t.Nz == 64) GX_ZFFT(8);
+        else if (t.Nz == 96) GX_ZFFT(12);
+        else GX_ZFFT(16);
+#undef GX_ZFFT
+        return e != cudaSuccess ? e : cudaGetLastError();
+    }
     static bool attr = false;
     if (!attr) {
         cudaError_t e = cudaFuncSetAttribute(lin_rhs_kernel<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
@@ -909,13 +1044,13 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
         if (e != cudaSuccess) return e;
         attr = true;
     }
-    dim3 grid((t.nk + kLinTK - 1) / kLinTK, t.Nl, t.Ns * t.Nm);
+    dim3 grid(t.Ns * t.Nm, t.Nl, (t.nk + kLinTK - 1) / kLinTK);
     const bool b4 = t.Nz % 4 == 0;
     const bool split = t.Nl <= 4 || t.linked;
     if (split && t.Nl <= 8) {
         // pointwise terms with the stencil in registers, then the z-operator terms added on top (measured faster
         // for Nl <= 4 only: with 8 Laguerre moments the 5 x 10 stencil costs 135 registers and the occupancy)
-        dim3 gp((unsigned)(((size_t)t.Nz * t.nk + 255) / 256), t.Ns * t.Nm);
+        dim3 gp(t.Ns * t.Nm, (unsigned)(((size_t)t.Nz * t.nk + 255) / 256));
         if (t.Nl <= 4) {
             if (accumulate) lin_point_kernel<4, true><<<gp, 256, 0, st>>>(t, g, phi, out);
             else lin_point_kernel<4, false><<<gp, 256, 0, st>>>(t, g, phi, out);

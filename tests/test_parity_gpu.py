@@ -605,3 +605,32 @@ def test_em_field_solve_parity(torch_cuda):
             else:
                 assert O.relative_max_error(a.cpu().numpy(), r) <= TOL, (beta, nm)
     grid.close()
+
+
+@pytest.mark.parametrize("Nz,Nl,Nm", [(64, 6, 5), (96, 2, 4), (128, 6, 4), (128, 4, 5)])
+def test_linear_rhs_parity_z_fft_path(torch_cuda, Nz, Nl, Nm):
+    """Long field lines (Nz = 64, 96, 128): the parallel derivative and |k_par| by FFT in z (Eq. 4.10-4.11)
+    instead of circulant products, in the fused kernel (Nl > 4) and behind the pointwise kernel (Nl <= 4)."""
+    torch = torch_cuda
+    cfg = I.Config("zfft", 16, 16, Nz, Nl, Nm, [I.Species(tprim=3.0, fprim=1.0, nu_ss=0.01)], geometry="harmonics", seed=900 + Nz + Nl)
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = _grid(cfg, geo)
+    g, phi = torch.from_numpy(G).cuda(), torch.from_numpy(Phi).cuda()
+    out = torch.full_like(g, float("nan"))
+    grid.linear_rhs(g, phi, out)
+    torch.cuda.synchronize()
+    out = out.cpu().numpy()
+    ref = _oracle_lin(cfg, geo, G, Phi)
+    assert np.all(np.isfinite(out))
+    assert O.relative_max_error(out, ref) <= TOL
+    for m in range(cfg.Nm):
+        assert O.relative_max_error(out[0, m], ref[0, m]) <= 5 * TOL, m
+    # accumulate form (gx_rhs) through the same kernels
+    out2 = torch.full_like(g, float("nan"))
+    grid.rhs(g, out2)
+    torch.cuda.synchronize()
+    ref2 = OL.rhs(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species, tau_fac=cfg.tau_fac)
+    assert O.relative_max_error(out2.cpu().numpy(), ref2) <= TOL
+    grid.close()
