@@ -238,6 +238,92 @@ def fp32_ubench(B, sm_mhz, n_sm, full=False):
     return out
 
 
+# ------------------------------------------------------------------------------- tensor-core DFT question
+def run_tcdft(args):
+    """`--tcdft`: would the radix-16 stages pay as split-TF32 matrix products on the tensor cores?  Measures
+    (i) the library's register radix-16 (scalar and packed), (ii) the TF32 and BF16 tensor rates of this GPU on a
+    large library GEMM (cuBLAS, which runs tcgen05 kernels on sm_100a: an upper bound for any hand-written tile),
+    (iii) the accuracy of the 3-term split DFT16 = Xh Wh + Xh Wl + Xl Wh on the tensor cores against fp64.  A
+    16-point complex DFT as a real matrix product is a [32 x 32] matrix per vector: 1024 MACs, x3 for the split."""
+    import torch
+    from paper_2209_06731_b200 import binding as B
+    dev = torch.device("cuda", 0)
+    n_sm = torch.cuda.get_device_properties(dev).multi_processor_count
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    clk = (peaks.get("sm_max_mhz") or 1965.0) * 1e6
+    out = {"leg": "tcdft", "n_sm": n_sm, "sm_clock_mhz": clk / 1e6}
+    # (i) register radix-16
+    for packed, name in [(0, "radix16_scalar"), (1, "radix16_packed")]:
+        best = 0.0
+        for nt, bps in [(192, 2), (256, 2), (128, 4)]:
+            try:
+                ms, n = B.gx_ubench_dft16(packed, nt, bps, 512)
+                best = max(best, n / (ms * 1e-3))
+            except B.GxError:
+                pass
+        out[name] = {"transforms_per_s": best, "cycles_per_transform_per_sm": clk * n_sm / best}
+    # (ii) tensor rates on a large GEMM
+    def gemm_rate(dtype, allow_tf32):
+        torch.backends.cuda.matmul.allow_tf32 = allow_tf32
+        n = 8192
+        a = torch.randn(n, n, device=dev, dtype=dtype)
+        b = torch.randn(n, n, device=dev, dtype=dtype)
+        for _ in range(2):
+            a @ b
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record()
+        for _ in range(5):
+            a @ b
+        e1.record()
+        torch.cuda.synchronize()
+        return 5 * 2.0 * n ** 3 / (e0.elapsed_time(e1) * 1e-3)
+    tf32 = gemm_rate(torch.float32, True)
+    bf16 = gemm_rate(torch.bfloat16, False)
+    fp32 = gemm_rate(torch.float32, False)
+    out["gemm_flops_per_s"] = {"tf32": tf32, "bf16": bf16, "fp32_cuda_cores": fp32}
+    macs = 32 * 32
+    for name, rate, terms in [("dft16_as_tf32_3term", tf32, 3), ("dft16_as_bf16_6term", bf16, 6)]:
+        cyc = terms * 2.0 * macs / (rate / (clk * n_sm))
+        out[name] = {"cycles_per_transform_per_sm_upper_bound": cyc,
+                     "note": "tensor pipe only at the measured library GEMM rate: no operand split, staging or TMEM read-back"}
+    # (iii) accuracy of the 3-term split on the real tensor cores
+    torch.backends.cuda.matmul.allow_tf32 = True
+    nb = 1 << 16
+    x = torch.randn(nb, 32, device=dev, dtype=torch.float64)
+    k = torch.arange(16, device=dev, dtype=torch.float64)
+    ang = 2.0 * np.pi * torch.outer(k, k) / 16.0
+    c, sn = torch.cos(ang), torch.sin(ang)
+    w = torch.zeros(32, 32, device=dev, dtype=torch.float64)      # interleaved (re, im): y = x W, inverse DFT e^{+i ang}
+    w[0::2, 0::2], w[0::2, 1::2], w[1::2, 0::2], w[1::2, 1::2] = c, sn, -sn, c
+    ref = x @ w
+    def tf32_round(t):                                          # keep 10 explicit mantissa bits (round to nearest even)
+        i = t.float().view(torch.int32)
+        i = (i + 0x00000FFF + ((i >> 13) & 1)) & ~0x1FFF
+        return i.view(torch.float32)
+    xf, wf = x.float(), w.float()
+    xh, wh = tf32_round(xf), tf32_round(wf)
+    xl, wl = xf - xh, wf - wh
+    y1 = (xh @ wh).double()
+    y3 = ((xh @ wh) + (xh @ wl) + (xl @ wh)).double()
+    scale = ref.abs().max()
+    torch.backends.cuda.matmul.allow_tf32 = False
+    yf = (xf @ wf).double()
+    out["accuracy_vs_fp64"] = {"tf32_1term": float((y1 - ref).abs().max() / scale), "tf32_3term": float((y3 - ref).abs().max() / scale),
+                               "fp32_matmul": float((yf - ref).abs().max() / scale)}
+    out["split_cost_lane_ops_per_transform"] = 2 * 32      # per real: one rounding op and one subtraction on the CUDA cores
+    r = out["radix16_packed"]["cycles_per_transform_per_sm"]
+    out["verdict"] = ("tensor form needs %.2f cycles per transform and SM at best (TF32, 3 terms) + %.2f cycles of FP32 pipe for the operand "
+                      "split, against %.2f measured for the register radix-16: not adopted" %
+                      (out["dft16_as_tf32_3term"]["cycles_per_transform_per_sm_upper_bound"], 64 / 123.0, r))
+    print(json.dumps(out))
+    return 0
+
+
 # ------------------------------------------------------------------------------- GPU leg
 def run_gpu(args):
     import torch
@@ -450,12 +536,15 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--skip-cpu-baseline", action="store_true", help="omit the oracle timing (ncu passes)")
     ap.add_argument("--skip-reference-point", action="store_true", help="omit the cuFFT+cuBLAS composition")
+    ap.add_argument("--tcdft", action="store_true", help="tensor-core DFT question: radix-16 in registers vs split-TF32 matrix form")
     ap.add_argument("--ubench", action="store_true", help="FP32 pipe micro-benchmark at more launch shapes (roofline.fp32_pipe_...)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     if args.impl == "reference":
         return run_reference(args)
+    if args.tcdft:
+        return run_tcdft(args)
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         # no launcher: start one process per GPU ourselves (same command the driver uses)
         import subprocess

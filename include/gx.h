@@ -187,6 +187,12 @@ const char* gx_last_error(gx_grid* g);
  * roofline.peak_measured from it ("the bench should also run a tiny FMA-peak kernel"). */
 int gx_ubench_fp32(int kind, int threads_per_block, int blocks_per_sm, int iters, double* ms, double* lane_ops);
 
+/* Register radix-16 micro-benchmark: `iters` 16-point complex DFTs (+ 15 twiddle multiplications each, as in a
+ * two-pass FFT) per thread, entirely in registers; packed != 0: two transforms per thread in the packed FP32 form of
+ * dft_packed.cuh.  *transforms = number of 16-point transforms done.  Used by `bench.py --tcdft`, which sets this
+ * rate against the tensor-core rate a split-TF32 matrix form of the same DFT could reach (profiles/r02_tensor_dft.md). */
+int gx_ubench_dft16(int packed, int threads_per_block, int blocks_per_sm, int iters, double* ms, double* transforms);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,7 +23,7 @@ FAMILY_NAMES = {0: "scalar", 3: "row", 5: "rx", 6: "rxp", 7: "rxw"}
 EXPORTED = ["gx_grid_create", "gx_grid_destroy", "gx_box_set", "gx_species_set", "gx_adiabatic_set",
             "gx_dissipation_set", "gx_boundary_set", "gx_damping_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_em", "gx_field_solve_em", "gx_nonlinear_rhs_host",
             "gx_field_solve", "gx_rhs", "gx_linear_rhs", "gx_ssprk3_step", "gx_query", "gx_export_maps",
-            "gx_export_tables", "gx_profile_set", "gx_profile_get", "gx_last_error", "gx_ubench_fp32"]
+            "gx_export_tables", "gx_profile_set", "gx_profile_get", "gx_last_error", "gx_ubench_fp32", "gx_ubench_dft16"]
 
 _lib = None
 
@@ -69,6 +69,7 @@ def load():
     lib.gx_last_error.argtypes = [vp]
     lib.gx_last_error.restype = C.c_char_p
     lib.gx_ubench_fp32.argtypes = [i, i, i, i, dp, dp]
+    lib.gx_ubench_dft16.argtypes = [i, i, i, i, dp, dp]
     for name in EXPORTED:
         if name != "gx_last_error":
             getattr(lib, name).restype = i
@@ -214,6 +215,13 @@ def gx_ubench_fp32(kind, threads_per_block=512, blocks_per_sm=2, iters=4096):
     ms, ops = C.c_double(), C.c_double()
     _check(None, load().gx_ubench_fp32(kind, threads_per_block, blocks_per_sm, iters, C.byref(ms), C.byref(ops)))
     return ms.value, ops.value
+
+
+def gx_ubench_dft16(packed, threads_per_block=192, blocks_per_sm=2, iters=512):
+    """-> (milliseconds, 16-point transforms done) of the register radix-16 micro-benchmark (include/gx.h)."""
+    ms, n = C.c_double(), C.c_double()
+    _check(None, load().gx_ubench_dft16(int(packed), threads_per_block, blocks_per_sm, iters, C.byref(ms), C.byref(n)))
+    return ms.value, n.value
 
 
 # ---- convenience wrapper (marshalling only) -------------------------------------------------------

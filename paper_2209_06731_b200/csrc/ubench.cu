@@ -4,6 +4,7 @@
 #include <cuda_runtime.h>
 
 #include "../../include/gx.h"
+#include "dft_packed.cuh"
 
 namespace {
 
@@ -35,7 +36,73 @@ template <int KIND> __global__ void fp32_kernel(float* sink, int iters, float se
     if (s == 123.456f) sink[0] = s;
 }
 
+// batched 16-point complex DFTs held in registers, the building block of the x passes: `iters` transforms per
+// thread back to back (each followed by one twiddle multiplication, as in a two-pass FFT), scalar or packed
+// (two transforms per thread in FADD2/FFMA2 form)
+template <bool PACKED> __global__ void dft16_kernel(float* sink, int iters, float seed) {
+    using namespace gx;
+    if constexpr (PACKED) {
+        pk::c2 v[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+            v[i] = pk::make_c2(pk::pk2(seed + i + threadIdx.x * 1e-3f, seed - i), pk::pk2(0.5f * i, seed * i - threadIdx.x * 1e-3f));
+        for (int it = 0; it < iters; ++it) {
+            pk::dft<16, +1>(v);
+#pragma unroll
+            for (int i = 1; i < 16; ++i) v[i] = pk::cmul_s(v[i], 0.0624f, 0.0012f * i);
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) s += pk::lo(v[i].re) + pk::hi(v[i].im);
+        if (s == 123.456f) sink[0] = s;
+    } else {
+        float2 v[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i) v[i] = make_float2(seed + i + threadIdx.x * 1e-3f, 0.5f * i - seed);
+        for (int it = 0; it < iters; ++it) {
+            dft<16, +1>(v);
+#pragma unroll
+            for (int i = 1; i < 16; ++i) v[i] = cmul(v[i], make_float2(0.0624f, 0.0012f * i));
+        }
+        float s = 0.f;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) s += v[i].x + v[i].y;
+        if (s == 123.456f) sink[0] = s;
+    }
+}
+
 }  // namespace
+
+extern "C" int gx_ubench_dft16(int packed, int threads_per_block, int blocks_per_sm, int iters, double* ms, double* transforms) {
+    if (threads_per_block < 32 || threads_per_block > 1024 || blocks_per_sm < 1 || iters < 1 || !ms || !transforms) return GX_ERR_ARG;
+    int dev = 0, nsm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess)
+        return GX_ERR_CUDA;
+    float* sink = nullptr;
+    if (cudaMalloc(&sink, 4) != cudaSuccess) return GX_ERR_ALLOC;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int grid = nsm * blocks_per_sm;
+    void (*k)(float*, int, float) = packed ? dft16_kernel<true> : dft16_kernel<false>;
+    k<<<grid, threads_per_block>>>(sink, iters / 8 + 1, 0.37f);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        cudaEventRecord(e0);
+        k<<<grid, threads_per_block>>>(sink, iters, 0.37f);
+        cudaEventRecord(e1);
+        e = cudaEventSynchronize(e1);
+    }
+    float t = 0.f;
+    if (e == cudaSuccess) cudaEventElapsedTime(&t, e0, e1);
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (e != cudaSuccess) return GX_ERR_CUDA;
+    *ms = t;
+    *transforms = (double)grid * threads_per_block * (double)iters * (packed ? 2.0 : 1.0);
+    return GX_OK;
+}
 
 extern "C" int gx_ubench_fp32(int kind, int threads_per_block, int blocks_per_sm, int iters, double* ms, double* lane_ops) {
     if (kind < 0 || kind > 5 || threads_per_block < 32 || threads_per_block > 1024 || blocks_per_sm < 1 || iters < 1 || !ms ||
