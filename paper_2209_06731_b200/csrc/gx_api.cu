@@ -124,7 +124,8 @@ struct gx_grid {
     unsigned calls = 0;                         // number of gx_nonlinear_rhs calls issued (counter epoch)
     float2 *dgbuf = nullptr, *dphibuf = nullptr, *doutbuf = nullptr;   // for the *_host entry point: Hermite-block buffers each way
     unsigned* dcount_blk = nullptr;             // arrival counters of the block-wise evaluations of the *_host entry point
-    cudaStream_t st_in = nullptr, st_out = nullptr, st_cmp = nullptr;
+    cudaStream_t st_in = nullptr, st_out = nullptr, st_cmp = nullptr, st_lin = nullptr;
+    cudaEvent_t ev_phi = nullptr, ev_lin = nullptr;    // gx_rhs: linear terms on st_lin under the nonlinear kernels
     cudaEvent_t ev_user = nullptr;
     cudaGraphExec_t host_graph = nullptr;       // captured pipeline of the *_host entry point for the pointers below
     const void *hg_g = nullptr, *hg_phi = nullptr, *hg_out = nullptr;
@@ -286,6 +287,9 @@ int gx_grid_destroy(gx_grid* g) {
     if (g->host_graph) cudaGraphExecDestroy(g->host_graph);
     if (g->st_in) cudaStreamDestroy(g->st_in);
     if (g->st_cmp) cudaStreamDestroy(g->st_cmp);
+    if (g->st_lin) cudaStreamDestroy(g->st_lin);
+    if (g->ev_phi) cudaEventDestroy(g->ev_phi);
+    if (g->ev_lin) cudaEventDestroy(g->ev_lin);
     if (g->ev_user) cudaEventDestroy(g->ev_user);
     if (g->st_out) cudaStreamDestroy(g->st_out);
     cudaFree(g->dcount_blk);
@@ -469,7 +473,8 @@ namespace {
 // hold exactly those moments).  do_chi = false reuses the chi planes already in the workspace (same phi).
 // count / calls: arrival counters of the separate inverse-Laguerre kernel and their epoch.
 int nl_enqueue(gx_grid* g, NlParams p, int Nm_eff, bool do_chi, unsigned* count, unsigned* calls, cudaStream_t st,
-               cudaEvent_t* ev) {
+               cudaEvent_t* ev, cudaEvent_t before_out = nullptr) {
+    // before_out: event the stream waits for before the kernel that writes `out` (separate inverse-Laguerre kernel only)
     // calls == nullptr: the counters are zeroed by a memset node before the kernels and the target is J itself
     // (no epoch in the kernel arguments: the sequence can be captured in a CUDA graph and replayed)
     p.Nm = Nm_eff;
@@ -495,6 +500,7 @@ int nl_enqueue(gx_grid* g, NlParams p, int Nm_eff, bool do_chi, unsigned* count,
         const int nk = (int)g->nk;
         unsigned target = (unsigned)g->J;
         if (calls) { *calls += 1; target = *calls * (unsigned)g->J; }
+        if (before_out) GX_CUDA(g, cudaStreamWaitEvent(st, before_out, 0));
         cudaError_t e;
 #define GX_LAGINV(L, J)                                                                                        \
     e = (vec == 2) ? launch_pdl(gx::laguerre_inverse_kernel<L, J, 2>, grid, dim3(256), 0, st, p, nk, target)  \
@@ -755,13 +761,32 @@ int gx_rhs(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream) {
         return fail(g, GX_ERR_ARG, "gx_rhs: out must not alias g");
     if (misaligned(g_dev) || misaligned(out_dev)) return fail(g, GX_ERR_ARG, "gx_rhs: device pointers must be 16-byte aligned");
     if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_rhs: full geometry not set");
+    if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
     int rc;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
     if ((rc = gx_field_solve(g, g_dev, g->dphi_rhs, cuda_stream))) return rc;
-    if ((rc = gx_nonlinear_rhs(g, g_dev, g->dphi_rhs, out_dev, cuda_stream))) return rc;
-    cudaError_t e = gx::lin_rhs(g->lin, (const float2*)g_dev, g->dphi_rhs, (float2*)out_dev,
-                                /*accumulate=*/true, (cudaStream_t)cuda_stream);
+    const bool concurrent = !g->ks->fused_laguerre && !g->profile && std::getenv("GX_RHS_SERIAL") == nullptr;
+    if (!concurrent) {
+        if ((rc = gx_nonlinear_rhs(g, g_dev, g->dphi_rhs, out_dev, cuda_stream))) return rc;
+        cudaError_t e = gx::lin_rhs(g->lin, (const float2*)g_dev, g->dphi_rhs, (float2*)out_dev, /*accumulate=*/true, st);
+        if (e != cudaSuccess) return cuda_fail(g, e, "gx_rhs");
+        return GX_OK;
+    }
+    // The linear terms (memory-bound, they write out) run on a second stream under the chi and bracket kernels
+    // (FP32-bound, they do not touch out); the inverse-Laguerre kernel then adds -N on top.
+    if (!g->st_lin) {
+        GX_CUDA(g, cudaStreamCreateWithFlags(&g->st_lin, cudaStreamNonBlocking));
+        GX_CUDA(g, cudaEventCreateWithFlags(&g->ev_phi, cudaEventDisableTiming));
+        GX_CUDA(g, cudaEventCreateWithFlags(&g->ev_lin, cudaEventDisableTiming));
+    }
+    GX_CUDA(g, cudaEventRecord(g->ev_phi, st));
+    GX_CUDA(g, cudaStreamWaitEvent(g->st_lin, g->ev_phi, 0));
+    cudaError_t e = gx::lin_rhs(g->lin, (const float2*)g_dev, g->dphi_rhs, (float2*)out_dev, /*accumulate=*/false, g->st_lin);
     if (e != cudaSuccess) return cuda_fail(g, e, "gx_rhs");
-    return GX_OK;
+    GX_CUDA(g, cudaEventRecord(g->ev_lin, g->st_lin));
+    NlParams p = make_params(g, g_dev, g->dphi_rhs, out_dev);
+    p.accumulate = 1;
+    return nl_enqueue(g, p, g->Nm, true, g->dcount, &g->calls, st, nullptr, g->ev_lin);
 }
 
 int gx_ssprk3_step(gx_grid* g, void* g_dev, double dt, void* cuda_stream) {

@@ -83,6 +83,7 @@ struct NlParams {
     // electromagnetic evaluations (gx_nonlinear_rhs_em) hand the chi kernels ready-made spectral planes
     // chi_{s,z,j}(k): phi then holds one plane per unit (s,z,j) and M one shared plane of ones
     int phi_by_unit, M_shared;
+    int accumulate;       // inverse-Laguerre kernel: out += instead of out =
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -585,6 +586,12 @@ __global__ void __launch_bounds__(256) laguerre_inverse_kernel(const NlParams p,
                     for (int c = 0; c < 2 * VEC; ++c) acc[c] = fmaf(t, bj[c], acc[c]);
                 }
             V* dst = reinterpret_cast<V*>(p.out + (((size_t)(s * p.Nm + m) * p.Nl + l) * p.Nz + z) * nk) + kv;
+            if (p.accumulate) {                      // gx_rhs: the linear terms are already in out (written concurrently)
+                const V prev = *dst;
+                const float* pv = reinterpret_cast<const float*>(&prev);
+#pragma unroll
+                for (int c = 0; c < 2 * VEC; ++c) acc[c] += pv[c];
+            }
             *dst = *reinterpret_cast<V*>(acc);
         }
     }
