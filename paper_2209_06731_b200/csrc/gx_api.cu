@@ -120,6 +120,12 @@ struct gx_grid {
     float2 *dchis = nullptr, *dg_em = nullptr, *dout_em = nullptr;
     float2 *dtwx = nullptr, *dtwy = nullptr, *ddchi = nullptr, *dbhat = nullptr;
     unsigned* dcount = nullptr;
+    int chi_buf = 0;                            // dchi buffer of the current chi planes
+    unsigned* ddone = nullptr;                  // chained calls: bracket units that have finished reading dchi (all calls)
+    unsigned* dchi_ready = nullptr;             // chained calls: [2][s][z][j] epoch of the call that wrote the chi plane
+    bool chi_chained = false;                   // the current chi planes were written by a chained call (flags valid)
+    unsigned chi_epoch = 0;                     // epoch of the chained call that wrote the current chi planes
+    unsigned done_total = 0, done_at_chi = 0;   // its value once every chained call so far is done / just before the latest call with new chi planes
     unsigned* dchi_flag = nullptr;              // [s][z][j] epoch of the last call that produced the chi plane (persistent family)
     unsigned calls = 0;                         // number of gx_nonlinear_rhs calls issued (counter epoch)
     float2 *dgbuf = nullptr, *dphibuf = nullptr, *doutbuf = nullptr;   // for the *_host entry point: Hermite-block buffers each way
@@ -267,10 +273,14 @@ int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out
 
     const size_t szj = (size_t)Ns * Nz * g->J;
     if ((rc = dev_alloc(g, &g->dM, szj * g->nk))) return rc;
-    if ((rc = dev_alloc(g, &g->ddchi, szj * Nx * Ny))) return rc;
+    if ((rc = dev_alloc(g, &g->ddchi, 2 * szj * Nx * Ny))) return rc;     // two buffers: chi of call N+1 under the tail of call N
     if ((rc = dev_alloc(g, &g->dbhat, szj * Nm * g->nk))) return rc;
     if ((rc = dev_alloc(g, &g->dcount, (size_t)Ns * Nm * Nz))) return rc;
     GX_CUDA(g, cudaMemset(g->dcount, 0, (size_t)Ns * Nm * Nz * sizeof(unsigned)));
+    if ((rc = dev_alloc(g, &g->dchi_ready, 2 * szj))) return rc;
+    GX_CUDA(g, cudaMemset(g->dchi_ready, 0, 2 * szj * sizeof(unsigned)));
+    if ((rc = dev_alloc(g, &g->ddone, 4))) return rc;
+    GX_CUDA(g, cudaMemset(g->ddone, 0, 4 * sizeof(unsigned)));
     if ((rc = dev_alloc(g, &g->dchi_flag, szj))) return rc;
     GX_CUDA(g, cudaMemset(g->dchi_flag, 0, szj * sizeof(unsigned)));
     return GX_OK;
@@ -280,7 +290,7 @@ int gx_grid_destroy(gx_grid* g) {
     if (!g) return GX_ERR_ARG;
     cudaFree(g->dT); cudaFree(g->dTinv); cudaFree(g->dM); cudaFree(g->dMB); cudaFree(g->dones); cudaFree(g->dkp2);
     cudaFree(g->dbmag2); cudaFree(g->dchis); cudaFree(g->dg_em); cudaFree(g->dout_em); cudaFree(g->dtwx); cudaFree(g->dtwy);
-    cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dcount); cudaFree(g->dchi_flag); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
+    cudaFree(g->ddchi); cudaFree(g->dbhat); cudaFree(g->dcount); cudaFree(g->ddone); cudaFree(g->dchi_ready); cudaFree(g->dchi_flag); cudaFree(g->dgbuf); cudaFree(g->dphibuf); cudaFree(g->doutbuf);
     cudaFree(g->dphi_rhs); cudaFree(g->drk_y); cudaFree(g->drk_k);
     for (auto e : g->ev_pool) cudaEventDestroy(e);
     for (auto e : g->ev_host) cudaEventDestroy(e);
@@ -480,6 +490,15 @@ int nl_enqueue(gx_grid* g, NlParams p, int Nm_eff, bool do_chi, unsigned* count,
     p.Nm = Nm_eff;
     p.count = count;
     const int szj = g->Ns * g->Nz * g->J;
+    if (do_chi) g->chi_buf ^= 1;
+    p.dchi = g->ddchi + (size_t)g->chi_buf * szj * g->Nx * g->Ny;
+    // a8 inside the bracket kernel (last node unit of an (s,m,z) to arrive) unless out already holds the linear terms
+    const bool fuse_a8 = g->ks->closer && g->J <= 5 && g->Nl <= 4 && !before_out && !p.accumulate && std::getenv("GX_A8_KERNEL") == nullptr;
+    p.ZG = 1;
+    if (fuse_a8)                               // spacing between the J node units of an (s,m,z): only the closer needs it
+        for (int c = 2; c <= 4; ++c)
+            if (g->Nz % c == 0) p.ZG = c;
+    if (const char* e = std::getenv("GX_ZG")) { const int c = std::atoi(e); if (c >= 1 && g->Nz % c == 0) p.ZG = c; }
     if (!calls && !g->ks->fused_laguerre)
         GX_CUDA(g, cudaMemsetAsync(count, 0, (size_t)g->Ns * Nm_eff * g->Nz * sizeof(unsigned), st));
     if (g->ks->launch_call) {
@@ -489,17 +508,39 @@ int nl_enqueue(gx_grid* g, NlParams p, int Nm_eff, bool do_chi, unsigned* count,
         if (ev) { GX_CUDA(g, cudaEventRecord(ev[2], st)); GX_CUDA(g, cudaEventRecord(ev[3], st)); }
         return GX_OK;
     }
-    if (do_chi) GX_CUDA(g, g->ks->launch_chi(p, szj, st));
+    // Outside graph capture (calls != nullptr) the chi grid carries the PDL attribute: after a call whose last kernel
+    // is the bracket grid it starts while that grid's last wave still runs.  A foreign kernel in front of it never
+    // triggers early, so phi / g written by the caller's own kernels are complete before the chi grid starts.
+    unsigned target = (unsigned)g->J;
+    if (!g->ks->fused_laguerre && calls) { *calls += 1; target = *calls * (unsigned)g->J; }
+    p.a8_target = fuse_a8 ? target : 0u;
+    // (a call that reuses chi planes is chained only if the chained flags describe those planes)
+    // Calls with the separate inverse-Laguerre kernel (gx_rhs) are not chained: that kernel never triggers early.
+    const bool chained = calls && fuse_a8 && g->ks->launch_chi_pdl && std::getenv("GX_CHI_SERIAL") == nullptr && (do_chi || g->chi_chained);
+    if (do_chi) g->chi_chained = chained;
+    if (chained) {
+        // Counters instead of grid-completion order (nl_row_kernels.cuh): the chi grid of this call writes the dchi
+        // buffer that was read by the calls before the latest one with new chi planes; all their units have left the
+        // row phase once done reaches the total recorded just before that call (wrap-safe sequence arithmetic).
+        p.done = g->ddone;
+        if (do_chi) { p.chi_need = g->done_at_chi; g->done_at_chi = g->done_total; g->chi_epoch = *calls; }
+        g->done_total += (unsigned)(szj * Nm_eff);
+        p.chi_ready = g->dchi_ready + (size_t)g->chi_buf * szj;
+        p.chi_epoch = g->chi_epoch;
+    }
+    if (do_chi) {
+        auto chi = !chained ? g->ks->launch_chi
+                            : (std::getenv("GX_CHI_WIDE") && g->ks->launch_chi_pdl_wide ? g->ks->launch_chi_pdl_wide : g->ks->launch_chi_pdl);
+        GX_CUDA(g, chi(p, szj, st));
+    }
     if (ev) GX_CUDA(g, cudaEventRecord(ev[1], st));
     GX_CUDA(g, g->ks->launch_bracket(p, szj * Nm_eff, st));
     if (ev) GX_CUDA(g, cudaEventRecord(ev[2], st));
-    if (!g->ks->fused_laguerre) {
+    if (!g->ks->fused_laguerre && !fuse_a8) {
         const int vec = (g->nk % 2 == 0) ? 2 : 1;
         const int nkv = (int)(g->nk / vec);
         dim3 grid((unsigned)((nkv + 255) / 256), (unsigned)(g->Ns * Nm_eff * g->Nz));
         const int nk = (int)g->nk;
-        unsigned target = (unsigned)g->J;
-        if (calls) { *calls += 1; target = *calls * (unsigned)g->J; }
         if (before_out) GX_CUDA(g, cudaStreamWaitEvent(st, before_out, 0));
         cudaError_t e;
 #define GX_LAGINV(L, J)                                                                                        \

@@ -21,6 +21,12 @@ struct KernelSet {
     bool fused_laguerre;   // the bracket kernel writes `out` itself (a8 fused): no third launch
     // one persistent kernel for the whole call (chi planes + bracket units + a8); launch_chi/bracket unused then
     cudaError_t (*launch_call)(const NlParams&, unsigned* chi_flag, unsigned epoch, int n_items, cudaStream_t);
+    // the bracket kernel can do a8 itself in the CTA that completes an (s,m,z) (NlParams::a8_target != 0)
+    bool closer = false;
+    // chi launcher with the PDL attribute: the chi planes of call N+1 start under the tail of call N (other dchi buffer)
+    // (bracket-sized CTAs: they fit next to the bracket CTAs of the previous call's last wave)
+    cudaError_t (*launch_chi_pdl)(const NlParams&, int units, cudaStream_t) = nullptr;
+    cudaError_t (*launch_chi_pdl_wide)(const NlParams&, int units, cudaStream_t) = nullptr;   // same, launch_chi's CTA shape
 };
 
 // Launch with the programmatic-stream-serialization attribute (PDL): the grid may begin before the

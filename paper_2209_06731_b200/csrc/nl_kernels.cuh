@@ -66,6 +66,20 @@ struct PlaneCfg {
     static_assert(SMEM_BYTES <= 232448, "plane does not fit in shared memory");
 };
 
+// Arrival on a counter with release semantics (everything this thread has observed, including the other threads'
+// stores ordered before it by a CTA barrier, is visible to whoever acquires the new value).  Unlike
+// __threadfence() + atomicAdd the thread does not wait for its stores to be acknowledged: it can exit at once.
+__device__ __forceinline__ void arrive_release(unsigned* counter) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(counter) : "memory");
+}
+
+// Thread context of a phase function: the whole CTA.  (A two-units-per-CTA variant with one named barrier per
+// group was measured in round 2: 67.5 against 57.3 us.)
+struct CtaSync {
+    __device__ __forceinline__ int tid() const { return (int)threadIdx.x; }
+    __device__ __forceinline__ void sync() const { __syncthreads(); }
+};
+
 struct NlParams {
     const float2* g;      // [s][m][l][z][kx][ky]
     const float2* phi;    // [z][kx][ky]
@@ -84,6 +98,14 @@ struct NlParams {
     // chi_{s,z,j}(k): phi then holds one plane per unit (s,z,j) and M one shared plane of ones
     int phi_by_unit, M_shared;
     int accumulate;       // inverse-Laguerre kernel: out += instead of out =
+    unsigned a8_target;   // != 0 (row family): the node unit j = J-1 does a8 itself once count == a8_target - 1 (no third kernel)
+    int ZG;               // row family: z values per block group of the unit order (divides Nz)
+    // chained calls (row family, gx_api.cu nl_enqueue): `done` counts the bracket units, over all calls, that have
+    // finished reading dchi; the chi grid of a call may overwrite its dchi buffer once done >= chi_need
+    unsigned* done;
+    unsigned chi_need;
+    unsigned* chi_ready;  // chained calls: [s][z][j] of the current dchi buffer, epoch of the call that wrote the plane
+    unsigned chi_epoch;
 };
 
 // ------------------------------------------------------------------------------------------------
@@ -93,13 +115,13 @@ struct NlParams {
 // kx >= 0, always kept with kx < 0, always padding, or decided by n2 at run time (at most two n1).
 // For column q < 0 the reality condition gives f(a,q) = conj f(-a,-q): row index and the sign of the
 // imaginary part flip, which keeps every address of the form base + compile-time offset.
-template <class C, bool GLOBAL_F>
+template <class C, bool GLOBAL_F, class SY = CtaSync>
 __device__ __forceinline__ void x_inverse(float2* __restrict__ W, const float2* __restrict__ twx,
-                                          float dkx, float dky, const float2* __restrict__ F) {
+                                          float dkx, float dky, const float2* __restrict__ F, const SY sy = SY()) {
     constexpr int NX = C::NX, K = C::K, NCOL = C::NCOL, NAKY = C::NAKY, NAKX = C::NAKX;
     constexpr int R1 = C::RX1, R2 = C::RX2;
     // pass 1: for each (n2, column): DFT_R1 over n1 of input n = n1*R2+n2, twiddle, in-place slot
-    for (int t = threadIdx.x; t < R2 * NCOL; t += C::NT) {
+    for (int t = sy.tid(); t < R2 * NCOL; t += C::NT) {
         const int n2 = t / NCOL, c = t - n2 * NCOL;
         const bool neg = c >= NAKY;                       // column q < 0
         const int qa = neg ? NCOL - c : c;                // |q|
@@ -148,9 +170,9 @@ __device__ __forceinline__ void x_inverse(float2* __restrict__ W, const float2* 
         for (int k1 = 0; k1 < R1; ++k1)
             W[(k1 * R2 + n2) * NCOL + c] = k1 == 0 ? v[0] : cmul(v[k1], twx[n2 * k1]);
     }
-    __syncthreads();
+    sy.sync();
     // pass 2: for each (k1, column): DFT_R2 over n2; position k1*R2+k2 <- x = k1 + R1*k2
-    for (int t = threadIdx.x; t < R1 * NCOL; t += C::NT) {
+    for (int t = sy.tid(); t < R1 * NCOL; t += C::NT) {
         const int k1 = t / NCOL, c = t - k1 * NCOL;
         float2 v[R2];
 #pragma unroll
@@ -159,7 +181,7 @@ __device__ __forceinline__ void x_inverse(float2* __restrict__ W, const float2* 
 #pragma unroll
         for (int k2 = 0; k2 < R2; ++k2) W[(k1 * R2 + k2) * NCOL + c] = v[k2];
     }
-    __syncthreads();
+    sy.sync();
 }
 
 template <class C>
@@ -200,12 +222,12 @@ __device__ __forceinline__ void y_inverse_pass1(const float2* __restrict__ W, fl
 
 // forward x transform on the naky kept columns; W holds Bhat(x, q) at permuted x positions.
 // Writes the 2K+1 kept kx rows (compact order) times `scale` to out[i*NAKY + q].
-template <class C>
+template <class C, class SY = CtaSync>
 __device__ __forceinline__ void x_forward(float2* __restrict__ W, const float2* __restrict__ twx,
-                                          float2* __restrict__ out, float scale) {
+                                          float2* __restrict__ out, float scale, const SY sy = SY()) {
     constexpr int NX = C::NX, K = C::K, NCOL = C::NCOL, NAKY = C::NAKY, NAKX = C::NAKX;
     constexpr int R1 = C::RX1, R2 = C::RX2;
-    for (int t = threadIdx.x; t < R1 * NAKY; t += C::NT) {
+    for (int t = sy.tid(); t < R1 * NAKY; t += C::NT) {
         const int a = t / NAKY, q = t - a * NAKY;
         float2 v[R2];
 #pragma unroll
@@ -215,8 +237,8 @@ __device__ __forceinline__ void x_forward(float2* __restrict__ W, const float2* 
         for (int d = 0; d < R2; ++d)
             W[(a * R2 + d) * NCOL + q] = d == 0 ? v[0] : cmul_conj(v[d], twx[a * d]);
     }
-    __syncthreads();
-    for (int t = threadIdx.x; t < R2 * NAKY; t += C::NT) {
+    sy.sync();
+    for (int t = sy.tid(); t < R2 * NAKY; t += C::NT) {
         const int d = t / NAKY, q = t - d * NAKY;
         float2 v[R1];
 #pragma unroll
@@ -303,22 +325,24 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, unsigned by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-template <class C>
+template <class C, class SY = CtaSync>
 __device__ __forceinline__ void stage_combine_tma(float2* __restrict__ raw, float2* __restrict__ S,
                                                   unsigned long long* bar, unsigned& parity,
                                                   const float2* __restrict__ planes,
-                                                  size_t lstride, const float* __restrict__ coef, int Nl) {
+                                                  size_t lstride, const float* __restrict__ coef, int Nl,
+                                                  const SY sy = SY()) {
     constexpr int NK = C::NK, NT = C::NT, NK2 = NK / 2;
     constexpr int CAP = (C::W_ELEMS + C::S_ELEMS) / NK;          // planes per chunk
     constexpr int PER = (NK2 + NT - 1) / NT;                     // float4 (2 complex) per thread
+    const int tid = sy.tid();
     static_assert(CAP >= 1 && NK % 2 == 0, "TMA staging needs 16-byte planes that fit");
-    const float4* __restrict__ raw4 = reinterpret_cast<const float4*>(raw) + threadIdx.x;
+    const float4* __restrict__ raw4 = reinterpret_cast<const float4*>(raw) + tid;
     float4 acc[PER];
 #pragma unroll
     for (int u = 0; u < PER; ++u) acc[u] = make_float4(0.f, 0.f, 0.f, 0.f);
     for (int l0 = 0; l0 < Nl; l0 += CAP) {
         const int nl = min(CAP, Nl - l0);
-        if (threadIdx.x == 0) {
+        if (tid == 0) {
             asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
             mbar_expect_tx(bar, (unsigned)(nl * NK * sizeof(float2)));
             for (int l = 0; l < nl; ++l)
@@ -331,7 +355,7 @@ __device__ __forceinline__ void stage_combine_tma(float2* __restrict__ raw, floa
             const float4* __restrict__ src = raw4 + l * NK2;
 #pragma unroll
             for (int u = 0; u < PER; ++u) {
-                if ((u + 1) * NT <= NK2 || (int)threadIdx.x + u * NT < NK2) {
+                if ((u + 1) * NT <= NK2 || tid + u * NT < NK2) {
                     const float4 f = src[u * NT];
                     acc[u].x = fmaf(t, f.x, acc[u].x);
                     acc[u].y = fmaf(t, f.y, acc[u].y);
@@ -340,12 +364,12 @@ __device__ __forceinline__ void stage_combine_tma(float2* __restrict__ raw, floa
                 }
             }
         }
-        __syncthreads();                                         // raw region consumed
+        sy.sync();                                             // raw region consumed
     }
-    float4* __restrict__ S4 = reinterpret_cast<float4*>(S) + threadIdx.x;
+    float4* __restrict__ S4 = reinterpret_cast<float4*>(S) + tid;
 #pragma unroll
     for (int u = 0; u < PER; ++u)
-        if ((u + 1) * NT <= NK2 || (int)threadIdx.x + u * NT < NK2) S4[u * NT] = acc[u];
+        if ((u + 1) * NT <= NK2 || tid + u * NT < NK2) S4[u * NT] = acc[u];
 }
 
 template <class C>
@@ -540,7 +564,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
     // ---- publish: this node's Bhat plane is complete (release: stores -> barrier -> fence -> atomic).
     // The inverse-Laguerre grid, already resident under PDL, waits per (s,m,z) on this counter.
     __syncthreads();                 // orders every thread's stores before thread 0's gpu-scope fence (cumulative)
-    if (threadIdx.x == 0) { __threadfence(); atomicAdd(p.count + (s * p.Nm + m) * p.Nz + z, 1u); }
+    if (threadIdx.x == 0) arrive_release(p.count + (s * p.Nm + m) * p.Nz + z);
 }
 
 // ================================================================================================

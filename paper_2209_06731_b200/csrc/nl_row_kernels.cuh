@@ -20,6 +20,20 @@
 
 namespace gx {
 
+// Development builds (-DGX_PHASE_TIMING): %globaltimer at the phase boundaries of EVERY bracket CTA (slot 7: SM id),
+// read back with gx_debug_cta_log(): the timeline of a whole launch (waves, tail, closers).
+#ifdef GX_PHASE_TIMING
+static __device__ long long gx_cta_log[4 * 8192 * 16];     // [call & 3][block][slot]
+static __device__ long long gx_chi_log[4 * 256 * 4];        // [call & 3][block][start, before the done wait, after it, end]
+__device__ __forceinline__ long long gx_globaltimer() { long long t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
+__device__ __forceinline__ long long gx_smid() { unsigned s; asm volatile("mov.u32 %0, %%smid;" : "=r"(s)); return (long long)s; }
+#define GX_CTA(i) do { if (threadIdx.x == 0 && blockIdx.x < 8192) gx_cta_log[(((p.a8_target / (unsigned)p.J) & 3u) * 8192 + blockIdx.x) * 16 + (i)] = (i) == 7 ? gx_smid() : gx_globaltimer(); } while (0)
+#define GX_CHI(i) do { if (threadIdx.x == 0 && blockIdx.x < 256) gx_chi_log[(((p.a8_target / (unsigned)p.J) & 3u) * 256 + blockIdx.x) * 4 + (i)] = gx_globaltimer(); } while (0)
+#else
+#define GX_CTA(i) do { } while (0)
+#define GX_CHI(i) do { } while (0)
+#endif
+
 template <int NX_, int NY_, int RX1_, int RX2_, int NT_, int MINB_>
 struct RowCfg {
     static constexpr int NX = NX_, NY = NY_, RX1 = RX1_, RX2 = RX2_, NT = NT_, MINB = MINB_;
@@ -94,6 +108,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_row_kernel(const Nl
     const float2* __restrict__ phi = p.phi + (size_t)(p.phi_by_unit ? unit : z) * C::NK;
     const float* __restrict__ M = p.M + (size_t)(p.M_shared ? 0 : unit) * C::NK;
     pdl_launch_dependents();
+    GX_CHI(0);
     for (int i = threadIdx.x; i < C::NX; i += C::NT) twx[i] = p.twx[i];
     for (int i = threadIdx.x; i < C::NK; i += C::NT) {
         const float2 f = __ldg(phi + i);
@@ -102,6 +117,22 @@ __global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_row_kernel(const Nl
     }
     __syncthreads();
     x_inverse<C, false>(W, twx, p.dkx, p.dky, S);
+    GX_CHI(1);
+    if (p.done) {
+        // Launched with the PDL attribute, this grid starts under the tail of the previous call's bracket grid.  It
+        // writes the dchi buffer that the call BEFORE the previous one read: wait until all of that call's units
+        // have left their row phase (normally long ago; x_inverse above ends with a CTA barrier, the one below
+        // publishes thread 0's observation).
+        if (threadIdx.x == 0) {
+            unsigned c;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(c) : "l"(p.done) : "memory");
+                if ((int)(c - p.chi_need) < 0) __nanosleep(200);
+            } while ((int)(c - p.chi_need) < 0);
+        }
+        __syncthreads();
+    }
+    GX_CHI(2);
     float2* __restrict__ dchi = p.dchi + (size_t)unit * C::NX * C::NY;
     for (int row = threadIdx.x; row < C::NX; row += C::NT) {
         float2 v[64];
@@ -109,49 +140,174 @@ __global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_row_kernel(const Nl
 #pragma unroll
         for (int y = 0; y < 64; ++y) dchi[y * C::NX + row] = v[y];
     }
+    // Unchained launches keep the transitive order "bracket N+1 past its pdl_wait => chi N+1 complete => call N
+    // complete"; chained ones (p.done) order the reuse of dchi, bhat and out through counters instead, so that the
+    // next call's units can run under this call's tail.
+    if (!p.done) pdl_wait();
+    else {
+        // chained: publish this plane (release: stores -> barrier -> release store of the flag); its bracket units wait for the
+        // flag, not for the whole grid
+        __syncthreads();
+        if (threadIdx.x == 0)
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.chi_ready + unit), "r"(p.chi_epoch) : "memory");
+    }
+    GX_CHI(3);
 }
 
-// ================================================================================================
-// a2-a7 for one (s,m,z,j): Bhat_j(k) = F_k[ d_y chi d_x gt - d_x chi d_y gt ], 2/3-rule truncated.
-template <class C>
-__global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlParams p) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    float2* W = reinterpret_cast<float2*>(smem_raw);
-    float2* S = W + C::W_ELEMS;
-    float2* twx = S + C::S_ELEMS;
-    constexpr int NX = C::NX, NY = C::NY, NK = C::NK;
+// a8 by the LAST node unit (j = J-1) of an (s,m,z), after its own plane is in bhat like everyone else's:
+// out_l = - sum_j Tinv[l][j] Bhat_j.  The J-1 other node units were dispatched earlier (lower block indices); thread 0
+// waits for their arrivals and fetches min(J, CAP) node planes with bulk copies into the (now free) W + S region, a
+// last plane comes through registers.  Deliberately small, rolled code: it runs in one CTA out of J, so its
+// instructions are cold in the instruction cache (a fully unrolled fused variant spent 7 us per closer on fetches).
+// J <= CAP + 1 and Nl <= 4 (the host falls back to the separate inverse-Laguerre kernel otherwise).
+template <class C, class SY>
+__device__ __noinline__ void closer_sum(float2* __restrict__ raw, const float2* bh, const size_t jstride, float2* __restrict__ out0,
+                                        const size_t lstride, const float* __restrict__ Tinv, const int J, const int Nl,
+                                        const unsigned* cnt, const unsigned want, unsigned long long* bar, const unsigned parity,
+                                        const SY sy, const NlParams& p) {
+    constexpr int NK = C::NK, NK2 = NK / 2, NT = C::NT;
+    constexpr int CAP = (C::W_ELEMS + C::S_ELEMS) / NK;
+    __shared__ float Tsm[4 * 8];              // -Tinv[l][j] (out = -N), zero-padded to [4][8]
+    const int tid = sy.tid();
+    if (tid < 32) {
+        const int l = tid >> 3, jn = tid & 7;
+        Tsm[tid] = (l < Nl && jn < J) ? -__ldg(Tinv + l * J + jn) : 0.f;
+    }
+    const int nt = min(J, CAP);
+    // plane CAP (this unit's own plane when J = CAP + 1) through registers, requested first: the round trip to L2
+    // (about 1 us under this kernel's load) passes while thread 0 waits and the bulk copies arrive
+    constexpr int PER = (NK2 + NT - 1) / NT;
+    float4 e[PER];
+    {
+        const float4* last4 = reinterpret_cast<const float4*>(bh + (size_t)CAP * jstride) + tid;
+#pragma unroll
+        for (int u = 0; u < PER; ++u)
+            e[u] = (J > CAP && tid + u * NT < NK2) ? __ldcg(last4 + u * NT) : make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    GX_CTA(8);
+    if (tid == 0) {
+        unsigned c;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(c) : "l"(cnt) : "memory");
+            if (c != want) __nanosleep(64);
+        } while (c != want);
+        GX_CTA(9);
+        // the bulk copies (async proxy) read what other CTAs stored through the generic proxy; W + S were last
+        // touched through the generic proxy by this CTA (x_forward, ordered by the barrier before this call)
+        if (J <= CAP) __threadfence();        // this unit's own plane is among the copied ones
+        asm volatile("fence.proxy.async;" ::: "memory");
+        mbar_expect_tx(bar, (unsigned)(nt * NK * sizeof(float2)));
+        for (int jn = 0; jn < nt; ++jn) bulk_g2s(raw + jn * NK, bh + jn * jstride, NK * sizeof(float2), bar);
+    }
+    sy.sync();                                // thread 0's acquire reaches everyone; Tsm complete
+    GX_CTA(10);
+    mbar_wait(bar, parity);
+    GX_CTA(11);
+    const float4* __restrict__ raw4 = reinterpret_cast<const float4*>(raw) + tid;
+    float4* out4 = reinterpret_cast<float4*>(out0) + tid;
+    const size_t lstride4 = lstride / 2;
+#pragma unroll
+    for (int u = 0; u < PER; ++u) {
+        if (tid + u * NT < NK2) {
+            float4 acc[4];
+#pragma unroll
+            for (int l = 0; l < 4; ++l) {
+                const float t = Tsm[l * 8 + CAP];
+                acc[l] = make_float4(t * e[u].x, t * e[u].y, t * e[u].z, t * e[u].w);
+            }
+#pragma unroll
+            for (int jn = 0; jn < CAP; ++jn) {
+                if (jn < nt) {
+                    const float4 b = raw4[jn * NK2 + u * NT];
+#pragma unroll
+                    for (int l = 0; l < 4; ++l) {
+                        const float t = Tsm[l * 8 + jn];
+                        acc[l].x = fmaf(t, b.x, acc[l].x);
+                        acc[l].y = fmaf(t, b.y, acc[l].y);
+                        acc[l].z = fmaf(t, b.z, acc[l].z);
+                        acc[l].w = fmaf(t, b.w, acc[l].w);
+                    }
+                }
+            }
+#pragma unroll
+            for (int l = 0; l < 4; ++l)
+                if (l < Nl) out4[l * lstride4 + u * NT] = acc[l];
+        }
+    }
+    GX_CTA(12);
+}
 
-    const int unit = blockIdx.x;                 // ((s*Nz + z)*J + j)*Nm + m
-    const int m = unit % p.Nm;
-    const int szj = unit / p.Nm;
-    const int j = szj % p.J;
-    const int z = (szj / p.J) % p.Nz;
-    const int s = szj / (p.J * p.Nz);
+// unit = (((s*(Nz/ZG) + zg)*J + j)*ZG + zi)*Nm + m, z = zg*ZG + zi: the Nm units that share a chi plane stay
+// neighbours, the J node units of one (s,m,z) lie ZG*Nm blocks apart (the last one, which does a8 in fused calls,
+// starts late enough to find most of the other planes complete)
+struct UnitIdx { int s, m, z, j, szj; };
+__device__ __forceinline__ UnitIdx decode_unit(const NlParams& p, const int unit) {
+    UnitIdx ix;
+    ix.m = unit % p.Nm;
+    int r = unit / p.Nm;
+    const int zi = r % p.ZG; r /= p.ZG;
+    ix.j = r % p.J; r /= p.J;
+    ix.z = (r % (p.Nz / p.ZG)) * p.ZG + zi;
+    ix.s = r / (p.Nz / p.ZG);
+    ix.szj = (ix.s * p.Nz + ix.z) * p.J + ix.j;
+    return ix;
+}
+
+template <class C, class SY, bool CHAIN>
+__device__ __forceinline__ void bracket_row_unit(const NlParams& p, const int unit, float2* __restrict__ W,
+                                                 float2* __restrict__ S, const float2* __restrict__ twx,
+                                                 unsigned long long* stage_bar, float* Tsh, const SY sy) {
+    constexpr int NX = C::NX, NY = C::NY, NK = C::NK;
+    const int tid = sy.tid();
+    const UnitIdx ix = decode_unit(p, unit);
+    const int s = ix.s, m = ix.m, z = ix.z, j = ix.j, szj = ix.szj;
     const size_t lstride = (size_t)p.Nz * NK;
     const float2* __restrict__ g0 = p.g + ((size_t)(s * p.Nm + m) * p.Nl * p.Nz + z) * NK;
 
-    __shared__ unsigned long long stage_bar;
-    __shared__ float Tsh[16];
     unsigned bar_parity = 0;
-    GX_PHASE(0);
-    if (threadIdx.x == 0) mbar_init(&stage_bar, 1);
-    if (threadIdx.x < p.Nl) Tsh[threadIdx.x] = __ldg(p.T + j * p.Nl + threadIdx.x);
-    __syncthreads();
+    GX_CTA(0);
+    GX_CTA(7);
+    // The next grid in the stream may be scheduled as soon as every CTA of this one has started: the separate
+    // inverse-Laguerre grid (waits on the arrival counters) or, in chained calls, the chi grid of the NEXT call
+    // (reuse of dchi / bhat / out is ordered by the counters below, not by grid completion).
     pdl_launch_dependents();
-    for (int i = threadIdx.x; i < NX; i += C::NT) twx[i] = p.twx[i];
+    __shared__ unsigned slot_seen;                    // (kept in shared memory: no register lives across the row phase)
+    if (CHAIN && p.done && p.a8_target != 0u && tid == 0) {    // requested now, looked at before x_forward (latency hidden)
+        unsigned c;
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(c) : "l"(p.count + (s * p.Nm + m) * p.Nz + z) : "memory");
+        slot_seen = c;
+    }
+    unsigned chi_seen = 0;
+    if (CHAIN && p.done && tid == 0)                           // same for the flag of this unit's chi plane
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(chi_seen) : "l"(p.chi_ready + szj) : "memory");
+    if (tid == 0) mbar_init(stage_bar, 1);
+    if (tid < p.Nl) Tsh[tid] = __ldg(p.T + j * p.Nl + tid);
+    sy.sync();
     // ---- a2: forward Laguerre transform l -> node j, fused into the TMA-staged load
-    stage_combine_tma<C>(W, S, &stage_bar, bar_parity, g0, lstride, Tsh, p.Nl);
-    __syncthreads();
-    GX_PHASE(1);
+    stage_combine_tma<C, SY>(W, S, stage_bar, bar_parity, g0, lstride, Tsh, p.Nl, sy);
+    sy.sync();
+    GX_CTA(1);
     // ---- a3 + a4 (x part)
-    x_inverse<C, false>(W, twx, p.dkx, p.dky, S);
-    GX_PHASE(2);
+    x_inverse<C, false, SY>(W, twx, p.dkx, p.dky, S, sy);
+    GX_CTA(2);
 
     const float2* dchi = p.dchi + (size_t)szj * NX * NY;
-    pdl_wait();                     // chi planes of this call are complete and visible from here on
-    GX_PHASE(3);
+    if (!CHAIN || !p.done) pdl_wait();        // chi planes of this call are complete and visible from here on
+    else {
+        // chained: every chi CTA of this call is resident (this grid is scheduled after all of them have started);
+        // wait for this unit's own plane only
+        if (tid == 0) {
+            unsigned c = chi_seen;
+            while (c != p.chi_epoch) {
+                __nanosleep(100);
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(c) : "l"(p.chi_ready + szj) : "memory");
+            }
+        }
+        sy.sync();
+    }
+    GX_CTA(3);
     // ---- a4 (y part) + a5 + a6 (y part) + a7 (ky), one x row per thread, all in registers
-    for (int row = threadIdx.x; row < NX; row += C::NT) {
+    for (int row = tid; row < NX; row += C::NT) {
         float2* __restrict__ Wr = W + row * C::NCOL;
         const float2* dc = dchi + row;     // written by the chi grid that overlaps this one (PDL): coherent loads after pdl_wait
         // chi pairs of the first output group are requested before the transform starts, those of group
@@ -198,15 +354,58 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
         }
         row_forward_real<C>(Wr, b);
     }
-    __syncthreads();
-    GX_PHASE(4);
+    sy.sync();
+    GX_CTA(4);
+    // the row phase needs every register: nothing but blockIdx is carried across it, the indices are formed again
+    int unit2 = unit;
+    if (CHAIN) asm volatile("" : "+r"(unit2));
+    const UnitIdx iy = CHAIN ? decode_unit(p, unit2) : ix;
+    unsigned* cnt = p.count + (iy.s * p.Nm + iy.m) * p.Nz + iy.z;
+    if (CHAIN && p.done && tid == 0) {
+        atomicAdd(p.done, 1u);          // this unit has read its chi pairs (values consumed before the barrier above)
+        if (p.a8_target != 0u) {
+            // chained calls: the previous call's closer of this (s,m,z) must have read the bhat slots (and written
+            // out) before this call overwrites them; its last action is the arrival that completes count
+            unsigned c = slot_seen;
+            while ((int)(c - (p.a8_target - (unsigned)p.J)) < 0) {
+                __nanosleep(100);
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(c) : "l"(cnt) : "memory");
+            }
+        }
+    }
     // ---- a6 (x part) + a7 (keep |kx| <= K)
-    x_forward<C>(W, twx, p.bhat + (size_t)unit * NK, p.scale);
+    x_forward<C, SY>(W, twx, p.bhat + ((size_t)iy.szj * p.Nm + iy.m) * NK, p.scale, sy);
 
     // ---- publish (see bracket_kernel)
-    __syncthreads();
-    GX_PHASE(5);
-    if (threadIdx.x == 0) { __threadfence(); atomicAdd(p.count + (s * p.Nm + m) * p.Nz + z, 1u); }
+    sy.sync();
+    GX_CTA(5);
+    if (CHAIN && p.a8_target != 0u && iy.j == p.J - 1) {
+        // ---- a8: this unit closes its (s,m,z); its own plane is read back with the others
+        closer_sum<C, SY>(W, p.bhat + ((size_t)((iy.s * p.Nz + iy.z) * p.J) * p.Nm + iy.m) * NK, (size_t)p.Nm * NK,
+                          p.out + (((size_t)(iy.s * p.Nm + iy.m) * p.Nl) * p.Nz + iy.z) * NK, (size_t)p.Nz * NK, p.Tinv, p.J, p.Nl,
+                          cnt, p.a8_target - 1u, stage_bar, bar_parity, sy, p);
+        sy.sync();
+        if (tid == 0) arrive_release(cnt);     // completes the epoch (+J per call): out is written, bhat read
+        GX_CTA(6);
+        return;
+    }
+    if (tid == 0) arrive_release(cnt);
+    GX_CTA(6);
+}
+
+// CHAIN = false: the plain kernel (separate inverse-Laguerre grid, grid-completion order); CHAIN = true adds the
+// closer (a8 in the last node unit) and the counter-ordered chaining of consecutive calls.  Two instantiations: the
+// extra code paths cost registers in the row phase (57.5 -> 60-63 us for the Cyclone plane when compiled in).
+template <class C, bool CHAIN>
+__global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlParams p) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float2* W = reinterpret_cast<float2*>(smem_raw);
+    float2* S = W + C::W_ELEMS;
+    float2* twx = S + C::S_ELEMS;
+    __shared__ unsigned long long stage_bar;
+    __shared__ float Tsh[16];
+    for (int i = threadIdx.x; i < C::NX; i += C::NT) twx[i] = p.twx[i];
+    bracket_row_unit<C, CtaSync, CHAIN>(p, blockIdx.x, W, S, twx, &stage_bar, Tsh, CtaSync());
 }
 
 }  // namespace gx

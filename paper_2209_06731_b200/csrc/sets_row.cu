@@ -7,20 +7,27 @@ namespace {
 // ---- row family (nl_row_kernels.cuh): whole y direction of an x row in one thread's registers; NY = 64
 template <class CB, class CC> cudaError_t prepare_row() {
     cudaError_t e = set_smem(gx::chi_planes_row_kernel<CC>, CC::SMEM_BYTES);
-    return e != cudaSuccess ? e : set_smem(gx::bracket_row_kernel<CB>, CB::SMEM_BYTES);
+    if (e == cudaSuccess) e = set_smem(gx::chi_planes_row_kernel<CB>, CB::SMEM_BYTES);
+    if (e == cudaSuccess) e = set_smem(gx::bracket_row_kernel<CB, true>, CB::SMEM_BYTES);
+    return e != cudaSuccess ? e : set_smem(gx::bracket_row_kernel<CB, false>, CB::SMEM_BYTES);
 }
 template <class C> cudaError_t launch_chi_row_t(const NlParams& p, int units, cudaStream_t st) {
     gx::chi_planes_row_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
     return cudaGetLastError();
 }
+template <class C> cudaError_t launch_chi_row_pdl_t(const NlParams& p, int units, cudaStream_t st) {
+    return launch_pdl(gx::chi_planes_row_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
+}
 template <class C> cudaError_t launch_bracket_row_t(const NlParams& p, int units, cudaStream_t st) {
-    return launch_pdl(gx::bracket_row_kernel<C>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
+    const bool chain = p.done != nullptr || p.a8_target != 0u;
+    return chain ? launch_pdl(gx::bracket_row_kernel<C, true>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p)
+                 : launch_pdl(gx::bracket_row_kernel<C, false>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
 }
 template <class CB, class CC> constexpr KernelSet make_row_set() {
     static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1,
                   "chi and bracket kernels must share the x radices (same permuted x order)");
     return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, GX_FAMILY_ROW, &prepare_row<CB, CC>, &launch_chi_row_t<CC>,
-                     &launch_bracket_row_t<CB>, false, nullptr};
+                     &launch_bracket_row_t<CB>, false, nullptr, true, &launch_chi_row_pdl_t<CB>, &launch_chi_row_pdl_t<CC>};
 }
 using R64x64   = gx::RowCfg<64, 64, 8, 8, 64, 6>;
 using R128x64  = gx::RowCfg<128, 64, 16, 8, 128, 3>;
@@ -37,6 +44,12 @@ const KernelSet* find_row(int Nx, int Ny) { return find_in(kRowSets, Nx, Ny); }
 }  // namespace gxhost
 
 #ifdef GX_PHASE_TIMING
+extern "C" int gx_debug_cta_log(long long* out) {
+    return cudaMemcpyFromSymbol(out, gx::gx_cta_log, sizeof(long long) * 4 * 8192 * 16) == cudaSuccess ? 0 : -1;
+}
+extern "C" int gx_debug_chi_log(long long* out) {
+    return cudaMemcpyFromSymbol(out, gx::gx_chi_log, sizeof(long long) * 4 * 256 * 4) == cudaSuccess ? 0 : -1;
+}
 extern "C" int gx_debug_phase_clocks(long long* out) {
     return cudaMemcpyFromSymbol(out, gx::gx_phase_clk, sizeof(long long) * 64 * 32) == cudaSuccess ? 0 : -1;
 }
