@@ -113,7 +113,14 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
                     const double* cvdrift, const double* cvdrift0, const double* bgrad,
                     const double* jacobian, double gradpar);
 
-/* out = -N[g, phi]  (the hot path).  Device pointers; enqueued on `cuda_stream`. */
+/* out = -N[g, phi]  (the hot path).  Device pointers; enqueued on `cuda_stream`.
+ * Stream semantics are the usual ones: g and phi must have been produced by work enqueued earlier on the stream
+ * (or be complete), and anything enqueued after the call sees `out` complete.  Consecutive calls on one handle
+ * overlap on the device where the kernel family supports it (NY = 64: the potential planes and the first units of a
+ * call run under the last wave of the previous call; the reuse of the workspace and of `out` is ordered by device
+ * counters, the two calls may write the same `out`).  Inputs of a call must not be overwritten before the call has
+ * completed in stream order -- as for any asynchronous call.  Environment: GX_CHI_SERIAL=1 disables the overlap,
+ * GX_A8_KERNEL=1 keeps the inverse Laguerre transform a separate kernel (development aids). */
 int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev,
                      void* cuda_stream);
 

@@ -863,7 +863,10 @@ int gx_query(gx_grid* g, int what, long long* value) {
         case GX_Q_G_ELEMS: *value = (long long)g->Ns * g->Nm * g->Nl * g->Nz * g->nk; break;
         case GX_Q_PHI_ELEMS: *value = (long long)g->Nz * g->nk; break;
         case GX_Q_WORKSPACE_BYTES: *value = (long long)g->bytes; break;
-        case GX_Q_LAUNCHES_PER_NL: *value = (g->ks && g->ks->launch_call) ? 1 : (g->ks && g->ks->fused_laguerre) ? 2 : 3; break;
+        case GX_Q_LAUNCHES_PER_NL:        // a8 inside the bracket kernel (row family, J <= 5, Nl <= 4): chi + bracket
+            *value = (g->ks && g->ks->launch_call) ? 1
+                   : (g->ks && (g->ks->fused_laguerre || (g->ks->closer && g->J <= 5 && g->Nl <= 4 && !std::getenv("GX_A8_KERNEL")))) ? 2 : 3;
+            break;
         case GX_Q_LAUNCHES_PER_RHS: *value = ((g->ks && g->ks->launch_call) ? 1 : (g->ks && g->ks->fused_laguerre) ? 2 : 3) + gx::kLinLaunchesFieldSolve + gx::kLinLaunchesRhs; break;
         case GX_Q_NL_FLOPS: *value = nl_flops(g); break;
         case GX_Q_KERNEL_FAMILY: *value = g->ks ? g->ks->family : -1; break;

@@ -49,6 +49,8 @@ struct PlaneCfg {
     static constexpr bool STAGE = STAGE_;
     static constexpr int K = (NX - 1) / 3, Q = (NY - 1) / 3;
     static constexpr int NAKX = 2 * K + 1, NAKY = Q + 1, NCOL = 2 * Q + 1, NK = NAKX * NAKY;
+    static constexpr int NKP = NK;               // elements of a compact plane in memory (differs from NK in transposed row configs)
+    static constexpr bool TR = false;
     static constexpr int HB = RB / 2, NBATCH = NX / RB;
     static constexpr int W_ELEMS = NX * NCOL;
     static constexpr int S_ELEMS = (STAGE && NK > NY * RB) ? NK : NY * RB;
@@ -220,11 +222,48 @@ __device__ __forceinline__ void y_inverse_pass1(const float2* __restrict__ W, fl
     __syncthreads();
 }
 
+// ---- transposed configurations (nl_row_kernels.cuh, RowCfg<..., TR = true>): the kernel works on the transposed
+// plane (its x is the physical y and vice versa, so that the 64-point direction is the one held in registers), the
+// arrays in memory keep the physical compact layout [ikx][ky], ikx in FFT order over 2Q+1 values, ky = 0..K.
+// With f'(a, q) = f(kx = q, ky = a) and the reality condition f(-k) = conj f(k):
+//   physical (kx >= 0, ky)      <-> internal (a = ky, q = kx)
+//   physical (kx <  0, ky >  0) <-> conj of internal (a = -ky, q = -kx)
+//   physical (kx =  0, ky >  0) also gives internal (a = -ky, q = 0) = conj;  physical (kx < 0, ky = 0) = conj internal (0, -kx).
+template <class C>
+__device__ __forceinline__ void tr_scatter(float2* __restrict__ S, const int i, const float2 v) {
+    constexpr int NAKYP = C::K + 1;
+    const int ikx = i / NAKYP, ky = i - ikx * NAKYP;
+    const float2 vc = make_float2(v.x, -v.y);
+    if (ikx <= C::Q) {
+        S[ky * C::NAKY + ikx] = v;
+        if (ikx == 0 && ky > 0) S[(C::NAKX - ky) * C::NAKY] = vc;
+    } else if (ky > 0) {
+        S[(C::NAKX - ky) * C::NAKY + (C::NCOL - ikx)] = vc;
+    }
+}
+struct LinearStore {      // compact internal index = memory index
+    __device__ __forceinline__ void operator()(float2* __restrict__ out, const int i, const int q, const int naky, const float2 v) const {
+        out[i * naky + q] = v;
+    }
+};
+template <class C> struct TrStore {      // internal (row i of the compact kx' order, q) -> physical [ikx][ky]
+    __device__ __forceinline__ void operator()(float2* __restrict__ out, const int i, const int q, const int, const float2 v) const {
+        constexpr int NAKYP = C::K + 1;
+        const float2 vc = make_float2(v.x, -v.y);
+        if (i <= C::K) {                                   // a = i >= 0: (kx = q, ky = i)
+            out[q * NAKYP + i] = v;
+            if (i == 0 && q > 0) out[(C::NCOL - q) * NAKYP] = vc;
+        } else if (q > 0) {                                // a = i - NAKX < 0: (kx = -q, ky = NAKX - i)
+            out[(C::NCOL - q) * NAKYP + (C::NAKX - i)] = vc;
+        }
+    }
+};
+
 // forward x transform on the naky kept columns; W holds Bhat(x, q) at permuted x positions.
 // Writes the 2K+1 kept kx rows (compact order) times `scale` to out[i*NAKY + q].
-template <class C, class SY = CtaSync>
+template <class C, class SY = CtaSync, class ST = LinearStore>
 __device__ __forceinline__ void x_forward(float2* __restrict__ W, const float2* __restrict__ twx,
-                                          float2* __restrict__ out, float scale, const SY sy = SY()) {
+                                          float2* __restrict__ out, float scale, const SY sy = SY(), const ST store = ST()) {
     constexpr int NX = C::NX, K = C::K, NCOL = C::NCOL, NAKY = C::NAKY, NAKX = C::NAKX;
     constexpr int R1 = C::RX1, R2 = C::RX2;
     for (int t = sy.tid(); t < R1 * NAKY; t += C::NT) {
@@ -251,7 +290,7 @@ __device__ __forceinline__ void x_forward(float2* __restrict__ W, const float2* 
                 int i = -1;
                 if (n <= K) i = n;
                 else if (n >= NX - K) i = n - NX + NAKX;
-                if (i >= 0) out[i * NAKY + q] = make_float2(v[cc].x * scale, v[cc].y * scale);
+                if (i >= 0) store(out, i, q, NAKY, make_float2(v[cc].x * scale, v[cc].y * scale));
             }
         }
     }
@@ -331,7 +370,7 @@ __device__ __forceinline__ void stage_combine_tma(float2* __restrict__ raw, floa
                                                   const float2* __restrict__ planes,
                                                   size_t lstride, const float* __restrict__ coef, int Nl,
                                                   const SY sy = SY()) {
-    constexpr int NK = C::NK, NT = C::NT, NK2 = NK / 2;
+    constexpr int NK = C::NKP, NT = C::NT, NK2 = NK / 2;     // planes as they lie in memory
     constexpr int CAP = (C::W_ELEMS + C::S_ELEMS) / NK;          // planes per chunk
     constexpr int PER = (NK2 + NT - 1) / NT;                     // float4 (2 complex) per thread
     const int tid = sy.tid();
@@ -366,10 +405,20 @@ __device__ __forceinline__ void stage_combine_tma(float2* __restrict__ raw, floa
         }
         sy.sync();                                             // raw region consumed
     }
-    float4* __restrict__ S4 = reinterpret_cast<float4*>(S) + tid;
+    if constexpr (C::TR) {
 #pragma unroll
-    for (int u = 0; u < PER; ++u)
-        if ((u + 1) * NT <= NK2 || tid + u * NT < NK2) S4[u * NT] = acc[u];
+        for (int u = 0; u < PER; ++u)
+            if ((u + 1) * NT <= NK2 || tid + u * NT < NK2) {
+                const int i = 2 * (tid + u * NT);
+                tr_scatter<C>(S, i, make_float2(acc[u].x, acc[u].y));
+                tr_scatter<C>(S, i + 1, make_float2(acc[u].z, acc[u].w));
+            }
+    } else {
+        float4* __restrict__ S4 = reinterpret_cast<float4*>(S) + tid;
+#pragma unroll
+        for (int u = 0; u < PER; ++u)
+            if ((u + 1) * NT <= NK2 || tid + u * NT < NK2) S4[u * NT] = acc[u];
+    }
 }
 
 template <class C>

@@ -34,14 +34,21 @@ __device__ __forceinline__ long long gx_smid() { unsigned s; asm volatile("mov.u
 #define GX_CHI(i) do { } while (0)
 #endif
 
-template <int NX_, int NY_, int RX1_, int RX2_, int NT_, int MINB_>
+// TR_ = true: the kernel's (NX, NY) is the TRANSPOSE of the physical plane (physical Nx = NY = 64, Ny = NX): the
+// 64-point direction is always the one held in registers.  Memory keeps the physical compact layout (NKP elements
+// per plane); the transposition happens where a plane enters (tr_scatter) and leaves (TrStore) shared memory, the
+// host swaps dkx / dky and flips the sign of the bracket (nl_kernels.cuh, gx_api.cu).
+template <int NX_, int NY_, int RX1_, int RX2_, int NT_, int MINB_, bool TR_ = false>
 struct RowCfg {
     static constexpr int NX = NX_, NY = NY_, RX1 = RX1_, RX2 = RX2_, NT = NT_, MINB = MINB_;
+    static constexpr bool TR = TR_;
     static constexpr int K = (NX - 1) / 3, Q = (NY - 1) / 3;
     static constexpr int NAKX = 2 * K + 1, NAKY = Q + 1, NCOL = 2 * Q + 1, NK = NAKX * NAKY;
+    static constexpr int NKP = TR ? NCOL * (K + 1) : NK;         // plane in memory: [2Q+1 kx][K+1 ky] when transposed
+    static constexpr int NKM = NK > NKP ? NK : NKP;
     static constexpr int W_ELEMS = NX * NCOL;
     // compact plane after the Laguerre combine; padded so that W + S hold 4 raw planes for the TMA staging
-    static constexpr int S_MIN = 4 * NK > W_ELEMS ? 4 * NK - W_ELEMS : 0;
+    static constexpr int S_MIN = 4 * NKM > W_ELEMS ? 4 * NKM - W_ELEMS : 0;
     static constexpr int S_ELEMS = ((NK > S_MIN ? NK : S_MIN) + 1) / 2 * 2;
     static constexpr int SMEM_BYTES = (W_ELEMS + S_ELEMS + NX) * (int)sizeof(float2);
     static constexpr bool STAGE = true;
@@ -60,7 +67,7 @@ struct RowCfg {
     }
     static constexpr zm_t ZMY = zero_mask_y();
     static_assert(NY == 64, "the single-thread y transform is written for 64 points");
-    static_assert(RX1 * RX2 == NX && NK % 2 == 0, "radix split / 16-byte planes");
+    static_assert(RX1 * RX2 == NX && NK % 2 == 0 && NKP % 2 == 0, "radix split / 16-byte planes");
     static_assert(SMEM_BYTES <= 232448, "plane does not fit in shared memory");
 };
 
@@ -105,15 +112,16 @@ __global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_row_kernel(const Nl
     float2* twx = S + C::S_ELEMS;
     const int unit = blockIdx.x;                 // (s*Nz + z)*J + j
     const int z = (unit / p.J) % p.Nz;
-    const float2* __restrict__ phi = p.phi + (size_t)(p.phi_by_unit ? unit : z) * C::NK;
-    const float* __restrict__ M = p.M + (size_t)(p.M_shared ? 0 : unit) * C::NK;
+    const float2* __restrict__ phi = p.phi + (size_t)(p.phi_by_unit ? unit : z) * C::NKP;
+    const float* __restrict__ M = p.M + (size_t)(p.M_shared ? 0 : unit) * C::NKP;
     pdl_launch_dependents();
     GX_CHI(0);
     for (int i = threadIdx.x; i < C::NX; i += C::NT) twx[i] = p.twx[i];
-    for (int i = threadIdx.x; i < C::NK; i += C::NT) {
+    for (int i = threadIdx.x; i < C::NKP; i += C::NT) {
         const float2 f = __ldg(phi + i);
         const float m = __ldg(M + i);
-        S[i] = make_float2(f.x * m, f.y * m);
+        if constexpr (C::TR) tr_scatter<C>(S, i, make_float2(f.x * m, f.y * m));
+        else S[i] = make_float2(f.x * m, f.y * m);
     }
     __syncthreads();
     x_inverse<C, false>(W, twx, p.dkx, p.dky, S);
@@ -165,7 +173,7 @@ __device__ __noinline__ void closer_sum(float2* __restrict__ raw, const float2* 
                                         const size_t lstride, const float* __restrict__ Tinv, const int J, const int Nl,
                                         const unsigned* cnt, const unsigned want, unsigned long long* bar, const unsigned parity,
                                         const SY sy, const NlParams& p) {
-    constexpr int NK = C::NK, NK2 = NK / 2, NT = C::NT;
+    constexpr int NK = C::NKP, NK2 = NK / 2, NT = C::NT;      // node planes lie in memory in the physical layout
     constexpr int CAP = (C::W_ELEMS + C::S_ELEMS) / NK;
     __shared__ float Tsm[4 * 8];              // -Tinv[l][j] (out = -N), zero-padded to [4][8]
     const int tid = sy.tid();
@@ -257,7 +265,7 @@ template <class C, class SY, bool CHAIN>
 __device__ __forceinline__ void bracket_row_unit(const NlParams& p, const int unit, float2* __restrict__ W,
                                                  float2* __restrict__ S, const float2* __restrict__ twx,
                                                  unsigned long long* stage_bar, float* Tsh, const SY sy) {
-    constexpr int NX = C::NX, NY = C::NY, NK = C::NK;
+    constexpr int NX = C::NX, NY = C::NY, NK = C::NKP;      // NK: plane stride of g, bhat, out in memory
     const int tid = sy.tid();
     const UnitIdx ix = decode_unit(p, unit);
     const int s = ix.s, m = ix.m, z = ix.z, j = ix.j, szj = ix.szj;
@@ -374,7 +382,8 @@ __device__ __forceinline__ void bracket_row_unit(const NlParams& p, const int un
         }
     }
     // ---- a6 (x part) + a7 (keep |kx| <= K)
-    x_forward<C, SY>(W, twx, p.bhat + ((size_t)iy.szj * p.Nm + iy.m) * NK, p.scale, sy);
+    using Store = typename std::conditional<C::TR, TrStore<C>, LinearStore>::type;
+    x_forward<C, SY, Store>(W, twx, p.bhat + ((size_t)iy.szj * p.Nm + iy.m) * NK, p.scale, sy);
 
     // ---- publish (see bracket_kernel)
     sy.sync();
