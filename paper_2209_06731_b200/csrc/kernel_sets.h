@@ -27,6 +27,9 @@ struct KernelSet {
     // (bracket-sized CTAs: they fit next to the bracket CTAs of the previous call's last wave)
     cudaError_t (*launch_chi_pdl)(const NlParams&, int units, cudaStream_t) = nullptr;
     cudaError_t (*launch_chi_pdl_wide)(const NlParams&, int units, cudaStream_t) = nullptr;   // same, launch_chi's CTA shape
+    // the kernels work on the transposed plane (RowCfg<..., TR = true>): the host swaps dkx / dky and the x / y twiddle
+    // tables and flips the sign of the bracket
+    bool transposed = false;
 };
 
 // Launch with the programmatic-stream-serialization attribute (PDL): the grid may begin before the

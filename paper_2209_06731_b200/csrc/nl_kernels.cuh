@@ -278,7 +278,9 @@ __device__ __forceinline__ void x_forward(float2* __restrict__ W, const float2* 
     }
     sy.sync();
     for (int t = sy.tid(); t < R2 * NAKY; t += C::NT) {
-        const int d = t / NAKY, q = t - d * NAKY;
+        // lanes run along q (contiguous in the compact layout); transposed configurations store along the row index
+        // instead, which is n = d + R2*cc: there d is the fastest index of a warp
+        const int d = C::TR ? t % R2 : t / NAKY, q = C::TR ? t / R2 : t - d * NAKY;
         float2 v[R1];
 #pragma unroll
         for (int a = 0; a < R1; ++a) v[a] = W[(a * R2 + d) * NCOL + q];

@@ -24,19 +24,23 @@ template <class C> cudaError_t launch_bracket_row_t(const NlParams& p, int units
                  : launch_pdl(gx::bracket_row_kernel<C, false>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
 }
 template <class CB, class CC> constexpr KernelSet make_row_set() {
-    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1,
+    static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::TR == CC::TR,
                   "chi and bracket kernels must share the x radices (same permuted x order)");
-    return KernelSet{CB::NX, CB::NY, CB::SMEM_BYTES, GX_FAMILY_ROW, &prepare_row<CB, CC>, &launch_chi_row_t<CC>,
-                     &launch_bracket_row_t<CB>, false, nullptr, true, &launch_chi_row_pdl_t<CB>, &launch_chi_row_pdl_t<CC>};
+    return KernelSet{CB::TR ? CB::NY : CB::NX, CB::TR ? CB::NX : CB::NY, CB::SMEM_BYTES, GX_FAMILY_ROW, &prepare_row<CB, CC>,
+                     &launch_chi_row_t<CC>, &launch_bracket_row_t<CB>, false, nullptr, true, &launch_chi_row_pdl_t<CB>,
+                     &launch_chi_row_pdl_t<CC>, CB::TR};
 }
 using R64x64   = gx::RowCfg<64, 64, 8, 8, 64, 6>;
 using R128x64  = gx::RowCfg<128, 64, 16, 8, 128, 3>;
 using R192x64  = gx::RowCfg<192, 64, 16, 12, 192, 2>;
 using RC192x64 = gx::RowCfg<192, 64, 16, 12, 384, 1>;   // chi planes: < 1 wave, more threads for the x passes
 using R256x64  = gx::RowCfg<256, 64, 16, 16, 256, 1>;
+// physical 64 x 192 (the paper's W7-X grid) on the transposed 192 x 64 kernels
+using T64x192  = gx::RowCfg<192, 64, 16, 12, 192, 2, true>;
+using TC64x192 = gx::RowCfg<192, 64, 16, 12, 384, 1, true>;
 const KernelSet kRowSets[] = {
     make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, RC192x64>(),
-    make_row_set<R256x64, R256x64>(),
+    make_row_set<R256x64, R256x64>(), make_row_set<T64x192, TC64x192>(),
 };
 
 }  // namespace
