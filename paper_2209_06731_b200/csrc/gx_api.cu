@@ -520,6 +520,9 @@ int nl_enqueue(gx_grid* g, NlParams p, int Nm_eff, bool do_chi, unsigned* count,
     unsigned target = (unsigned)g->J;
     if (!g->ks->fused_laguerre && calls) { *calls += 1; target = *calls * (unsigned)g->J; }
     p.a8_target = fuse_a8 ? target : 0u;
+    // GX_CLUSTER=1: a8 over the distributed shared memory of a J-CTA cluster instead of the closer.  Measured slower
+    // (Cyclone 64.4 against 56.7 us per call: co-scheduling of 5 CTAs and two cluster barriers per unit), kept as an option.
+    p.cluster = (fuse_a8 && g->J <= 8 && std::getenv("GX_CLUSTER") != nullptr) ? 1 : 0;
     // (a call that reuses chi planes is chained only if the chained flags describe those planes)
     // Calls with the separate inverse-Laguerre kernel (gx_rhs) are not chained: that kernel never triggers early.
     const bool chained = calls && fuse_a8 && g->ks->launch_chi_pdl && std::getenv("GX_CHI_SERIAL") == nullptr && (do_chi || g->chi_chained);

@@ -106,6 +106,7 @@ struct NlParams {
     // finished reading dchi; the chi grid of a call may overwrite its dchi buffer once done >= chi_need
     unsigned* done;
     unsigned chi_need;
+    int cluster;          // row family: the J node units of an (s,m,z) are one thread-block cluster (a8 over distributed shared memory)
     unsigned* chi_ready;  // chained calls: [s][z][j] of the current dchi buffer, epoch of the call that wrote the plane
     unsigned chi_epoch;
 };
@@ -627,10 +628,12 @@ template <int MAXL, int MAXJ, int VEC>
 __global__ void __launch_bounds__(256) laguerre_inverse_kernel(const NlParams p, int nk, unsigned target) {
     using V = typename std::conditional<VEC == 2, float4, float2>::type;
     const int kv = blockIdx.x * blockDim.x + threadIdx.x;      // index in units of VEC complex
-    const int smz = blockIdx.y;                                 // (s*Nm + m)*Nz + z
-    const int z = smz % p.Nz;
-    const int m = (smz / p.Nz) % p.Nm;
-    const int s = smz / (p.Nz * p.Nm);
+    // blocks are handed out in the order in which the bracket grid completes the (s,m,z): z before m (a block that
+    // waits for a late z would otherwise hold one of the few slots left beside the bracket CTAs)
+    const int m = blockIdx.y % p.Nm;
+    const int z = (blockIdx.y / p.Nm) % p.Nz;
+    const int s = blockIdx.y / (p.Nz * p.Nm);
+    const int smz = (s * p.Nm + m) * p.Nz + z;
     __shared__ float Ti[MAXL * MAXJ];
     for (int i = threadIdx.x; i < p.Nl * p.J; i += blockDim.x) Ti[i] = -__ldg(p.Tinv + i);   // out = -N
     if (threadIdx.x == 0) {

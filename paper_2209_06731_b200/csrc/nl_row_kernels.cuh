@@ -245,12 +245,81 @@ __device__ __noinline__ void closer_sum(float2* __restrict__ raw, const float2* 
     GX_CTA(12);
 }
 
+// ---- thread-block clusters (MODE 2 of bracket_row_kernel): the J node units of one (s,m,z) form one cluster, keep
+// their Bhat_j planes in shared memory and do a8 over distributed shared memory -- no bhat workspace, no closer.
+__device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ float4 ld_dsmem_f4(const void* local_smem_ptr, const unsigned rank) {
+    unsigned ra;
+    float4 v;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(smem_u32(local_smem_ptr)), "r"(rank));
+    asm volatile("ld.shared::cluster.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(ra) : "memory");
+    return v;
+}
+__device__ __forceinline__ void arrive_release_n(unsigned* counter, const unsigned n) {
+    asm volatile("red.release.gpu.global.add.u32 [%0], %1;" ::"l"(counter), "r"(n) : "memory");
+}
+
+// a8 of one (s,m,z) by its cluster: CTA `rank` owns every J-th group of NT float4 slots of the plane, reads that
+// group from the S region of all J CTAs and writes out_l = - sum_j Tinv[l][j] Bhat_j.  J <= 8, Nl <= 4.
+template <class C, class SY>
+__device__ __noinline__ void cluster_laguerre_inverse(const float2* S, float2* __restrict__ out0, const size_t lstride,
+                                                      const float* __restrict__ Tinv, const int J, const int Nl,
+                                                      const unsigned rank, const SY sy) {
+    constexpr int NK2 = C::NKP / 2, NT = C::NT;
+    __shared__ float Tsm[4 * 8];              // -Tinv[l][j] (out = -N), zero-padded to [4][8]
+    const int tid = sy.tid();
+    if (tid < 32) {
+        const int l = tid >> 3, jn = tid & 7;
+        Tsm[tid] = (l < Nl && jn < J) ? -__ldg(Tinv + l * J + jn) : 0.f;
+    }
+    sy.sync();
+    const float4* S4 = reinterpret_cast<const float4*>(S);
+    float4* out4 = reinterpret_cast<float4*>(out0);
+    const size_t lstride4 = lstride / 2;
+    for (int i = (int)rank * NT + tid; i < NK2; i += J * NT) {
+        float4 b[8];
+#pragma unroll
+        for (int jn = 0; jn < 8; ++jn)
+            b[jn] = jn < J ? ld_dsmem_f4(S4 + i, (unsigned)jn) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+        for (int l = 0; l < 4; ++l) {
+            if (l < Nl) {
+                float4 a = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                for (int jn = 0; jn < 8; ++jn) {
+                    const float t = Tsm[l * 8 + jn];
+                    a.x = fmaf(t, b[jn].x, a.x);
+                    a.y = fmaf(t, b[jn].y, a.y);
+                    a.z = fmaf(t, b[jn].z, a.z);
+                    a.w = fmaf(t, b[jn].w, a.w);
+                }
+                out4[l * lstride4 + i] = a;
+            }
+        }
+    }
+}
+
 // unit = (((s*(Nz/ZG) + zg)*J + j)*ZG + zi)*Nm + m, z = zg*ZG + zi: the Nm units that share a chi plane stay
 // neighbours, the J node units of one (s,m,z) lie ZG*Nm blocks apart (the last one, which does a8 in fused calls,
 // starts late enough to find most of the other planes complete)
+// Cluster mode: unit = ((s*Nz + z)*Nm + m)*J + j: the J node units of an (s,m,z) are the CTAs of one cluster.
 struct UnitIdx { int s, m, z, j, szj; };
+template <int MODE>
 __device__ __forceinline__ UnitIdx decode_unit(const NlParams& p, const int unit) {
     UnitIdx ix;
+    if (MODE == 2) {
+        ix.j = unit % p.J;
+        int r = unit / p.J;
+        ix.m = r % p.Nm; r /= p.Nm;
+        ix.z = r % p.Nz;
+        ix.s = r / p.Nz;
+        ix.szj = (ix.s * p.Nz + ix.z) * p.J + ix.j;
+        return ix;
+    }
     ix.m = unit % p.Nm;
     int r = unit / p.Nm;
     const int zi = r % p.ZG; r /= p.ZG;
@@ -261,13 +330,14 @@ __device__ __forceinline__ UnitIdx decode_unit(const NlParams& p, const int unit
     return ix;
 }
 
-template <class C, class SY, bool CHAIN>
+template <class C, class SY, int MODE>
 __device__ __forceinline__ void bracket_row_unit(const NlParams& p, const int unit, float2* __restrict__ W,
                                                  float2* __restrict__ S, const float2* __restrict__ twx,
                                                  unsigned long long* stage_bar, float* Tsh, const SY sy) {
     constexpr int NX = C::NX, NY = C::NY, NK = C::NKP;      // NK: plane stride of g, bhat, out in memory
     const int tid = sy.tid();
-    const UnitIdx ix = decode_unit(p, unit);
+    constexpr bool CHAIN = MODE != 0;
+    const UnitIdx ix = decode_unit<MODE>(p, unit);
     const int s = ix.s, m = ix.m, z = ix.z, j = ix.j, szj = ix.szj;
     const size_t lstride = (size_t)p.Nz * NK;
     const float2* __restrict__ g0 = p.g + ((size_t)(s * p.Nm + m) * p.Nl * p.Nz + z) * NK;
@@ -367,7 +437,7 @@ __device__ __forceinline__ void bracket_row_unit(const NlParams& p, const int un
     // the row phase needs every register: nothing but blockIdx is carried across it, the indices are formed again
     int unit2 = unit;
     if (CHAIN) asm volatile("" : "+r"(unit2));
-    const UnitIdx iy = CHAIN ? decode_unit(p, unit2) : ix;
+    const UnitIdx iy = CHAIN ? decode_unit<MODE>(p, unit2) : ix;
     unsigned* cnt = p.count + (iy.s * p.Nm + iy.m) * p.Nz + iy.z;
     if (CHAIN && p.done && tid == 0) {
         atomicAdd(p.done, 1u);          // this unit has read its chi pairs (values consumed before the barrier above)
@@ -381,6 +451,19 @@ __device__ __forceinline__ void bracket_row_unit(const NlParams& p, const int un
             }
         }
     }
+    if constexpr (MODE == 2) {
+        // ---- a6 (x part) + a7 into this CTA's S region, then a8 over the cluster's distributed shared memory
+        using StoreC = typename std::conditional<C::TR, TrStore<C>, LinearStore>::type;
+        x_forward<C, SY, StoreC>(W, twx, S, p.scale, sy);
+        GX_CTA(5);
+        cluster_sync_all();            // every node plane of this (s,m,z) is complete and visible cluster-wide
+        cluster_laguerre_inverse<C, SY>(S, p.out + (((size_t)(iy.s * p.Nm + iy.m) * p.Nl) * p.Nz + iy.z) * NK, (size_t)p.Nz * NK,
+                                        p.Tinv, p.J, p.Nl, cluster_ctarank(), sy);
+        cluster_sync_all();            // nobody leaves while its plane is still being read; all of out is written
+        if (tid == 0 && iy.j == 0) arrive_release_n(cnt, (unsigned)p.J);     // completes the epoch (+J per call)
+        GX_CTA(6);
+        return;
+    }
     // ---- a6 (x part) + a7 (keep |kx| <= K)
     using Store = typename std::conditional<C::TR, TrStore<C>, LinearStore>::type;
     x_forward<C, SY, Store>(W, twx, p.bhat + ((size_t)iy.szj * p.Nm + iy.m) * NK, p.scale, sy);
@@ -388,7 +471,7 @@ __device__ __forceinline__ void bracket_row_unit(const NlParams& p, const int un
     // ---- publish (see bracket_kernel)
     sy.sync();
     GX_CTA(5);
-    if (CHAIN && p.a8_target != 0u && iy.j == p.J - 1) {
+    if (MODE == 1 && p.a8_target != 0u && iy.j == p.J - 1) {
         // ---- a8: this unit closes its (s,m,z); its own plane is read back with the others
         closer_sum<C, SY>(W, p.bhat + ((size_t)((iy.s * p.Nz + iy.z) * p.J) * p.Nm + iy.m) * NK, (size_t)p.Nm * NK,
                           p.out + (((size_t)(iy.s * p.Nm + iy.m) * p.Nl) * p.Nz + iy.z) * NK, (size_t)p.Nz * NK, p.Tinv, p.J, p.Nl,
@@ -405,7 +488,8 @@ __device__ __forceinline__ void bracket_row_unit(const NlParams& p, const int un
 // CHAIN = false: the plain kernel (separate inverse-Laguerre grid, grid-completion order); CHAIN = true adds the
 // closer (a8 in the last node unit) and the counter-ordered chaining of consecutive calls.  Two instantiations: the
 // extra code paths cost registers in the row phase (57.5 -> 60-63 us for the Cyclone plane when compiled in).
-template <class C, bool CHAIN>
+// (MODE 2: the chained kernel with the cluster epilogue instead of the closer; launched with cluster dimension J.)
+template <class C, int MODE>
 __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlParams p) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float2* W = reinterpret_cast<float2*>(smem_raw);
@@ -414,7 +498,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_row_kernel(const NlPar
     __shared__ unsigned long long stage_bar;
     __shared__ float Tsh[16];
     for (int i = threadIdx.x; i < C::NX; i += C::NT) twx[i] = p.twx[i];
-    bracket_row_unit<C, CtaSync, CHAIN>(p, blockIdx.x, W, S, twx, &stage_bar, Tsh, CtaSync());
+    bracket_row_unit<C, CtaSync, MODE>(p, blockIdx.x, W, S, twx, &stage_bar, Tsh, CtaSync());
 }
 
 }  // namespace gx

@@ -8,8 +8,9 @@ namespace {
 template <class CB, class CC> cudaError_t prepare_row() {
     cudaError_t e = set_smem(gx::chi_planes_row_kernel<CC>, CC::SMEM_BYTES);
     if (e == cudaSuccess) e = set_smem(gx::chi_planes_row_kernel<CB>, CB::SMEM_BYTES);
-    if (e == cudaSuccess) e = set_smem(gx::bracket_row_kernel<CB, true>, CB::SMEM_BYTES);
-    return e != cudaSuccess ? e : set_smem(gx::bracket_row_kernel<CB, false>, CB::SMEM_BYTES);
+    if (e == cudaSuccess) e = set_smem(gx::bracket_row_kernel<CB, 1>, CB::SMEM_BYTES);
+    if (e == cudaSuccess) e = set_smem(gx::bracket_row_kernel<CB, 2>, CB::SMEM_BYTES);
+    return e != cudaSuccess ? e : set_smem(gx::bracket_row_kernel<CB, 0>, CB::SMEM_BYTES);
 }
 template <class C> cudaError_t launch_chi_row_t(const NlParams& p, int units, cudaStream_t st) {
     gx::chi_planes_row_kernel<C><<<units, C::NT, C::SMEM_BYTES, st>>>(p);
@@ -20,8 +21,19 @@ template <class C> cudaError_t launch_chi_row_pdl_t(const NlParams& p, int units
 }
 template <class C> cudaError_t launch_bracket_row_t(const NlParams& p, int units, cudaStream_t st) {
     const bool chain = p.done != nullptr || p.a8_target != 0u;
-    return chain ? launch_pdl(gx::bracket_row_kernel<C, true>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p)
-                 : launch_pdl(gx::bracket_row_kernel<C, false>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
+    if (chain && p.cluster) {       // the J node units of an (s,m,z) as one cluster, PDL attribute as for the others
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(units); cfg.blockDim = dim3(C::NT); cfg.dynamicSmemBytes = C::SMEM_BYTES; cfg.stream = st;
+        cudaLaunchAttribute at[2];
+        at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        at[0].val.programmaticStreamSerializationAllowed = 1;
+        at[1].id = cudaLaunchAttributeClusterDimension;
+        at[1].val.clusterDim.x = (unsigned)p.J; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 2;
+        return cudaLaunchKernelEx(&cfg, gx::bracket_row_kernel<C, 2>, p);
+    }
+    return chain ? launch_pdl(gx::bracket_row_kernel<C, 1>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p)
+                 : launch_pdl(gx::bracket_row_kernel<C, 0>, dim3(units), dim3(C::NT), C::SMEM_BYTES, st, p);
 }
 template <class CB, class CC> constexpr KernelSet make_row_set() {
     static_assert(CB::NX == CC::NX && CB::NY == CC::NY && CB::RX1 == CC::RX1 && CB::TR == CC::TR,

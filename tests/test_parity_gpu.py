@@ -304,13 +304,16 @@ def test_kernel_families_agree_with_oracle(torch_cuda, monkeypatch, family, name
     grid.close()
 
 
-@pytest.mark.parametrize("name", ["cyclone", "kinetic", "nx64"])
-def test_chained_calls_match_isolated_calls(torch_cuda, name):
+@pytest.mark.parametrize("name,cluster", [("cyclone", False), ("kinetic", False), ("nx64", False), ("cyclone", True), ("w7x-shape", True)])
+def test_chained_calls_match_isolated_calls(torch_cuda, monkeypatch, name, cluster):
     """Consecutive gx_nonlinear_rhs calls on one stream overlap on the device (row family: the chi planes of call
     N+1 start under the tail of call N; dchi is double-buffered; bhat, out and the counters are reused across calls and
     ordered by flags, not by grid completion).  Eight back-to-back calls with DIFFERENT states and potentials, two of
-    them writing the same output buffer, must give bit for bit what each call gives alone, and the oracle's result."""
+    them writing the same output buffer, must give bit for bit what each call gives alone, and the oracle's result.
+    (The transposed 64 x 192 configuration is covered by the w7x-shape case.)"""
     torch = torch_cuda
+    if cluster:          # optional variant: a8 over the distributed shared memory of a J-CTA cluster (GX_CLUSTER, read per call)
+        monkeypatch.setenv("GX_CLUSTER", "1")
     cfg = I.named_config(name)
     geo = I.geometry_arrays(cfg)
     sm = sorted({(s, m) for s in range(cfg.Ns) for m in (0, cfg.Nm // 2, cfg.Nm - 1)})
