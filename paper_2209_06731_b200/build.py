@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgx.so")
 OBJ = os.path.join(HERE, "build")
-SOURCES = ["gx_api.cu", "sets_scalar.cu", "sets_row.cu", "sets_rx.cu", "ubench.cu"]
+SOURCES = ["gx_api.cu", "sets_scalar.cu", "sets_scalar2.cu", "sets_row.cu", "sets_rx.cu", "ubench.cu"]
 HEADERS = ["dft_regs.cuh", "dft_packed.cuh", "kernel_sets.h", "nl_rx_kernels.cuh", "nl_kernels.cuh", "nl_row_kernels.cuh",
            "linear_kernels.cuh"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

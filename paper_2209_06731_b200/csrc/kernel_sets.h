@@ -56,7 +56,8 @@ inline int sm_count() {
 }
 
 
-const KernelSet* find_scalar(int Nx, int Ny);      // sets_scalar.cu
+const KernelSet* find_scalar(int Nx, int Ny);      // sets_scalar.cu (falls through to sets_scalar2.cu)
+const KernelSet* find_scalar_more(int Nx, int Ny); // sets_scalar2.cu
 const KernelSet* find_row(int Nx, int Ny);         // sets_row.cu
 const KernelSet* find_rx(int Nx, int Ny, int family);   // sets_rx.cu: GX_FAMILY_RX / RXP / RXW
 

@@ -42,6 +42,7 @@ template <class CB, class CC> constexpr KernelSet make_row_set() {
                      &launch_chi_row_t<CC>, &launch_bracket_row_t<CB>, false, nullptr, true, &launch_chi_row_pdl_t<CB>,
                      &launch_chi_row_pdl_t<CC>, CB::TR};
 }
+using R96x64   = gx::RowCfg<96, 64, 8, 12, 96, 4>;
 using R64x64   = gx::RowCfg<64, 64, 8, 8, 64, 6>;
 using R128x64  = gx::RowCfg<128, 64, 16, 8, 128, 3>;
 using R192x64  = gx::RowCfg<192, 64, 16, 12, 192, 2>;
@@ -50,9 +51,12 @@ using R256x64  = gx::RowCfg<256, 64, 16, 16, 256, 1>;
 // physical 64 x 192 (the paper's W7-X grid) on the transposed 192 x 64 kernels
 using T64x192  = gx::RowCfg<192, 64, 16, 12, 192, 2, true>;
 using TC64x192 = gx::RowCfg<192, 64, 16, 12, 384, 1, true>;
+using T64x96   = gx::RowCfg<96, 64, 8, 12, 96, 4, true>;
+using T64x256  = gx::RowCfg<256, 64, 16, 16, 256, 1, true>;
 const KernelSet kRowSets[] = {
     make_row_set<R64x64, R64x64>(), make_row_set<R128x64, R128x64>(), make_row_set<R192x64, RC192x64>(),
-    make_row_set<R256x64, R256x64>(), make_row_set<T64x192, TC64x192>(),
+    make_row_set<R256x64, R256x64>(), make_row_set<T64x192, TC64x192>(), make_row_set<R96x64, R96x64>(),
+    make_row_set<T64x96, T64x96>(), make_row_set<T64x256, T64x256>(),
 };
 
 }  // namespace

@@ -39,5 +39,8 @@ const KernelSet kKernelSets[] = {
 };
 
 }  // namespace
-const KernelSet* find_scalar(int Nx, int Ny) { return find_in(kKernelSets, Nx, Ny); }
+const KernelSet* find_scalar(int Nx, int Ny) {
+    const KernelSet* k = find_in(kKernelSets, Nx, Ny);
+    return k ? k : find_scalar_more(Nx, Ny);
+}
 }  // namespace gxhost

@@ -304,6 +304,29 @@ def test_kernel_families_agree_with_oracle(torch_cuda, monkeypatch, family, name
     grid.close()
 
 
+@pytest.mark.parametrize("Nx,Ny,family", [(48, 48, "scalar"), (96, 96, "scalar"), (128, 96, "scalar"), (192, 96, "scalar"),
+                                          (96, 192, "scalar"), (96, 64, "row"), (64, 96, "row"), (64, 256, "row")])
+def test_more_plane_shapes(torch_cuda, Nx, Ny, family):
+    """Further (Nx, Ny) instantiations -- the paper's other perpendicular grids (Ny = 96 with Nx = 96 ... 192) and the
+    transposed row configurations for Nx = 64 -- full array against the oracle, two species-free small batches."""
+    cfg = I.Config(f"shape{Nx}x{Ny}", Nx, Ny, 3, 3, 2, [I.Species(tprim=6.9, fprim=2.2, nu_ss=0.01)], seed=I.BASE_SEED + 40 + Nx + Ny)
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    Phi = _oracle_phi(cfg, geo, G)
+    grid = _grid(cfg, geo)
+    from paper_2209_06731_b200 import binding
+    assert binding.FAMILY_NAMES[grid.query(binding.GX_Q_KERNEL_FAMILY)] == family
+    out = _gpu_nl(torch_cuda, grid, G, Phi)
+    out2 = _gpu_nl(torch_cuda, grid, G, Phi)
+    assert np.array_equal(out, out2)
+    ref = _oracle_nl(cfg, geo, G, Phi, method="dft")
+    assert O.relative_max_error(out, ref) <= TOL, (Nx, Ny, O.relative_max_error(out, ref))
+    for l in range(cfg.Nl):
+        a, r = out[:, :, l], ref[:, :, l]
+        assert np.max(np.abs(a - r)) <= TOL * np.max(np.abs(r)), (Nx, Ny, l)
+    grid.close()
+
+
 @pytest.mark.parametrize("name,cluster", [("cyclone", False), ("kinetic", False), ("nx64", False), ("cyclone", True), ("w7x-shape", True)])
 def test_chained_calls_match_isolated_calls(torch_cuda, monkeypatch, name, cluster):
     """Consecutive gx_nonlinear_rhs calls on one stream overlap on the device (row family: the chi planes of call
