@@ -200,6 +200,7 @@ NlParams make_params(gx_grid* g, const void* gd, const void* phid, void* outd) {
     p.dky = (float)g->dky;
     p.scale = (float)(1.0 / ((double)g->Nx * (double)g->Ny));
     p.Nz = g->Nz; p.Nl = g->Nl; p.Nm = g->Nm; p.Ns = g->Ns; p.J = g->J;
+    if (g->ks && g->ks->family == GX_FAMILY_ROW) p.scale *= 0.5f;      // row_forward_real leaves twice the coefficients
     if (g->ks && g->ks->transposed) {
         // the kernels see x' = y, y' = x: {chi, g}' = -{chi, g}
         std::swap(p.dkx, p.dky);

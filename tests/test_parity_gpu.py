@@ -227,7 +227,7 @@ def test_zero_input_and_error_paths(torch_cuda):
             B.gx_grid_create(bad[0], bad[1], 4, 2, 2, 1)
         assert e.value.code == B.GX_ERR_ARG
     with pytest.raises(B.GxError) as e:
-        B.gx_grid_create(48, 48, 4, 2, 2, 1)       # valid size, no kernel instantiation
+        B.gx_grid_create(32, 32, 4, 2, 2, 1)       # valid size, no kernel instantiation
     assert e.value.code == B.GX_ERR_UNSUPPORTED
     h = B.gx_grid_create(16, 16, 4, 2, 2, 1)
     with pytest.raises(B.GxError) as e:
