@@ -377,6 +377,54 @@ def test_chained_calls_match_isolated_calls(torch_cuda, monkeypatch, name, clust
     grid.close()
 
 
+def test_mixed_call_sequences_on_one_handle(torch_cuda):
+    """Chained gx_nonlinear_rhs calls interleaved, without synchronisation, with gx_rhs (plain kernels + separate
+    inverse-Laguerre kernel), the electromagnetic call, gx_field_solve and the host entry point: every result equals
+    the one the same call gives alone (the counters' epochs and the two dchi buffers survive every transition)."""
+    torch = torch_cuda
+    cfg = I.named_config("cyclone")
+    geo = I.geometry_arrays(cfg)
+    sm = sorted({(0, m) for m in (0, 1, cfg.Nm - 1)})
+    G0 = I.make_state(cfg, geo, planes=sm)
+    grid = _grid(cfg, geo)
+    gs = [torch.from_numpy(((1.0 + 0.3 * i) * G0).astype(np.complex64)).cuda() for i in range(4)]
+    phis = [torch.empty(cfg.phi_shape, dtype=torch.complex64, device="cuda") for _ in range(4)]
+    for i in range(4):
+        grid.field_solve(gs[i], phis[i])
+    zero = torch.zeros_like(phis[0])
+    gh = gs[2].cpu().pin_memory(); ph = phis[2].cpu().pin_memory()
+    ops = ["nl", "nl", "rhs", "nl", "em", "nl", "rhs", "rhs", "nl", "host", "nl", "nl"]
+
+    def run(k, op, out):
+        i = k % 4
+        if op == "nl":
+            grid.nonlinear_rhs(gs[i], phis[i], out)
+        elif op == "rhs":
+            grid.rhs(gs[i], out)
+        elif op == "em":
+            grid.nonlinear_rhs_em(gs[i], phis[i], zero, zero, out)
+        else:
+            oh = torch.empty_like(gh).pin_memory()
+            grid.nonlinear_rhs_host(gh, ph, oh)
+            out.copy_(oh, non_blocking=False)
+
+    alone = []
+    for k, op in enumerate(ops):
+        out = torch.full_like(gs[0], float("nan"))
+        run(k, op, out)
+        torch.cuda.synchronize()
+        alone.append(out.cpu().numpy())
+    assert np.array_equal(alone[4], alone[0])             # apar = bpar = 0: the electromagnetic call is the electrostatic one
+    for rep in range(2):
+        outs = [torch.full_like(gs[0], float("nan")) for _ in ops]
+        for k, op in enumerate(ops):
+            run(k, op, outs[k])
+        torch.cuda.synchronize()
+        for k, op in enumerate(ops):
+            assert np.array_equal(outs[k].cpu().numpy(), alone[k]), (rep, k, op)
+    grid.close()
+
+
 # ------------------------------------------------------------------------------------------------
 # SURVEY row f1: linear terms and the full right-hand side against oracle/gx_linear.py
 import gx_linear as OL
