@@ -247,6 +247,7 @@ int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out
     *out = g;                       // returned even on failure below so that gx_last_error works
     if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
     GX_CUDA(g, g->ks->prepare());      // per device and per handle: no process-wide cache of function attributes
+    GX_CUDA(g, gx::lin_prepare());
 
     gauss_laguerre(g->J, g->xj, g->wj);
     g->hT.resize((size_t)g->J * Nl);

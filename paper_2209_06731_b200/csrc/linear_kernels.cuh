@@ -991,6 +991,23 @@ __global__ void __launch_bounds__(kZlinkThreads) lin_zlink_kernel(LinTables t, c
     }
 }
 
+// Opt-in shared-memory sizes of every linear kernel instantiation, on the current device (gx_grid_create: per
+// handle and per device, no process-wide cache).
+inline cudaError_t lin_prepare() {
+    constexpr int kMax = 200 * 1024;
+    cudaError_t e = cudaSuccess;
+#define GX_ATTR(K) if (e == cudaSuccess) e = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, kMax)
+    GX_ATTR((lin_rhs_kernel<true, 4>));  GX_ATTR((lin_rhs_kernel<false, 4>));
+    GX_ATTR((lin_rhs_kernel<true, 1>));  GX_ATTR((lin_rhs_kernel<false, 1>));
+    GX_ATTR((lin_rhs_kernel<true, 4, true>));  GX_ATTR((lin_rhs_kernel<true, 1, true>));
+    GX_ATTR((lin_rhs_kernel<true, 1, true, 8, 8>));   GX_ATTR((lin_rhs_kernel<true, 1, false, 8, 8>));   GX_ATTR((lin_rhs_kernel<false, 1, false, 8, 8>));
+    GX_ATTR((lin_rhs_kernel<true, 1, true, 8, 12>));  GX_ATTR((lin_rhs_kernel<true, 1, false, 8, 12>));  GX_ATTR((lin_rhs_kernel<false, 1, false, 8, 12>));
+    GX_ATTR((lin_rhs_kernel<true, 1, true, 8, 16>));  GX_ATTR((lin_rhs_kernel<true, 1, false, 8, 16>));  GX_ATTR((lin_rhs_kernel<false, 1, false, 8, 16>));
+    GX_ATTR(lin_zlink_kernel<4>);  GX_ATTR(lin_zlink_kernel<1>);
+#undef GX_ATTR
+    return e;
+}
+
 inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* phi, float2* out, bool accumulate,
                            cudaStream_t st) {
     if (!t.built) return cudaErrorNotReady;
@@ -1017,14 +1034,11 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
 #define GX_ZFFT(FB)                                                                                                        \
     do {                                                                                                                   \
         if (splitf) {                                                                                                      \
-            e = cudaFuncSetAttribute(lin_rhs_kernel<true, 1, true, 8, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-            if (e == cudaSuccess) lin_rhs_kernel<true, 1, true, 8, FB><<<gridf, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false);  \
+            lin_rhs_kernel<true, 1, true, 8, FB><<<gridf, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false);  \
         } else if (accumulate) {                                                                                           \
-            e = cudaFuncSetAttribute(lin_rhs_kernel<true, 1, false, 8, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-            if (e == cudaSuccess) lin_rhs_kernel<true, 1, false, 8, FB><<<gridf, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false); \
+            lin_rhs_kernel<true, 1, false, 8, FB><<<gridf, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false); \
         } else {                                                                                                           \
-            e = cudaFuncSetAttribute(lin_rhs_kernel<false, 1, false, 8, FB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem); \
-            if (e == cudaSuccess) lin_rhs_kernel<false, 1, false, 8, FB><<<gridf, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false); \
+            lin_rhs_kernel<false, 1, false, 8, FB><<<gridf, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false); \
         }                                                                                                                  \
     } while (0)
         if (t.Nz == 64) GX_ZFFT(8);
@@ -1032,17 +1046,6 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
         else GX_ZFFT(16);
 #undef GX_ZFFT
         return e != cudaSuccess ? e : cudaGetLastError();
-    }
-    static bool attr = false;
-    if (!attr) {
-        cudaError_t e = cudaFuncSetAttribute(lin_rhs_kernel<true, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<false, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<false, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<true, 4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_rhs_kernel<true, 1, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-        if (e != cudaSuccess) return e;
-        attr = true;
     }
     dim3 grid(t.Ns * t.Nm, t.Nl, (t.nk + kLinTK - 1) / kLinTK);
     const bool b4 = t.Nz % 4 == 0;
@@ -1070,13 +1073,6 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
         else lin_rhs_kernel<false, 1><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, t.linked);
     }
     if (t.linked) {
-        static bool attr2 = false;
-        if (!attr2) {
-            cudaError_t e = cudaFuncSetAttribute(lin_zlink_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-            if (e == cudaSuccess) e = cudaFuncSetAttribute(lin_zlink_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
-            if (e != cudaSuccess) return e;
-            attr2 = true;
-        }
         // two launches: the few long chains with room for the longest extended domain, the many short ones
         // (up to 4 links) with a small footprint so that 32 blocks fit an SM
         const int w0[2] = {0, t.nzwork_long}, wn[2] = {t.nzwork_long, t.nzwork - t.nzwork_long};
