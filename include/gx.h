@@ -119,7 +119,9 @@ int gx_geometry_set(gx_grid* g, const double* bmag, const double* gds2, const do
  * overlap on the device where the kernel family supports it (NY = 64: the potential planes and the first units of a
  * call run under the last wave of the previous call; the reuse of the workspace and of `out` is ordered by device
  * counters, the two calls may write the same `out`).  Inputs of a call must not be overwritten before the call has
- * completed in stream order -- as for any asynchronous call.  Environment: GX_CHI_SERIAL=1 disables the overlap,
+ * completed in stream order -- as for any asynchronous call.  The device compute calls cannot be recorded into a
+ * CUDA graph by the caller (their kernels take the call's epoch as an argument): GX_ERR_STATE while the stream is
+ * capturing; gx_nonlinear_rhs_host builds and replays a graph of its own.  Environment: GX_CHI_SERIAL=1 disables the overlap,
  * GX_A8_KERNEL=1 keeps the inverse Laguerre transform a separate kernel (development aids). */
 int gx_nonlinear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev,
                      void* cuda_stream);

@@ -498,6 +498,12 @@ int nl_enqueue(gx_grid* g, NlParams p, int Nm_eff, bool do_chi, unsigned* count,
     p.Nm = Nm_eff;
     p.count = count;
     const int szj = g->Ns * g->Nz * g->J;
+    if (calls) {
+        // the kernels take the call's epoch as an argument: a caller's CUDA graph would replay stale epochs
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (cudaStreamIsCapturing(st, &cs) == cudaSuccess && cs != cudaStreamCaptureStatusNone)
+            return fail(g, GX_ERR_STATE, "the compute calls cannot be recorded into a CUDA graph (gx_nonlinear_rhs_host replays its own)");
+    }
     if (do_chi) g->chi_buf ^= 1;
     p.dchi = g->ddchi + (size_t)g->chi_buf * szj * g->Nx * g->Ny;
     // a8 inside the bracket kernel (last node unit of an (s,m,z) to arrive) unless out already holds the linear terms

@@ -236,6 +236,40 @@ def test_zero_input_and_error_paths(torch_cuda):
     B.gx_grid_destroy(h)
 
 
+def test_compute_calls_refuse_stream_capture(torch_cuda):
+    """The kernels take the call's epoch as an argument, so a caller's CUDA graph would replay stale epochs: the
+    device compute calls return GX_ERR_STATE while their stream is capturing (and work again afterwards)."""
+    torch = torch_cuda
+    from paper_2209_06731_b200 import binding as B
+    cfg = I.named_config("tiny")
+    geo = I.geometry_arrays(cfg)
+    G = I.make_state(cfg, geo)
+    grid = _grid(cfg, geo)
+    g = torch.from_numpy(G).cuda()
+    phi = torch.from_numpy(_oracle_phi(cfg, geo, G)).cuda()
+    out = torch.empty_like(g)
+    grid.nonlinear_rhs(g, phi, out)
+    torch.cuda.synchronize()
+    ref = out.clone()
+    side = torch.cuda.Stream()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        graph.capture_begin()
+        try:
+            with pytest.raises(B.GxError) as e:
+                grid.nonlinear_rhs(g, phi, out)
+            assert e.value.code == B.GX_ERR_STATE
+            phi.mul_(1.0)                       # something to record: an empty capture is an error of its own
+        finally:
+            graph.capture_end()
+    torch.cuda.synchronize()
+    out.zero_()
+    grid.nonlinear_rhs(g, phi, out)
+    torch.cuda.synchronize()
+    assert torch.equal(out, ref)
+    grid.close()
+
+
 @pytest.mark.parametrize("name", ["tiny", "kinetic"])
 def test_host_entry_point_matches_device_entry_point(torch_cuda, name):
     """gx_nonlinear_rhs_host pipelines Hermite blocks over three streams (two species: strided block copies);
