@@ -118,9 +118,13 @@ struct NlParams {
 // kx >= 0, always kept with kx < 0, always padding, or decided by n2 at run time (at most two n1).
 // For column q < 0 the reality condition gives f(a,q) = conj f(-a,-q): row index and the sign of the
 // imaginary part flip, which keeps every address of the form base + compile-time offset.
-template <class C, bool GLOBAL_F, class SY = CtaSync>
+struct NoMid { __device__ __forceinline__ void operator()() const {} };
+// MID: called by every thread between the two passes (after the barrier): a place for work that only needs issue
+// slots, e.g. cache prefetches of data the next phase will read.
+template <class C, bool GLOBAL_F, class SY = CtaSync, class MID = NoMid>
 __device__ __forceinline__ void x_inverse(float2* __restrict__ W, const float2* __restrict__ twx,
-                                          float dkx, float dky, const float2* __restrict__ F, const SY sy = SY()) {
+                                          float dkx, float dky, const float2* __restrict__ F, const SY sy = SY(),
+                                          const MID mid = MID()) {
     constexpr int NX = C::NX, K = C::K, NCOL = C::NCOL, NAKY = C::NAKY, NAKX = C::NAKX;
     constexpr int R1 = C::RX1, R2 = C::RX2;
     // pass 1: for each (n2, column): DFT_R1 over n1 of input n = n1*R2+n2, twiddle, in-place slot
@@ -174,6 +178,7 @@ __device__ __forceinline__ void x_inverse(float2* __restrict__ W, const float2* 
             W[(k1 * R2 + n2) * NCOL + c] = k1 == 0 ? v[0] : cmul(v[k1], twx[n2 * k1]);
     }
     sy.sync();
+    mid();
     // pass 2: for each (k1, column): DFT_R2 over n2; position k1*R2+k2 <- x = k1 + R1*k2
     for (int t = sy.tid(); t < R1 * NCOL; t += C::NT) {
         const int k1 = t / NCOL, c = t - k1 * NCOL;

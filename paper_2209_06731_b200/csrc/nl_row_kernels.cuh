@@ -371,11 +371,27 @@ __device__ __forceinline__ void bracket_row_unit(const NlParams& p, const int un
     stage_combine_tma<C, SY>(W, S, stage_bar, bar_parity, g0, lstride, Tsh, p.Nl, sy);
     sy.sync();
     GX_CTA(1);
-    // ---- a3 + a4 (x part)
-    x_inverse<C, false, SY>(W, twx, p.dkx, p.dky, S, sy);
+    // ---- a3 + a4 (x part).  Chained calls whose chi plane was already complete when this unit started (every unit
+    // but those of the first wave): the chi rows of the first two output groups are requested into L1 between the
+    // two x passes -- an L2 round trip takes about 1 us under this kernel's load, the row phase would otherwise
+    // start with it
+    const float2* dchi = p.dchi + (size_t)szj * NX * NY;
+    __shared__ unsigned chi_early;
+    if (tid == 0) chi_early = (CHAIN && p.done && chi_seen == p.chi_epoch) ? 1u : 0u;
+    auto early_prefetch = [&]() {
+        if (CHAIN && chi_early) {
+            for (int row = tid; row < NX; row += C::NT) {
+#pragma unroll
+                for (int k2 = 0; k2 < 8; ++k2) {
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(dchi + row + (8 * k2) * NX));
+                    asm volatile("prefetch.global.L1 [%0];" ::"l"(dchi + row + (1 + 8 * k2) * NX));
+                }
+            }
+        }
+    };
+    x_inverse<C, false, SY, decltype(early_prefetch)>(W, twx, p.dkx, p.dky, S, sy, early_prefetch);
     GX_CTA(2);
 
-    const float2* dchi = p.dchi + (size_t)szj * NX * NY;
     if (!CHAIN || !p.done) pdl_wait();        // chi planes of this call are complete and visible from here on
     else {
         // chained: every chi CTA of this call is resident (this grid is scheduled after all of them have started);
