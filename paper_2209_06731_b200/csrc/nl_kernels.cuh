@@ -52,6 +52,10 @@ struct PlaneCfg {
     static constexpr int NKP = NK;               // elements of a compact plane in memory (differs from NK in transposed row configs)
     static constexpr bool TR = false;
     static constexpr int HB = RB / 2, NBATCH = NX / RB;
+    // Which two x rows share one complex forward y transform: rows p and p + NX/2 (lanes of a half-warp then read rows
+    // NX/2 apart, which lie in the same shared-memory banks whenever HB < 16: 26 % of the stellarator kernel's
+    // wavefronts were conflicts) or, for the small batches, the adjacent rows 2p and 2p + 1 (conflict-free for HB <= 8).
+    static constexpr bool ADJ = RB <= 16;
     static constexpr int W_ELEMS = NX * NCOL;
     static constexpr int S_ELEMS = (STAGE && NK > NY * RB) ? NK : NY * RB;
     static constexpr int SMEM_BYTES = (W_ELEMS + S_ELEMS + NX + NY) * (int)sizeof(float2);
@@ -207,7 +211,9 @@ __device__ __forceinline__ void y_inverse_pass1(const float2* __restrict__ W, fl
     constexpr int R1 = C::RY1, R2 = C::RY2;
     for (int t = threadIdx.x; t < R2 * RB; t += C::NT) {
         const int n2 = t / RB, r = t - n2 * RB;
-        const int row = PAIRED ? (r < HB ? bt * HB + r : bt * HB + (r - HB) + NX / 2) : bt * RB + r;
+        const int row = !PAIRED ? bt * RB + r
+                      : C::ADJ ? (r < HB ? bt * RB + 2 * r : bt * RB + 2 * (r - HB) + 1)
+                               : (r < HB ? bt * HB + r : bt * HB + (r - HB) + NX / 2);
         const float2* __restrict__ Wr = W + row * NCOL;
         const float2* __restrict__ WP = Wr + n2;                  // ky >= 0: column n
         const float2* __restrict__ WN = Wr + n2 - NY + NCOL;      // ky <  0: column n - NY + NCOL
@@ -554,7 +560,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 const int r = rp + h * HB;
-                const int row = bt * HB + rp + h * (NX / 2);
+                const int row = C::ADJ ? bt * RB + 2 * rp + h : bt * HB + rp + h * (NX / 2);
                 float2 v[R2];
 #pragma unroll
                 for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[(k1 * R2 + n2) * RB + r];
@@ -588,8 +594,8 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
 #pragma unroll
                 for (int a = 0; a < R1; ++a) u1[a] = u0[a];
             }
-            float2* __restrict__ W0 = W + (bt * HB + rp) * NCOL;
-            float2* __restrict__ W1 = W0 + (NX / 2) * NCOL;
+            float2* __restrict__ W0 = W + (C::ADJ ? bt * RB + 2 * rp : bt * HB + rp) * NCOL;
+            float2* __restrict__ W1 = W0 + (C::ADJ ? 1 : NX / 2) * NCOL;
 #pragma unroll
             for (int cc = 0; cc <= Q / R2; ++cc) {
                 // class d0: k = d0 + R2*cc, partner NY-k in class d1
