@@ -553,13 +553,13 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
     for (int bt = 0; bt < C::NBATCH; ++bt) {
         // ---- a4 (y part): rows p and p+NX/2 of the batch
         y_inverse_pass1<C, true>(W, S, twy, bt);
-        // ---- a4 (last pass) + a5 bracket + a6 (first forward pass), all in registers
-        for (int t = threadIdx.x; t < R1 * HB; t += C::NT) {
-            const int k1 = t / HB, rp = t - k1 * HB;
-            float2 c[R2];
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const int r = rp + h * HB;
+        if constexpr (2 * R1 * HB <= C::NT) {
+            // Small batches (the plane fills shared memory): R1*HB items would keep a quarter of the CTA busy through three
+            // transforms.  One thread per ROW does the last inverse pass and the bracket and leaves the real result in
+            // the slots it has just read; after a barrier one thread per row PAIR does the first forward pass.
+            for (int t = threadIdx.x; t < R1 * RB; t += C::NT) {
+                const int k1 = t / RB, r = t - k1 * RB;
+                const int h = r / HB, rp = r - h * HB;
                 const int row = C::ADJ ? bt * RB + 2 * rp + h : bt * HB + rp + h * (NX / 2);
                 float2 v[R2];
 #pragma unroll
@@ -568,53 +568,111 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
 #pragma unroll
                 for (int k2 = 0; k2 < R2; ++k2) {
                     const float2 d = dchi[(size_t)(k1 * R2 + k2) * NX + row];
-                    const float b = fmaf(d.y, v[k2].x, -d.x * v[k2].y);   // d_y chi d_x g - d_x chi d_y g
-                    if (h == 0) c[k2].x = b; else c[k2].y = b;
+                    S[(k1 * R2 + k2) * RB + r] = make_float2(fmaf(d.y, v[k2].x, -d.x * v[k2].y), 0.f);
                 }
             }
-            dft<R2, -1>(c);
+            __syncthreads();
+            for (int t = threadIdx.x; t < R1 * HB; t += C::NT) {
+                const int k1 = t / HB, rp = t - k1 * HB;
+                float2 c[R2];
 #pragma unroll
-            for (int d = 0; d < R2; ++d)
-                S[(k1 * R2 + d) * RB + rp] = d == 0 ? c[0] : cmul_conj(c[d], twy[k1 * d]);
-        }
-        __syncthreads();
-        // ---- a6 (last y pass) + a7 (keep ky <= Q) + separation of the packed row pair
-        for (int t = threadIdx.x; t < (R2 / 2 + 1) * HB; t += C::NT) {
-            const int dd = t / HB, rp = t - dd * HB;
-            const int d0 = dd, d1 = (R2 - dd) % R2;
-            float2 u0[R1], u1[R1];
+                for (int k2 = 0; k2 < R2; ++k2)
+                    c[k2] = make_float2(S[(k1 * R2 + k2) * RB + rp].x, S[(k1 * R2 + k2) * RB + rp + HB].x);
+                dft<R2, -1>(c);
 #pragma unroll
-            for (int a = 0; a < R1; ++a) u0[a] = S[(a * R2 + d0) * RB + rp];
-            dft<R1, -1>(u0);
-            if (d1 != d0) {
-#pragma unroll
-                for (int a = 0; a < R1; ++a) u1[a] = S[(a * R2 + d1) * RB + rp];
-                dft<R1, -1>(u1);
-            } else {
-#pragma unroll
-                for (int a = 0; a < R1; ++a) u1[a] = u0[a];
+                for (int d = 0; d < R2; ++d)
+                    S[(k1 * R2 + d) * RB + rp] = d == 0 ? c[0] : cmul_conj(c[d], twy[k1 * d]);
             }
-            float2* __restrict__ W0 = W + (C::ADJ ? bt * RB + 2 * rp : bt * HB + rp) * NCOL;
-            float2* __restrict__ W1 = W0 + (C::ADJ ? 1 : NX / 2) * NCOL;
+        } else {
+            // ---- a4 (last pass) + a5 bracket + a6 (first forward pass), all in registers
+            for (int t = threadIdx.x; t < R1 * HB; t += C::NT) {
+                const int k1 = t / HB, rp = t - k1 * HB;
+                float2 c[R2];
 #pragma unroll
-            for (int cc = 0; cc <= Q / R2; ++cc) {
-                // class d0: k = d0 + R2*cc, partner NY-k in class d1
-                {
-                    const int k = d0 + R2 * cc;
-                    if (k <= Q) {
-                        const float2 A = u0[cc];
-                        const float2 B = (d0 == 0) ? u1[(R1 - cc) % R1] : u1[R1 - 1 - cc];
-                        W0[k] = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));
-                        W1[k] = make_float2(0.5f * (A.y + B.y), 0.5f * (B.x - A.x));
+                for (int h = 0; h < 2; ++h) {
+                    const int r = rp + h * HB;
+                    const int row = C::ADJ ? bt * RB + 2 * rp + h : bt * HB + rp + h * (NX / 2);
+                    float2 v[R2];
+#pragma unroll
+                    for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[(k1 * R2 + n2) * RB + r];
+                    dft<R2, +1>(v);
+#pragma unroll
+                    for (int k2 = 0; k2 < R2; ++k2) {
+                        const float2 d = dchi[(size_t)(k1 * R2 + k2) * NX + row];
+                        const float b = fmaf(d.y, v[k2].x, -d.x * v[k2].y);   // d_y chi d_x g - d_x chi d_y g
+                        if (h == 0) c[k2].x = b; else c[k2].y = b;
                     }
                 }
+                dft<R2, -1>(c);
+#pragma unroll
+                for (int d = 0; d < R2; ++d)
+                    S[(k1 * R2 + d) * RB + rp] = d == 0 ? c[0] : cmul_conj(c[d], twy[k1 * d]);
+            }
+        }
+        __syncthreads();
+        if constexpr (2 * R1 * HB <= C::NT) {
+            // small batches: one thread per (class d, row pair) does the last forward pass in place, then, after a
+            // barrier, one thread per kept (ky, row pair) separates the packed rows (the fused loop below would keep
+            // (R2/2+1)*HB threads -- three warps of twelve -- busy through two transforms; it took a third of the kernel)
+            for (int t = threadIdx.x; t < R2 * HB; t += C::NT) {
+                const int d = t / HB, rp = t - d * HB;
+                float2 u[R1];
+#pragma unroll
+                for (int a = 0; a < R1; ++a) u[a] = S[(a * R2 + d) * RB + rp];
+                dft<R1, -1>(u);
+#pragma unroll
+                for (int a = 0; a < R1; ++a) S[(a * R2 + d) * RB + rp] = u[a];
+            }
+            __syncthreads();
+            for (int t = threadIdx.x; t < (Q + 1) * HB; t += C::NT) {
+                const int k = t / HB, rp = t - k * HB;
+                const int d = k % R2, cc = k / R2;
+                const int dp = (R2 - d) % R2, cp = d == 0 ? (R1 - cc) % R1 : R1 - 1 - cc;     // NY - k = dp + R2*cp
+                const float2 A = S[(cc * R2 + d) * RB + rp], B = S[(cp * R2 + dp) * RB + rp];
+                float2* __restrict__ W0 = W + (C::ADJ ? bt * RB + 2 * rp : bt * HB + rp) * NCOL;
+                float2* __restrict__ W1 = W0 + (C::ADJ ? 1 : NX / 2) * NCOL;
+                W0[k] = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));
+                W1[k] = make_float2(0.5f * (A.y + B.y), 0.5f * (B.x - A.x));
+            }
+        } else {
+            // ---- a6 (last y pass) + a7 (keep ky <= Q) + separation of the packed row pair
+            for (int t = threadIdx.x; t < (R2 / 2 + 1) * HB; t += C::NT) {
+                const int dd = t / HB, rp = t - dd * HB;
+                const int d0 = dd, d1 = (R2 - dd) % R2;
+                float2 u0[R1], u1[R1];
+#pragma unroll
+                for (int a = 0; a < R1; ++a) u0[a] = S[(a * R2 + d0) * RB + rp];
+                dft<R1, -1>(u0);
                 if (d1 != d0) {
-                    const int k = d1 + R2 * cc;
-                    if (k <= Q) {
-                        const float2 A = u1[cc];
-                        const float2 B = u0[R1 - 1 - cc];
-                        W0[k] = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));
-                        W1[k] = make_float2(0.5f * (A.y + B.y), 0.5f * (B.x - A.x));
+#pragma unroll
+                    for (int a = 0; a < R1; ++a) u1[a] = S[(a * R2 + d1) * RB + rp];
+                    dft<R1, -1>(u1);
+                } else {
+#pragma unroll
+                    for (int a = 0; a < R1; ++a) u1[a] = u0[a];
+                }
+                float2* __restrict__ W0 = W + (C::ADJ ? bt * RB + 2 * rp : bt * HB + rp) * NCOL;
+                float2* __restrict__ W1 = W0 + (C::ADJ ? 1 : NX / 2) * NCOL;
+#pragma unroll
+                for (int cc = 0; cc <= Q / R2; ++cc) {
+                    // class d0: k = d0 + R2*cc, partner NY-k in class d1
+                    {
+                        const int k = d0 + R2 * cc;
+                        if (k <= Q) {
+                            const float2 A = u0[cc];
+                            const float2 B = (d0 == 0) ? u1[(R1 - cc) % R1] : u1[R1 - 1 - cc];
+                            W0[k] = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));
+                            W1[k] = make_float2(0.5f * (A.y + B.y), 0.5f * (B.x - A.x));
+                        }
+                    }
+                    if (d1 != d0) {
+                        const int k = d1 + R2 * cc;
+                        if (k <= Q) {
+                            const float2 A = u1[cc];
+                            const float2 B = u0[R1 - 1 - cc];
+                            W0[k] = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));
+                            W1[k] = make_float2(0.5f * (A.y + B.y), 0.5f * (B.x - A.x));
+                        }
                     }
                 }
             }
