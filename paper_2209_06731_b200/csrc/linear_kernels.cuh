@@ -12,6 +12,8 @@
 
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
+#include <cstring>
 #include <string>
 #include <vector>
 
@@ -890,6 +892,121 @@ __global__ void __launch_bounds__(256) lin_point_kernel(LinTables t, const float
     }
 }
 
+// The same pointwise terms, marching along the Hermite index: one thread per (s, z, k) walks m = m0 .. m1-1 with the
+// five stencil planes H_{.,m-2..m+2} (all l) in registers, loads every G value exactly once (plane m+3 is requested
+// while m is evaluated) and reads the (s,z,k) tables once.  lin_point_kernel relies on L2 for the five-fold reuse
+// in m and keeps one batch of loads per thread in flight: ncu showed it latency-bound at 18 % of the DRAM bandwidth
+// (long scoreboard 7.7 per issue, 15 warps per SM; profiles/r02_linear.md).  gridDim.z splits the m range when
+// Ns*Nz*nk alone does not fill the machine (each chunk re-reads its four halo planes).
+template <int MAXL, bool ACC>
+__global__ void __launch_bounds__(128) lin_point_march_kernel(LinTables t, const float2* __restrict__ g,
+                                                              const float2* __restrict__ phi, float2* __restrict__ out,
+                                                              const int mchunk) {
+    const unsigned pl = (unsigned)(t.Nz * t.nk);
+    const unsigned zk = blockIdx.x * blockDim.x + threadIdx.x;
+    if (zk >= pl) return;
+    const int s = blockIdx.y;
+    const int m0 = blockIdx.z * mchunk, m1 = min(t.Nm, m0 + mchunk);
+    const int z = zk / t.nk, k = zk - z * t.nk;
+    const float zt = t.zt[s], vt = t.vt[s], tz = t.tz[s], nu = t.nu[s];
+    const float2 f = phi[zk];
+    float J[MAXL + 2];                                     // J[l + 1] = J_l, zero outside 0 <= l < Nl
+    J[0] = 0.f;
+#pragma unroll
+    for (int l = 0; l < MAXL; ++l) J[l + 1] = l < t.Nl ? t.Jl[(unsigned)(s * t.Nl + l) * pl + zk] : 0.f;
+    J[MAXL + 1] = 0.f;
+    const float bg = -vt * t.bgrad[z];
+    const float wk = tz * t.omd[zk], wb = tz * t.omd[pl + zk];
+    const float hv = t.hypv[zk];
+    const float dd = t.dend ? t.dend[zk] : 0.f;
+    const float ky = t.dky * (float)(k % t.naky);
+    const float b = t.bs[(unsigned)s * pl + zk];
+    const float sb = sqrtf(fmaxf(b, 0.f));
+    float2 up = make_float2(0.f, 0.f), uq = up, tb = up;
+    if (nu != 0.f && m0 <= 2) {
+        const float2* __restrict__ mo = t.mom + (size_t)s * 3 * pl + zk;
+        up = mo[0]; uq = mo[pl]; tb = mo[2 * (size_t)pl];
+    }
+    // H_{l,mm} = G_{l,mm} + (Z/tau) J_l Phi delta_{mm,0}; zero outside 0 <= mm < Nm, 0 <= l < Nl
+    auto load_plane = [&](const int mm, float2 (&row)[MAXL + 2]) {
+        row[0] = row[MAXL + 1] = make_float2(0.f, 0.f);
+        const bool mv = mm >= 0 && mm < t.Nm;
+        const int mc = min(max(mm, 0), t.Nm - 1);
+#pragma unroll
+        for (int l = 0; l < MAXL; ++l) {
+            float2 v = g[(unsigned)((s * t.Nm + mc) * t.Nl + min(l, t.Nl - 1)) * pl + zk];     // unconditional: all in flight
+            if (!(mv && l < t.Nl)) v = make_float2(0.f, 0.f);
+            else if (mm == 0) { v.x = fmaf(zt * J[l + 1], f.x, v.x); v.y = fmaf(zt * J[l + 1], f.y, v.y); }
+            row[l + 1] = v;
+        }
+    };
+    float2 h[6][MAXL + 2];                                 // h[i] = plane m - 2 + i; h[5] is the plane in flight
+#pragma unroll
+    for (int i = 0; i < 5; ++i) load_plane(m0 - 2 + i, h[i]);
+    for (int m = m0; m < m1; ++m) {
+        load_plane(m + 3, h[5]);
+        const float fm = (float)m;
+        const float sm1 = sqrtf(fm + 1.f), sm0 = sqrtf(fm);
+        const float cA = sqrtf((fm + 1.f) * (fm + 2.f)), cB = 2.f * fm + 1.f, cC = sqrtf(fm * fmaxf(fm - 1.f, 0.f));
+#pragma unroll
+        for (int l = 0; l < MAXL; ++l) {
+            if (l < t.Nl) {
+                const float fl = (float)l;
+                const float2 c0 = h[2][l + 1];
+                // mirror force
+                const float ca = -(fl + 1.f) * sm1, cb = -fl * sm1, cc = fl * sm0, cd = (fl + 1.f) * sm0;
+                float2 r;
+                r.x = bg * (ca * h[3][l + 1].x + cb * h[3][l].x + cc * h[1][l + 1].x + cd * h[1][l + 2].x);
+                r.y = bg * (ca * h[3][l + 1].y + cb * h[3][l].y + cc * h[1][l + 1].y + cd * h[1][l + 2].y);
+                // drifts: -i (tau/Z) w (...)
+                const float bx = wk * (cA * h[4][l + 1].x + cB * c0.x + cC * h[0][l + 1].x) +
+                                 wb * ((fl + 1.f) * h[2][l + 2].x + (2.f * fl + 1.f) * c0.x + fl * h[2][l].x);
+                const float by = wk * (cA * h[4][l + 1].y + cB * c0.y + cC * h[0][l + 1].y) +
+                                 wb * ((fl + 1.f) * h[2][l + 2].y + (2.f * fl + 1.f) * c0.y + fl * h[2][l].y);
+                r.x += by;
+                r.y -= bx;
+                const float jm = J[l], j0 = J[l + 1], jp = J[l + 2];
+                const float jt = fl * jm + 2.f * fl * j0 + (fl + 1.f) * jp;
+                if (m == 0 || m == 2) {                          // drive
+                    const float c = m == 0 ? t.fprim[s] * j0 + t.tprim[s] * jt : t.tprim[s] * j0 * 0.70710678118654752440f;
+                    r.x -= ky * c * f.y;
+                    r.y += ky * c * f.x;
+                }
+                if (nu != 0.f) {                                 // Dougherty
+                    const float damp = nu * (b + 2.f * fl + fm);
+                    r.x -= damp * c0.x;
+                    r.y -= damp * c0.y;
+                    if (m == 0) {
+                        const float cu = sb * (j0 + jm), ct = 2.f * jt;
+                        r.x = fmaf(nu, cu * uq.x + ct * tb.x, r.x);
+                        r.y = fmaf(nu, cu * uq.y + ct * tb.y, r.y);
+                    } else if (m == 1) {
+                        r.x = fmaf(nu * j0, up.x, r.x);
+                        r.y = fmaf(nu * j0, up.y, r.y);
+                    } else if (m == 2) {
+                        r.x = fmaf(nu * 1.41421356237309504880f * j0, tb.x, r.x);
+                        r.y = fmaf(nu * 1.41421356237309504880f * j0, tb.y, r.y);
+                    }
+                }
+                // hyper-viscosity acts on G, not H
+                const float gx_ = m == 0 ? c0.x - zt * j0 * f.x : c0.x, gy_ = m == 0 ? c0.y - zt * j0 * f.y : c0.y;
+                r.x -= hv * gx_;
+                r.y -= hv * gy_;
+                // wave-absorbing end layer (Eq. 4.30)
+                r.x -= dd * c0.x;
+                r.y -= dd * c0.y;
+                float2* __restrict__ o = out + ((unsigned)((s * t.Nm + m) * t.Nl + l) * pl + zk);
+                if (ACC) { const float2 prev = *o; r.x += prev.x; r.y += prev.y; }
+                *o = r;
+            }
+        }
+#pragma unroll
+        for (int i = 0; i < 5; ++i)
+#pragma unroll
+            for (int l = 0; l < MAXL + 2; ++l) h[i][l] = h[i + 1][l];
+    }
+}
+
 // Twist-and-shift linked z operators (Eq. 4.29): one block per (slice of a chain of linked modes,
 // l, (s,m)); the chain's extended periodic domain (L segments of Nz points, in order of increasing ballooning
 // angle) is staged in shared memory and the two circulant products of the slice's outputs are added to out.
@@ -991,6 +1108,26 @@ __global__ void __launch_bounds__(kZlinkThreads) lin_zlink_kernel(LinTables t, c
     }
 }
 
+// Launches the pointwise terms: the marching kernel (one thread per (s,z,k), m range split over gridDim.z until about
+// 300 k threads exist) unless GX_LIN_POINT=stencil asks for the per-(s,m) stencil kernel.
+template <int MAXL>
+inline void launch_lin_point(const LinTables& t, const float2* g, const float2* phi, float2* out, bool accumulate, cudaStream_t st) {
+    static const bool stencil = std::getenv("GX_LIN_POINT") && std::strcmp(std::getenv("GX_LIN_POINT"), "stencil") == 0;
+    const size_t pl = (size_t)t.Nz * t.nk;
+    if (stencil) {
+        dim3 gp(t.Ns * t.Nm, (unsigned)((pl + 255) / 256));
+        if (accumulate) lin_point_kernel<MAXL, true><<<gp, 256, 0, st>>>(t, g, phi, out);
+        else lin_point_kernel<MAXL, false><<<gp, 256, 0, st>>>(t, g, phi, out);
+        return;
+    }
+    int chunks = (int)((300000 + (size_t)t.Ns * pl - 1) / ((size_t)t.Ns * pl));
+    chunks = std::max(1, std::min(chunks, std::max(1, t.Nm / 2)));
+    const int mchunk = (t.Nm + chunks - 1) / chunks;
+    dim3 gp((unsigned)((pl + 127) / 128), t.Ns, (t.Nm + mchunk - 1) / mchunk);      // 128 threads: 117-183 registers each
+    if (accumulate) lin_point_march_kernel<MAXL, true><<<gp, 128, 0, st>>>(t, g, phi, out, mchunk);
+    else lin_point_march_kernel<MAXL, false><<<gp, 128, 0, st>>>(t, g, phi, out, mchunk);
+}
+
 // Opt-in shared-memory sizes of every linear kernel instantiation, on the current device (gx_grid_create: per
 // handle and per device, no process-wide cache).
 inline cudaError_t lin_prepare() {
@@ -1022,13 +1159,10 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
         dim3 gridf(t.Ns * t.Nm, t.Nl, (t.nk + kLinTK - 1) / kLinTK);
         const bool splitf = t.Nl <= 6;        // pointwise terms with the stencil in registers, z operators added on top
         if (splitf) {
-            dim3 gp(t.Ns * t.Nm, (unsigned)(((size_t)t.Nz * t.nk + 255) / 256));
             if (t.Nl <= 4) {
-                if (accumulate) lin_point_kernel<4, true><<<gp, 256, 0, st>>>(t, g, phi, out);
-                else lin_point_kernel<4, false><<<gp, 256, 0, st>>>(t, g, phi, out);
+                launch_lin_point<4>(t, g, phi, out, accumulate, st);
             } else {
-                if (accumulate) lin_point_kernel<6, true><<<gp, 256, 0, st>>>(t, g, phi, out);
-                else lin_point_kernel<6, false><<<gp, 256, 0, st>>>(t, g, phi, out);
+                launch_lin_point<6>(t, g, phi, out, accumulate, st);
             }
         }
 #define GX_ZFFT(FB)                                                                                                        \
@@ -1053,13 +1187,10 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
     if (split && t.Nl <= 8) {
         // pointwise terms with the stencil in registers, then the z-operator terms added on top (measured faster
         // for Nl <= 4 only: with 8 Laguerre moments the 5 x 10 stencil costs 135 registers and the occupancy)
-        dim3 gp(t.Ns * t.Nm, (unsigned)(((size_t)t.Nz * t.nk + 255) / 256));
         if (t.Nl <= 4) {
-            if (accumulate) lin_point_kernel<4, true><<<gp, 256, 0, st>>>(t, g, phi, out);
-            else lin_point_kernel<4, false><<<gp, 256, 0, st>>>(t, g, phi, out);
+            launch_lin_point<4>(t, g, phi, out, accumulate, st);
         } else {
-            if (accumulate) lin_point_kernel<8, true><<<gp, 256, 0, st>>>(t, g, phi, out);
-            else lin_point_kernel<8, false><<<gp, 256, 0, st>>>(t, g, phi, out);
+            launch_lin_point<8>(t, g, phi, out, accumulate, st);
         }
         if (!t.linked) {
             if (b4) lin_rhs_kernel<true, 4, true><<<grid, kLinTK * kLinZG, smem, st>>>(t, g, phi, out, false);
