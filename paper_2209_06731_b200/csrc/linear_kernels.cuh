@@ -610,18 +610,21 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
                        i0 = (unsigned)((s * t.Nm + m) * t.Nl + l) * pl, ij = (unsigned)(s * t.Nl + l) * pl;
         const float cp = vp ? sm1 : 0.f, cm = vm ? sm0 : 0.f;
         const float cphi = (vm && m == 1) ? sm0 * t.zt[s] : 0.f;          // H_{l,0} = G_{l,0} + (Z/tau) J_l Phi
-        for (int zb = zg; zb < t.Nz; zb += 4 * kLinZG) {
-            float2 a[4], b[4], c[4], f[4];
-            float jl[4];
+        // (the FFT path has Nz >= 64: eight z per thread and round trip; Phi and J_l only where they enter, m = 1)
+        constexpr int ZBATCH = FA > 0 ? 8 : 4;
+        for (int zb = zg; zb < t.Nz; zb += ZBATCH * kLinZG) {
+            float2 a[ZBATCH], b[ZBATCH], c[ZBATCH], f[ZBATCH];
+            float jl[ZBATCH];
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
+            for (int i = 0; i < ZBATCH; ++i) {
                 const int z = min(zb + i * kLinZG, t.Nz - 1);
                 const unsigned zk = (unsigned)(z * t.nk + kc);
                 a[i] = g[ip + zk]; b[i] = g[im + zk]; c[i] = g[i0 + zk];
-                f[i] = phi[zk]; jl[i] = t.Jl[ij + zk];
+                if (cphi != 0.f) { f[i] = phi[zk]; jl[i] = t.Jl[ij + zk]; }
+                else { f[i] = make_float2(0.f, 0.f); jl[i] = 0.f; }
             }
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
+            for (int i = 0; i < ZBATCH; ++i) {
                 const int z = zb + i * kLinZG;
                 if (z < t.Nz) {
                     const float w = cphi * jl[i];
@@ -641,6 +644,25 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
                              t.nuhyp[s] * t.mpow[m] * fabsf(t.gradpar), t.nuhyp[s] * t.mpow[m] != 0.f);
     }
     if (!live) return;
+    if constexpr (DERIV_ONLY && FA > 0) {
+        // out += (both z-operator terms): every previous value is requested before the first store -- the generic
+        // loop below reads and writes out once per z and the stores keep the next load from being issued early
+        // (16 dependent round trips per thread: the kernel ran at a sixth of the DRAM bandwidth)
+        constexpr int NZT = FA * FB / kLinZG;
+        static_assert(FA * FB % kLinZG == 0, "z per thread");
+        float2* __restrict__ o0 = out + ((unsigned)((s * t.Nm + m) * t.Nl + l) * (unsigned)(t.Nz * t.nk) + (unsigned)k);
+        float2 prev[NZT];
+#pragma unroll
+        for (int i = 0; i < NZT; ++i) prev[i] = o0[(unsigned)((zg + i * kLinZG) * t.nk)];
+        if (!skip_z) {
+#pragma unroll
+            for (int i = 0; i < NZT; ++i) {
+                const float2 r = S1[(zg + i * kLinZG) * kLinTK + tk];
+                o0[(unsigned)((zg + i * kLinZG) * t.nk)] = make_float2(prev[i].x + r.x, prev[i].y + r.y);
+            }
+        }
+        return;
+    }
     const float vt = t.vt[s], tz = t.tz[s], nu = t.nu[s];
     const float hyp = t.nuhyp[s] * t.mpow[m];
     const float ky = t.dky * (float)(k % t.naky);
