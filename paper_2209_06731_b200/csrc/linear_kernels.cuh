@@ -1205,10 +1205,11 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
     }
     dim3 grid(t.Ns * t.Nm, t.Nl, (t.nk + kLinTK - 1) / kLinTK);
     const bool b4 = t.Nz % 4 == 0;
-    const bool split = t.Nl <= 4 || t.linked;
+    static const bool fused8 = std::getenv("GX_LIN_FUSED8") != nullptr;      // development aid: the round-1 choice for Nl > 4
+    const bool split = t.Nl <= 4 || t.linked || !fused8;
     if (split && t.Nl <= 8) {
-        // pointwise terms with the stencil in registers, then the z-operator terms added on top (measured faster
-        // for Nl <= 4 only: with 8 Laguerre moments the 5 x 10 stencil costs 135 registers and the occupancy)
+        // pointwise terms (marching kernel), then the z-operator terms added on top.  With the per-(s,m) stencil kernel
+        // this paid for Nl <= 4 only (5 x 10 stencil values, 135 registers); with the marching kernel it pays for Nl = 8 too
         if (t.Nl <= 4) {
             launch_lin_point<4>(t, g, phi, out, accumulate, st);
         } else {
