@@ -716,6 +716,13 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
               }
           }
       }
+      // previous values of out for the whole z block before the first store (see the FFT path above)
+      float2 prevb[ZB];
+      if (ACC || DERIV_ONLY) {
+#pragma unroll
+          for (int zi = 0; zi < ZB; ++zi)
+              prevb[zi] = out[(unsigned)((s * t.Nm + m) * t.Nl + l) * (unsigned)(t.Nz * t.nk) + (unsigned)((z0 + zi) * t.nk + k)];
+      }
 #pragma unroll
       for (int zi = 0; zi < ZB; ++zi) {
         const int z = z0 + zi;
@@ -795,7 +802,7 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
         }
         }
         float2* __restrict__ o = out + ((unsigned)((s * t.Nm + m) * t.Nl + l) * (unsigned)(t.Nz * t.nk) + (unsigned)(z * t.nk + k));
-        if (ACC || DERIV_ONLY) { const float2 prev = *o; r.x += prev.x; r.y += prev.y; }
+        if (ACC || DERIV_ONLY) { r.x += prevb[zi].x; r.y += prevb[zi].y; }
         *o = r;
       }
     }
@@ -1131,7 +1138,7 @@ __global__ void __launch_bounds__(kZlinkThreads) lin_zlink_kernel(LinTables t, c
 }
 
 // Launches the pointwise terms: the marching kernel (one thread per (s,z,k), m range split over gridDim.z until about
-// 300 k threads exist) unless GX_LIN_POINT=stencil asks for the per-(s,m) stencil kernel.
+// 130 k threads exist) unless GX_LIN_POINT=stencil asks for the per-(s,m) stencil kernel.
 template <int MAXL>
 inline void launch_lin_point(const LinTables& t, const float2* g, const float2* phi, float2* out, bool accumulate, cudaStream_t st) {
     static const bool stencil = std::getenv("GX_LIN_POINT") && std::strcmp(std::getenv("GX_LIN_POINT"), "stencil") == 0;
@@ -1142,8 +1149,10 @@ inline void launch_lin_point(const LinTables& t, const float2* g, const float2* 
         else lin_point_kernel<MAXL, false><<<gp, 256, 0, st>>>(t, g, phi, out);
         return;
     }
-    int chunks = (int)((300000 + (size_t)t.Ns * pl - 1) / ((size_t)t.Ns * pl));
-    chunks = std::max(1, std::min(chunks, std::max(1, t.Nm / 2)));
+    int chunks = (int)((130000 + (size_t)t.Ns * pl - 1) / ((size_t)t.Ns * pl));     // measured: 2 chunks for Cyclone and kinetic, 1 above
+    static const int forced = std::getenv("GX_LIN_CHUNKS") ? std::atoi(std::getenv("GX_LIN_CHUNKS")) : 0;     // tuning aid
+    if (forced > 0) chunks = forced;
+    chunks = std::max(1, std::min(chunks, std::max(1, t.Nm / (forced > 0 ? 1 : 2))));
     const int mchunk = (t.Nm + chunks - 1) / chunks;
     dim3 gp((unsigned)((pl + 127) / 128), t.Ns, (t.Nm + mchunk - 1) / mchunk);      // 128 threads: 117-183 registers each
     if (accumulate) lin_point_march_kernel<MAXL, true><<<gp, 128, 0, st>>>(t, g, phi, out, mchunk);
