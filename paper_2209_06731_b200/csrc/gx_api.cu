@@ -560,13 +560,21 @@ int nl_enqueue(gx_grid* g, NlParams p, int Nm_eff, bool do_chi, unsigned* count,
         const int nk = (int)g->nk;
         if (before_out) GX_CUDA(g, cudaStreamWaitEvent(st, before_out, 0));
         cudaError_t e;
-#define GX_LAGINV(L, J)                                                                                        \
-    e = (vec == 2) ? launch_pdl(gx::laguerre_inverse_kernel<L, J, 2>, grid, dim3(256), 0, st, p, nk, target)  \
-                   : launch_pdl(gx::laguerre_inverse_kernel<L, J, 1>, grid, dim3(256), 0, st, p, nk, target)
+        const int mode = p.st_out ? 2 : (p.accumulate ? 1 : 0);
+#define GX_LAGINV_M(L, J, M)                                                                                      \
+    e = (vec == 2) ? launch_pdl(gx::laguerre_inverse_kernel<L, J, 2, M>, grid, dim3(256), 0, st, p, nk, target)  \
+                   : launch_pdl(gx::laguerre_inverse_kernel<L, J, 1, M>, grid, dim3(256), 0, st, p, nk, target)
+#define GX_LAGINV(L, J)                                                                  \
+    do {                                                                                 \
+        if (mode == 2) GX_LAGINV_M(L, J, 2);                                            \
+        else if (mode == 1) GX_LAGINV_M(L, J, 1);                                       \
+        else GX_LAGINV_M(L, J, 0);                                                      \
+    } while (0)
         if (g->Nl <= 4) GX_LAGINV(4, 5);
         else if (g->Nl <= 8) GX_LAGINV(8, 11);
         else GX_LAGINV(16, 23);
 #undef GX_LAGINV
+#undef GX_LAGINV_M
         GX_CUDA(g, e);
     }
     if (ev) GX_CUDA(g, cudaEventRecord(ev[3], st));
@@ -812,7 +820,20 @@ int gx_linear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_
     return GX_OK;
 }
 
+namespace {
+// One Runge-Kutta stage st.out = a y0 + b (y + dt rhs).  Where the right-hand side ends in the separate inverse-Laguerre
+// kernel, that kernel applies the stage itself (the rhs is then never stored: two passes over the state saved).
+struct RkStage { const float2* y0; const float2* y; float2* out; float a, b, dt; };
+int rhs_impl(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream, const RkStage* stage, bool* folded);
+}  // namespace
+
 int gx_rhs(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream) {
+    return rhs_impl(g, g_dev, out_dev, cuda_stream, nullptr, nullptr);
+}
+
+namespace {
+int rhs_impl(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream, const RkStage* stage, bool* folded) {
+    if (folded) *folded = false;
     if (!g) return GX_ERR_ARG;
     if (!g_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_rhs: null pointer");
     if (overlap(g_dev, out_dev, (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk * sizeof(float2)))
@@ -844,8 +865,14 @@ int gx_rhs(gx_grid* g, const void* g_dev, void* out_dev, void* cuda_stream) {
     GX_CUDA(g, cudaEventRecord(g->ev_lin, g->st_lin));
     NlParams p = make_params(g, g_dev, g->dphi_rhs, out_dev);
     p.accumulate = 1;
+    if (stage && std::getenv("GX_RK_UNFUSED") == nullptr) {
+        p.st_y0 = stage->y0; p.st_y = stage->y; p.st_out = stage->out;
+        p.st_a = stage->a; p.st_b = stage->b; p.st_dt = stage->dt;
+        if (folded) *folded = true;
+    }
     return nl_enqueue(g, p, g->Nm, true, g->dcount, &g->calls, st, nullptr, g->ev_lin);
 }
+}  // namespace
 
 int gx_ssprk3_step(gx_grid* g, void* g_dev, double dt, void* cuda_stream) {
     if (!g) return GX_ERR_ARG;
@@ -861,12 +888,18 @@ int gx_ssprk3_step(gx_grid* g, void* g_dev, double dt, void* cuda_stream) {
     float2* y0 = (float2*)g_dev;
     const float h = (float)dt;
     const int blocks = (int)std::min<size_t>((n + 255) / 256, 148 * 16);
-    if ((rc = gx_rhs(g, y0, g->drk_k, cuda_stream))) return rc;
-    gx::rk_stage_kernel<<<blocks, 256, 0, st>>>(g->drk_y, y0, y0, g->drk_k, 0.f, 1.f, h, n);              // g1
-    if ((rc = gx_rhs(g, g->drk_y, g->drk_k, cuda_stream))) return rc;
-    gx::rk_stage_kernel<<<blocks, 256, 0, st>>>(g->drk_y, y0, g->drk_y, g->drk_k, 0.75f, 0.25f, h, n);    // g2
-    if ((rc = gx_rhs(g, g->drk_y, g->drk_k, cuda_stream))) return rc;
-    gx::rk_stage_kernel<<<blocks, 256, 0, st>>>(y0, y0, g->drk_y, g->drk_k, 1.f / 3.f, 2.f / 3.f, h, n);  // g(t+dt)
+    // Stage results may overwrite the state the right-hand side was evaluated on (stage 2): the inverse-Laguerre block
+    // of an (s,m,z) runs after every bracket unit of that (s,m,z) has arrived and after the linear kernels (event),
+    // and no other unit reads those planes.
+    const RkStage stages[3] = {{y0, y0, g->drk_y, 0.f, 1.f, h},                              // g1
+                               {y0, g->drk_y, g->drk_y, 0.75f, 0.25f, h},                    // g2
+                               {y0, g->drk_y, y0, 1.f / 3.f, 2.f / 3.f, h}};                 // g(t+dt)
+    for (int i = 0; i < 3; ++i) {
+        bool folded = false;
+        if ((rc = rhs_impl(g, i == 0 ? y0 : g->drk_y, g->drk_k, cuda_stream, &stages[i], &folded))) return rc;
+        if (!folded)
+            gx::rk_stage_kernel<<<blocks, 256, 0, st>>>(stages[i].out, stages[i].y0, stages[i].y, g->drk_k, stages[i].a, stages[i].b, h, n);
+    }
     GX_CUDA(g, cudaGetLastError());
     return GX_OK;
 }

@@ -110,6 +110,11 @@ struct NlParams {
     // finished reading dchi; the chi grid of a call may overwrite its dchi buffer once done >= chi_need
     unsigned* done;
     unsigned chi_need;
+    // Runge-Kutta stage folded into the separate inverse-Laguerre kernel (gx_ssprk3_step): st_out = a y0 + b (y + dt rhs)
+    const float2* st_y0;
+    const float2* st_y;
+    float2* st_out;       // nullptr: off
+    float st_a, st_b, st_dt;
     int cluster;          // row family: the J node units of an (s,m,z) are one thread-block cluster (a8 over distributed shared memory)
     unsigned* chi_ready;  // chained calls: [s][z][j] of the current dchi buffer, epoch of the call that wrote the plane
     unsigned chi_epoch;
@@ -693,7 +698,8 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
 // when nk is even, else 1.  Launched with PDL: blocks become resident during the bracket kernel's last
 // wave and wait until the J node-units of their (s,m,z) have arrived (count >= target; the counters
 // grow by J per call, target = J * call number, so nothing is ever reset).
-template <int MAXL, int MAXJ, int VEC>
+// MODE 0: out = -N; 1: out += -N (gx_rhs: linear terms already there); 2: Runge-Kutta stage on top of mode 1.
+template <int MAXL, int MAXJ, int VEC, int MODE = 0>
 __global__ void __launch_bounds__(256) laguerre_inverse_kernel(const NlParams p, int nk, unsigned target) {
     using V = typename std::conditional<VEC == 2, float4, float2>::type;
     const int kv = blockIdx.x * blockDim.x + threadIdx.x;      // index in units of VEC complex
@@ -718,28 +724,55 @@ __global__ void __launch_bounds__(256) laguerre_inverse_kernel(const NlParams p,
     for (int j = 0; j < MAXJ; ++j)
         if (j < p.J)
             b[j] = __ldcg(reinterpret_cast<const V*>(p.bhat + ((size_t)((s * p.Nz + z) * p.J + j) * p.Nm + m) * nk) + kv);
+    // Moments in groups of four: what the result is combined with (the linear terms already in out: gx_rhs; the two
+    // states of a Runge-Kutta stage: gx_ssprk3_step) is requested for the whole group before its first store.
+    constexpr bool stage = MODE == 2, accumulate = MODE >= 1;
 #pragma unroll
-    for (int l = 0; l < MAXL; ++l) {
-        if (l < p.Nl) {
-            float acc[2 * VEC];
+    for (int l0 = 0; l0 < MAXL; l0 += 4) {
+        V prev[accumulate ? 4 : 1], vy0[stage ? 4 : 1], vy[stage ? 4 : 1];
 #pragma unroll
-            for (int c = 0; c < 2 * VEC; ++c) acc[c] = 0.f;
-#pragma unroll
-            for (int j = 0; j < MAXJ; ++j)
-                if (j < p.J) {
-                    const float t = Ti[l * p.J + j];
-                    const float* bj = reinterpret_cast<const float*>(&b[j]);
-#pragma unroll
-                    for (int c = 0; c < 2 * VEC; ++c) acc[c] = fmaf(t, bj[c], acc[c]);
+        for (int dl = 0; dl < 4; ++dl) {
+            const int l = l0 + dl;
+            if (l < p.Nl && accumulate) {
+                const size_t idx = (((size_t)(s * p.Nm + m) * p.Nl + l) * p.Nz + z) * nk;
+                prev[dl] = *(reinterpret_cast<const V*>(p.out + idx) + kv);
+                if constexpr (stage) {
+                    vy0[dl] = *(reinterpret_cast<const V*>(p.st_y0 + idx) + kv);
+                    vy[dl] = *(reinterpret_cast<const V*>(p.st_y + idx) + kv);
                 }
-            V* dst = reinterpret_cast<V*>(p.out + (((size_t)(s * p.Nm + m) * p.Nl + l) * p.Nz + z) * nk) + kv;
-            if (p.accumulate) {                      // gx_rhs: the linear terms are already in out (written concurrently)
-                const V prev = *dst;
-                const float* pv = reinterpret_cast<const float*>(&prev);
-#pragma unroll
-                for (int c = 0; c < 2 * VEC; ++c) acc[c] += pv[c];
             }
-            *dst = *reinterpret_cast<V*>(acc);
+        }
+#pragma unroll
+        for (int dl = 0; dl < 4; ++dl) {
+            const int l = l0 + dl;
+            if (l < p.Nl) {
+                float acc[2 * VEC];
+#pragma unroll
+                for (int c = 0; c < 2 * VEC; ++c) acc[c] = 0.f;
+#pragma unroll
+                for (int j = 0; j < MAXJ; ++j)
+                    if (j < p.J) {
+                        const float t = Ti[l * p.J + j];
+                        const float* bj = reinterpret_cast<const float*>(&b[j]);
+#pragma unroll
+                        for (int c = 0; c < 2 * VEC; ++c) acc[c] = fmaf(t, bj[c], acc[c]);
+                    }
+                const size_t idx = (((size_t)(s * p.Nm + m) * p.Nl + l) * p.Nz + z) * nk;
+                if constexpr (accumulate) {          // gx_rhs: the linear terms are already in out (written concurrently)
+                    const float* pv = reinterpret_cast<const float*>(&prev[dl]);
+#pragma unroll
+                    for (int c = 0; c < 2 * VEC; ++c) acc[c] += pv[c];
+                }
+                if constexpr (stage) {               // SSP-RK3 stage: st_out = a y0 + b (y + dt rhs); rhs itself is not stored
+                    const float* a0 = reinterpret_cast<const float*>(&vy0[dl]);
+                    const float* a1 = reinterpret_cast<const float*>(&vy[dl]);
+#pragma unroll
+                    for (int c = 0; c < 2 * VEC; ++c) acc[c] = fmaf(p.st_a, a0[c], p.st_b * fmaf(p.st_dt, acc[c], a1[c]));
+                    *(reinterpret_cast<V*>(p.st_out + idx) + kv) = *reinterpret_cast<V*>(acc);
+                } else {
+                    *(reinterpret_cast<V*>(p.out + idx) + kv) = *reinterpret_cast<V*>(acc);
+                }
+            }
         }
     }
 }
