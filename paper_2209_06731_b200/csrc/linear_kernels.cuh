@@ -1141,7 +1141,8 @@ __global__ void __launch_bounds__(kZlinkThreads) lin_zlink_kernel(LinTables t, c
 // 130 k threads exist) unless GX_LIN_POINT=stencil asks for the per-(s,m) stencil kernel.
 template <int MAXL>
 inline void launch_lin_point(const LinTables& t, const float2* g, const float2* phi, float2* out, bool accumulate, cudaStream_t st) {
-    static const bool stencil = std::getenv("GX_LIN_POINT") && std::strcmp(std::getenv("GX_LIN_POINT"), "stencil") == 0;
+    const char* lp = std::getenv("GX_LIN_POINT");            // read per call: the tests switch it
+    const bool stencil = lp && std::strcmp(lp, "stencil") == 0;
     const size_t pl = (size_t)t.Nz * t.nk;
     if (stencil) {
         dim3 gp(t.Ns * t.Nm, (unsigned)((pl + 255) / 256));

@@ -475,9 +475,13 @@ def _oracle_lin(cfg, geo, G, Phi):
     return OL.linear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species)
 
 
+@pytest.mark.parametrize("point", ["march", "stencil"])
 @pytest.mark.parametrize("name", ["tiny", "cyclone", "kinetic", "w7x-shape"])
-def test_linear_rhs_parity(torch_cuda, name):
+def test_linear_rhs_parity(torch_cuda, monkeypatch, name, point):
+    """point: the pointwise terms by the marching kernel (default) or by the per-(s,m) stencil kernel (GX_LIN_POINT)."""
     torch = torch_cuda
+    if point == "stencil":
+        monkeypatch.setenv("GX_LIN_POINT", "stencil")
     cfg = I.named_config(name)
     if name == "w7x-shape":
         cfg = I.Config(cfg.name, cfg.Nx, cfg.Ny, cfg.Nz, cfg.Nl, 4, cfg.species, geometry=cfg.geometry, seed=cfg.seed)
