@@ -610,8 +610,40 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
                        i0 = (unsigned)((s * t.Nm + m) * t.Nl + l) * pl, ij = (unsigned)(s * t.Nl + l) * pl;
         const float cp = vp ? sm1 : 0.f, cm = vm ? sm0 : 0.f;
         const float cphi = (vm && m == 1) ? sm0 * t.zt[s] : 0.f;          // H_{l,0} = G_{l,0} + (Z/tau) J_l Phi
-        // (the FFT path has Nz >= 64: eight z per thread and round trip; Phi and J_l only where they enter, m = 1)
-        constexpr int ZBATCH = FA > 0 ? 8 : 4;
+        if constexpr (FA > 0) {
+            // FFT path (Nz >= 64): the three input planes go to shared memory with cp.async -- all Nz/ZG x 3 requests of
+            // a thread in flight at once, no registers held -- and are combined in place afterwards
+            constexpr int NZT = FA * FB / kLinZG;
+            auto cp8 = [](float2* dst, const float2* src) {
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
+            };
+#pragma unroll
+            for (int i = 0; i < NZT; ++i) {
+                const int z = zg + i * kLinZG;
+                const unsigned zk = (unsigned)(z * t.nk + kc);
+                cp8(S1 + z * kLinTK + tk, g + ip + zk);
+                cp8(S3 + z * kLinTK + tk, g + im + zk);
+                cp8(S2 + z * kLinTK + tk, g + i0 + zk);
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+#pragma unroll
+            for (int i = 0; i < NZT; ++i) {
+                const int z = zg + i * kLinZG;
+                const float2 a = S1[z * kLinTK + tk], b = S3[z * kLinTK + tk];
+                float2 r = make_float2(cp * a.x + cm * b.x, cp * a.y + cm * b.y);
+                if (cphi != 0.f) {
+                    const unsigned zk = (unsigned)(z * t.nk + kc);
+                    const float2 f = phi[zk];
+                    const float w = cphi * t.Jl[ij + zk];
+                    r.x = fmaf(w, f.x, r.x); r.y = fmaf(w, f.y, r.y);
+                }
+                S1[z * kLinTK + tk] = live ? r : make_float2(0.f, 0.f);
+                if (!live) S2[z * kLinTK + tk] = make_float2(0.f, 0.f);
+            }
+        } else {
+        // (circulant path: four z per thread and round trip; Phi and J_l only where they enter, m = 1)
+        constexpr int ZBATCH = 4;
         for (int zb = zg; zb < t.Nz; zb += ZBATCH * kLinZG) {
             float2 a[ZBATCH], b[ZBATCH], c[ZBATCH], f[ZBATCH];
             float jl[ZBATCH];
@@ -634,6 +666,7 @@ __global__ void __launch_bounds__(kLinTK * kLinZG) lin_rhs_kernel(LinTables t, c
                     S2[z * kLinTK + tk] = live ? c[i] : make_float2(0.f, 0.f);
                 }
             }
+        }
         }
     }
     __syncthreads();
