@@ -491,7 +491,7 @@ __global__ void __launch_bounds__(256) lin_moments_kernel(LinTables t, const flo
     mo[2 * st] = make_float2((r2 * tp.x + 2.f * tq.x) * (1.f / 3.f), (r2 * tp.y + 2.f * tq.y) * (1.f / 3.f));
 }
 
-constexpr int kLinTK = 32;      // k per block
+constexpr int kLinTK = 16;      // k per block
 constexpr int kLinZG = 8;       // z groups per block
 
 // Spectral z operators by FFT (Eq. 4.10-4.11) for long field lines: for every column tk of the tile
