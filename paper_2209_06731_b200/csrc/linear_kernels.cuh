@@ -62,6 +62,8 @@ struct LinTables {
     int* ext_off = nullptr;        // [nchain] offset of the chain's circulant columns in ext_d / ext_a
     int* zwork = nullptr;          // [nzwork] (chain << 8 | slice): slices of kZlinkSlice outputs, longest chains first
     int nzwork = 0, nzwork_long = 0, short_ext = 0;   // items [0, nzwork_long) have more than short_ext points
+    int* zlong = nullptr;          // [nzlong] chains with more than short_ext points, longest first (lin_zlink_spectral_kernel)
+    int nzlong = 0;
     float* ext_d = nullptr;        // per distinct length L: column of gradpar * d/dzeta, L*Nz entries
     float* ext_a = nullptr;        // per distinct length L: column of |gradpar| * |k_zeta|
     float2* mom = nullptr;     // [s][3][z][k] workspace: u_par, u_perp, T of the Dougherty operator
@@ -78,7 +80,7 @@ inline void lin_tables_free(LinTables& t) {
     cudaFree(t.Jl); cudaFree(t.invD); cudaFree(t.fsfac); cudaFree(t.wz); cudaFree(t.bs);
     cudaFree(t.Dz); cudaFree(t.Az); cudaFree(t.twz); cudaFree(t.omd); cudaFree(t.hypv); cudaFree(t.dend); cudaFree(t.bgrad);
     cudaFree(t.mpow); cudaFree(t.mom);
-    cudaFree(t.chain_off); cudaFree(t.chain_mode); cudaFree(t.ext_off); cudaFree(t.ext_d); cudaFree(t.ext_a); cudaFree(t.zwork);
+    cudaFree(t.chain_off); cudaFree(t.chain_mode); cudaFree(t.ext_off); cudaFree(t.ext_d); cudaFree(t.ext_a); cudaFree(t.zwork); cudaFree(t.zlong);
     t = LinTables();
 }
 
@@ -254,6 +256,11 @@ inline bool lin_tables_build(const LinHostInput& in, LinTables& t, size_t& bytes
             if ((coff[(w >> 8) + 1] - coff[w >> 8]) * Nz > t.short_ext) t.nzwork_long++;
         if (max_ext > 255 * kZlinkSlice) { msg = "extended domain too long for the slice encoding"; return false; }
         if (!lin_upload(&t.zwork, work, bytes, msg)) return false;
+        std::vector<int> zlong;
+        for (int c : order)
+            if ((coff[c + 1] - coff[c]) * Nz > t.short_ext) zlong.push_back(c);
+        t.nzlong = (int)zlong.size();
+        if (t.nzlong > 0 && !lin_upload(&t.zlong, zlong, bytes, msg)) return false;
         if (!lin_upload(&t.chain_off, coff, bytes, msg) || !lin_upload(&t.chain_mode, cmode, bytes, msg) ||
             !lin_upload(&t.ext_off, eoff, bytes, msg) || !lin_upload(&t.ext_d, ed, bytes, msg) ||
             !lin_upload(&t.ext_a, ea, bytes, msg))
@@ -1170,6 +1177,135 @@ __global__ void __launch_bounds__(kZlinkThreads) lin_zlink_kernel(LinTables t, c
     }
 }
 
+// The same two operators for the LONG chains, in the harmonics of the extended domain.  N = L*Nz factorises: with point
+// n = Nz*n1 + n2 (segment n1, point n2) and harmonic jj = k1 + L*k2,
+//   X[k1 + L k2] = sum_n2 W_Nz^{n2 k2} W_N^{n2 k1} sum_n1 W_L^{n1 k1} x[Nz n1 + n2],        W_M = e^{-2 pi i/M},
+// i.e. a dense DFT over the L segments for every point of a segment, a twiddle and a dense Nz-point DFT per k1:
+// N (L + Nz) multiply-adds per transform instead of the N^2 of the circulant product (N up to 26 x 24 = 624 on the Cyclone
+// grid).  The operators are diagonal there, grad_par -> i gradpar j/L and |k_par| -> |gradpar| |j|/L for the signed
+// harmonic j (Nyquist dropped for the derivative, as in the table build above); one inverse transform of their sum.
+// One block per (chain, l, (s,m)); shared memory: X1, X2, T1, T2, W_N tables of N complex, W_L, W_Nz, the chain's modes.
+constexpr int kZspecThreads = 128;
+__global__ void __launch_bounds__(kZspecThreads) lin_zlink_spectral_kernel(LinTables t, const float2* __restrict__ g,
+                                                                          const float2* __restrict__ phi,
+                                                                          float2* __restrict__ out, const int cap) {
+    extern __shared__ __align__(16) unsigned char lin_smem[];
+    const int c = t.zlong[blockIdx.x];
+    const int s = blockIdx.z / t.Nm, m = blockIdx.z % t.Nm, l = blockIdx.y;
+    const int off = t.chain_off[c], L = t.chain_off[c + 1] - off, Nz = t.Nz, N = L * Nz;
+    float2* X1 = reinterpret_cast<float2*>(lin_smem);      // sqrt(m+1) H_{l,m+1} + sqrt(m) H_{l,m-1}; later the spectrum of the sum
+    float2* X2 = X1 + cap;                                  // G_{l,m}
+    float2* T1 = X2 + cap;
+    float2* T2 = T1 + cap;
+    float2* WN = T2 + cap;                                  // e^{-2 pi i j/N}
+    float2* WL = WN + cap;                                  // e^{-2 pi i j/L}, L <= cap/Nz
+    float2* WZ = WL + cap / Nz;                             // e^{-2 pi i j/Nz}
+    int* modes = reinterpret_cast<int*>(WZ + Nz);
+    const int tid = threadIdx.x;
+    for (int i = tid; i < N; i += kZspecThreads) { float sn, cs; sincospif(-2.f * (float)i / (float)N, &sn, &cs); WN[i] = make_float2(cs, sn); }
+    for (int i = tid; i < L; i += kZspecThreads) { float sn, cs; sincospif(-2.f * (float)i / (float)L, &sn, &cs); WL[i] = make_float2(cs, sn); modes[i] = t.chain_mode[off + i]; }
+    for (int i = tid; i < Nz; i += kZspecThreads) { float sn, cs; sincospif(-2.f * (float)i / (float)Nz, &sn, &cs); WZ[i] = make_float2(cs, sn); }
+    const unsigned pl = (unsigned)(Nz * t.nk);
+    const bool vp = m + 1 < t.Nm, vm = m - 1 >= 0;
+    const float cp = vp ? sqrtf((float)(m + 1)) : 0.f, cm = vm ? sqrtf((float)m) : 0.f;
+    const float cphi = (vm && m == 1) ? cm * t.zt[s] : 0.f;
+    const float hyp = t.nuhyp[s] * t.mpow[m], vt = t.vt[s];
+    const unsigned ip = (unsigned)((s * t.Nm + (vp ? m + 1 : m)) * t.Nl + l) * pl,
+                   im = (unsigned)((s * t.Nm + (vm ? m - 1 : m)) * t.Nl + l) * pl,
+                   i0 = (unsigned)((s * t.Nm + m) * t.Nl + l) * pl, ij = (unsigned)(s * t.Nl + l) * pl;
+    __syncthreads();
+    for (int i = tid; i < N; i += kZspecThreads) {
+        const int seg = i / Nz, z = i - seg * Nz;
+        const unsigned zk = (unsigned)(z * t.nk + modes[seg]);
+        const float2 a = g[ip + zk], b = g[im + zk];
+        float2 v = make_float2(cp * a.x + cm * b.x, cp * a.y + cm * b.y);
+        if (cphi != 0.f) {
+            const float w = cphi * t.Jl[ij + zk];
+            const float2 f = phi[zk];
+            v.x = fmaf(w, f.x, v.x);
+            v.y = fmaf(w, f.y, v.y);
+        }
+        X1[i] = v;
+        X2[i] = g[i0 + zk];
+    }
+    __syncthreads();
+    const bool with_hyp = hyp != 0.f;
+    // ---- forward, step A: T[k1*Nz + n2] = W_N^{n2 k1} sum_n1 W_L^{n1 k1} x[Nz n1 + n2]
+    for (int i = tid; i < N; i += kZspecThreads) {
+        const int k1 = i / Nz, n2 = i - k1 * Nz;
+        float2 a1 = make_float2(0.f, 0.f), a2 = a1;
+        int w = 0;                                          // (n1 k1) mod L
+        for (int n1 = 0; n1 < L; ++n1) {
+            const float2 tw = WL[w];
+            const float2 x1 = X1[n1 * Nz + n2];
+            a1.x = fmaf(tw.x, x1.x, fmaf(-tw.y, x1.y, a1.x)); a1.y = fmaf(tw.x, x1.y, fmaf(tw.y, x1.x, a1.y));
+            if (with_hyp) {
+                const float2 x2 = X2[n1 * Nz + n2];
+                a2.x = fmaf(tw.x, x2.x, fmaf(-tw.y, x2.y, a2.x)); a2.y = fmaf(tw.x, x2.y, fmaf(tw.y, x2.x, a2.y));
+            }
+            w += k1; if (w >= L) w -= L;
+        }
+        const float2 tn = WN[(n2 * k1) % N];
+        T1[i] = make_float2(a1.x * tn.x - a1.y * tn.y, a1.x * tn.y + a1.y * tn.x);
+        T2[i] = make_float2(a2.x * tn.x - a2.y * tn.y, a2.x * tn.y + a2.y * tn.x);
+    }
+    __syncthreads();
+    // ---- forward, step B: X[k1 + L k2] = sum_n2 W_Nz^{n2 k2} T[k1*Nz + n2]; the operators; the sum's spectrum -> X1[k1*Nz + k2]
+    const float cd = -vt * t.gradpar / (float)L, ca = -hyp * fabsf(t.gradpar) / (float)L;
+    for (int i = tid; i < N; i += kZspecThreads) {
+        const int k1 = i / Nz, kk2 = i - k1 * Nz;
+        float2 b1 = make_float2(0.f, 0.f), b2 = b1;
+        int w = 0;                                          // (n2 k2) mod Nz
+        for (int n2 = 0; n2 < Nz; ++n2) {
+            const float2 tw = WZ[w];
+            const float2 x1 = T1[k1 * Nz + n2];
+            b1.x = fmaf(tw.x, x1.x, fmaf(-tw.y, x1.y, b1.x)); b1.y = fmaf(tw.x, x1.y, fmaf(tw.y, x1.x, b1.y));
+            if (with_hyp) {
+                const float2 x2 = T2[k1 * Nz + n2];
+                b2.x = fmaf(tw.x, x2.x, fmaf(-tw.y, x2.y, b2.x)); b2.y = fmaf(tw.x, x2.y, fmaf(tw.y, x2.x, b2.y));
+            }
+            w += kk2; if (w >= Nz) w -= Nz;
+        }
+        const int jj = k1 + L * kk2;
+        const int j = jj <= N / 2 ? jj : jj - N;
+        const float fd = (N % 2 == 0 && jj == N / 2) ? 0.f : cd * (float)j;      // -v_t * (i gradpar j/L): times i below
+        const float fa = ca * fabsf((float)j);
+        X1[i] = make_float2(-fd * b1.y + fa * b2.x, fd * b1.x + fa * b2.y);
+    }
+    __syncthreads();
+    // ---- inverse, step C: U[k1*Nz + n2] = conj W_N^{n2 k1} sum_k2 conj W_Nz^{n2 k2} Y[k1 + L k2]
+    for (int i = tid; i < N; i += kZspecThreads) {
+        const int k1 = i / Nz, n2 = i - k1 * Nz;
+        float2 u = make_float2(0.f, 0.f);
+        int w = 0;
+        for (int kk2 = 0; kk2 < Nz; ++kk2) {
+            const float2 tw = WZ[w];
+            const float2 y = X1[k1 * Nz + kk2];
+            u.x = fmaf(tw.x, y.x, fmaf(tw.y, y.y, u.x)); u.y = fmaf(tw.x, y.y, fmaf(-tw.y, y.x, u.y));      // y * conj(tw)
+            w += n2; if (w >= Nz) w -= Nz;
+        }
+        const float2 tn = WN[(n2 * k1) % N];
+        T1[i] = make_float2(u.x * tn.x + u.y * tn.y, u.y * tn.x - u.x * tn.y);
+    }
+    __syncthreads();
+    // ---- inverse, step D: y[Nz n1 + n2] = (1/N) sum_k1 conj W_L^{n1 k1} U[k1*Nz + n2]; added to out
+    const float rn = 1.f / (float)N;
+    for (int i = tid; i < N; i += kZspecThreads) {
+        const int n1 = i / Nz, n2 = i - n1 * Nz;
+        float2* __restrict__ o = out + (i0 + (unsigned)(n2 * t.nk + modes[n1]));
+        const float2 prev = *o;                             // requested before the sum
+        float2 y = make_float2(0.f, 0.f);
+        int w = 0;
+        for (int k1 = 0; k1 < L; ++k1) {
+            const float2 tw = WL[w];
+            const float2 u = T1[k1 * Nz + n2];
+            y.x = fmaf(tw.x, u.x, fmaf(tw.y, u.y, y.x)); y.y = fmaf(tw.x, u.y, fmaf(-tw.y, u.x, y.y));
+            w += n1; if (w >= L) w -= L;
+        }
+        *o = make_float2(fmaf(rn, y.x, prev.x), fmaf(rn, y.y, prev.y));
+    }
+}
+
 // Launches the pointwise terms: the marching kernel (one thread per (s,z,k), m range split over gridDim.z until about
 // 130 k threads exist) unless GX_LIN_POINT=stencil asks for the per-(s,m) stencil kernel.
 template <int MAXL>
@@ -1205,7 +1341,7 @@ inline cudaError_t lin_prepare() {
     GX_ATTR((lin_rhs_kernel<true, 1, true, 8, 8>));   GX_ATTR((lin_rhs_kernel<true, 1, false, 8, 8>));   GX_ATTR((lin_rhs_kernel<false, 1, false, 8, 8>));
     GX_ATTR((lin_rhs_kernel<true, 1, true, 8, 12>));  GX_ATTR((lin_rhs_kernel<true, 1, false, 8, 12>));  GX_ATTR((lin_rhs_kernel<false, 1, false, 8, 12>));
     GX_ATTR((lin_rhs_kernel<true, 1, true, 8, 16>));  GX_ATTR((lin_rhs_kernel<true, 1, false, 8, 16>));  GX_ATTR((lin_rhs_kernel<false, 1, false, 8, 16>));
-    GX_ATTR(lin_zlink_kernel<4>);  GX_ATTR(lin_zlink_kernel<1>);
+    GX_ATTR(lin_zlink_kernel<4>);  GX_ATTR(lin_zlink_kernel<1>);  GX_ATTR(lin_zlink_spectral_kernel);
 #undef GX_ATTR
     return e;
 }
@@ -1274,7 +1410,16 @@ inline cudaError_t lin_rhs(const LinTables& t, const float2* g, const float2* ph
         // (up to 4 links) with a small footprint so that 32 blocks fit an SM
         const int w0[2] = {0, t.nzwork_long}, wn[2] = {t.nzwork_long, t.nzwork - t.nzwork_long};
         const int cap[2] = {t.max_ext, t.short_ext};
-        for (int part = 0; part < 2; ++part) {
+        const char* zl = std::getenv("GX_ZLINK");               // "dense": the circulant products for the long chains too
+        const bool spectral = t.nzlong > 0 && !(zl && std::strcmp(zl, "dense") == 0);
+        if (spectral) {
+            const size_t sm = (size_t)t.max_ext * 5 * sizeof(float2) + (size_t)(t.max_ext / t.Nz + t.Nz) * sizeof(float2) +
+                              (size_t)(t.max_ext / t.Nz) * sizeof(int);
+            if (sm > 200 * 1024) return cudaErrorInvalidConfiguration;
+            dim3 gl(t.nzlong, t.Nl, t.Ns * t.Nm);
+            lin_zlink_spectral_kernel<<<gl, kZspecThreads, sm, st>>>(t, g, phi, out, t.max_ext);
+        }
+        for (int part = spectral ? 1 : 0; part < 2; ++part) {
             if (wn[part] <= 0) continue;
             const size_t sm = (size_t)cap[part] * (2 * sizeof(float2) + 4 * sizeof(float)) + (size_t)(cap[part] / t.Nz) * sizeof(int);
             if (sm > 200 * 1024) return cudaErrorInvalidConfiguration;
