@@ -640,10 +640,13 @@ def test_calls_on_a_side_stream_and_interleaved_grids(torch_cuda):
         grid.close()
 
 
-@pytest.mark.parametrize("name", ["tiny", "cyclone", "kinetic"])
-def test_linear_rhs_parity_with_twist_shift_linking(torch_cuda, name):
-    """gx_boundary_set(1): the z operators act on the linked extended domains of Eq. 4.29."""
+@pytest.mark.parametrize("name,zlink", [("tiny", "spectral"), ("cyclone", "spectral"), ("kinetic", "spectral"), ("cyclone", "dense")])
+def test_linear_rhs_parity_with_twist_shift_linking(torch_cuda, monkeypatch, name, zlink):
+    """gx_boundary_set(1): the z operators act on the linked extended domains of Eq. 4.29.  Chains of more
+    than four links go through the harmonics of the extended domain (default) or through circulant products (GX_ZLINK=dense)."""
     torch = torch_cuda
+    if zlink == "dense":
+        monkeypatch.setenv("GX_ZLINK", "dense")
     from paper_2209_06731_b200 import binding
     cfg = I.named_config(name)
     geo = I.geometry_arrays(cfg)
