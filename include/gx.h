@@ -167,6 +167,22 @@ int gx_ssprk3_step(gx_grid* g, void* g_dev, double dt, void* cuda_stream);
 /* Linear part only (gx_rhs without -N), given phi; used to test the linear terms on their own. */
 int gx_linear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream);
 
+/* gx_linear_rhs for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): same arguments, same kernels, same result, but the one workspace the call
+ * needs -- the Dougherty field-particle moments mom[s][3][z][k] of Eq. 4.14-4.18, complex
+ * fp32 -- lives in a file-scope `static __device__` array of the library instead of the handle's
+ * allocation.  The call performs no cudaMalloc / cudaFree and calls no allocating library routine; the
+ * array's device address is resolved (cudaGetSymbolAddress) when the handle is created.
+ * Limit: 3 * Ns * Nz * nakx * naky <= GX_STATIC_SCRATCH_ELEMS complex values (4 MiB; every GPU that
+ * loads the library holds it until the process exits); larger grids return GX_ERR_UNSUPPORTED with a
+ * message naming both numbers (gx_last_error) and enqueue nothing.
+ * The array is shared by every call, every handle and every stream on a device and keeps the last
+ * call's contents.  Nothing in it has to start at zero: every element a call reads is written earlier in
+ * that same call.  Two calls that overlap on the GPU (different streams, or different handles on one
+ * device) race on it; calls on one stream are ordered and safe.  Other errors as gx_linear_rhs. */
+#define GX_STATIC_SCRATCH_ELEMS (1u << 19)
+int gx_linear_rhs_static(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream);
+
 int gx_query(gx_grid* g, int what, long long* value);
 
 /* Parity exports (HOST outputs; any pointer may be NULL): compact kx integers [nakx], ky integers

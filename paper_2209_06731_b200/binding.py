@@ -22,7 +22,7 @@ FAMILY_NAMES = {0: "scalar", 3: "row", 5: "rx", 6: "rxp", 7: "rxw"}
 
 EXPORTED = ["gx_grid_create", "gx_grid_destroy", "gx_box_set", "gx_species_set", "gx_adiabatic_set",
             "gx_dissipation_set", "gx_boundary_set", "gx_damping_set", "gx_geometry_set", "gx_nonlinear_rhs", "gx_nonlinear_rhs_em", "gx_field_solve_em", "gx_nonlinear_rhs_host",
-            "gx_field_solve", "gx_rhs", "gx_linear_rhs", "gx_ssprk3_step", "gx_query", "gx_export_maps",
+            "gx_field_solve", "gx_rhs", "gx_linear_rhs", "gx_linear_rhs_static", "gx_ssprk3_step", "gx_query", "gx_export_maps",
             "gx_export_tables", "gx_profile_set", "gx_profile_get", "gx_last_error", "gx_ubench_fp32", "gx_ubench_dft16"]
 
 _lib = None
@@ -60,6 +60,7 @@ def load():
     lib.gx_field_solve.argtypes = [vp, vp, vp, vp]
     lib.gx_rhs.argtypes = [vp, vp, vp, vp]
     lib.gx_linear_rhs.argtypes = [vp, vp, vp, vp, vp]
+    lib.gx_linear_rhs_static.argtypes = [vp, vp, vp, vp, vp]
     lib.gx_ssprk3_step.argtypes = [vp, vp, d, vp]
     lib.gx_query.argtypes = [vp, i, C.POINTER(C.c_longlong)]
     lib.gx_export_maps.argtypes = [vp, vp, vp, vp, vp, vp, vp]
@@ -159,6 +160,10 @@ def gx_rhs(h, g_ptr, out_ptr, stream=0):
 
 def gx_linear_rhs(h, g_ptr, phi_ptr, out_ptr, stream=0):
     _check(h, load().gx_linear_rhs(h, g_ptr, phi_ptr, out_ptr, stream))
+
+
+def gx_linear_rhs_static(h, g_ptr, phi_ptr, out_ptr, stream=0):
+    _check(h, load().gx_linear_rhs_static(h, g_ptr, phi_ptr, out_ptr, stream))
 
 
 def gx_ssprk3_step(h, g_ptr, dt, stream=0):
@@ -299,6 +304,11 @@ class Grid:
 
     def linear_rhs(self, g, phi, out):
         gx_linear_rhs(self.h, self._chk(g, "g"), self._chk(phi, "phi"), self._chk(out, "g"), self._stream())
+        return out
+
+    def linear_rhs_static(self, g, phi, out):
+        """gx_linear_rhs with its workspace in the library's static device array (no allocation in the call)."""
+        gx_linear_rhs_static(self.h, self._chk(g, "g"), self._chk(phi, "phi"), self._chk(out, "g"), self._stream())
         return out
 
     def ssprk3_step(self, g, dt):

@@ -8,6 +8,7 @@
 #include <cstdlib>
 #include <cstdint>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -138,6 +139,7 @@ struct gx_grid {
     std::vector<cudaEvent_t> ev_host;
     gx::LinTables lin;                                                  // linear-term tables
     float2* dphi_rhs = nullptr;                                         // phi of gx_rhs
+    float2* static_mom = nullptr;                                       // device address of gx_static_mom on this handle's device (gx_linear_rhs_static)
     float2 *drk_y = nullptr, *drk_k = nullptr;                          // SSP-RK3 stage and slope buffers
     size_t bytes = 0, lin_bytes = 0;
     bool profile = false;
@@ -146,7 +148,36 @@ struct gx_grid {
     std::string err;
 };
 
+// Scratch of the allocation-free entry point gx_linear_rhs_static: the Dougherty field-particle moments
+// mom[s][3][z][k] (Eq. 4.14-4.18) of ONE call.  4 MiB per GPU that loads the library, held until the process exits.
+// In host code `gx_static_mom` is only the host-side stand-in of the symbol, never a device address: the address is
+// resolved once per device by static_mom_address() below and handed to the kernels through LinTables::mom.
+constexpr size_t kStaticMomElems = GX_STATIC_SCRATCH_ELEMS;
+static __device__ __align__(256) float2 gx_static_mom[kStaticMomElems];
+
 namespace {
+
+constexpr int kMaxDevices = 64;
+std::mutex static_mom_mutex;
+float2* static_mom_of_device[kMaxDevices] = {};
+
+// Set-up time, with the handle's device current: device address of gx_static_mom on that device (cached per device).
+cudaError_t static_mom_address(float2** out) {
+    *out = nullptr;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(static_mom_mutex);
+    if (!static_mom_of_device[dev]) {
+        void* ptr = nullptr;
+        e = cudaGetSymbolAddress(&ptr, gx_static_mom);
+        if (e != cudaSuccess) return e;
+        static_mom_of_device[dev] = (float2*)ptr;
+    }
+    *out = static_mom_of_device[dev];
+    return cudaSuccess;
+}
 
 constexpr int kHostBufs = 3;       // Hermite-block buffers each way of gx_nonlinear_rhs_host
 bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
@@ -248,6 +279,7 @@ int gx_grid_create(int Nx, int Ny, int Nz, int Nl, int Nm, int Ns, gx_grid** out
     if (!g->ks) return fail(g, GX_ERR_UNSUPPORTED, "no kernel instantiation for this (Nx,Ny)");
     GX_CUDA(g, g->ks->prepare());      // per device and per handle: no process-wide cache of function attributes
     GX_CUDA(g, gx::lin_prepare());
+    GX_CUDA(g, static_mom_address(&g->static_mom));      // set-up for gx_linear_rhs_static (nothing allocated)
 
     gauss_laguerre(g->J, g->xj, g->wj);
     g->hT.resize((size_t)g->J * Nl);
@@ -817,6 +849,30 @@ int gx_linear_rhs(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_
     cudaError_t e = gx::lin_rhs(g->lin, (const float2*)g_dev, (const float2*)phi_dev, (float2*)out_dev,
                                 /*accumulate=*/false, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(g, e, "gx_linear_rhs");
+    return GX_OK;
+}
+
+// Same kernels and launch configuration as gx_linear_rhs; the only difference is where the moments workspace lives.
+// Calls no cudaMalloc / cudaFree / allocating library routine (lin_rhs only launches kernels).
+int gx_linear_rhs_static(gx_grid* g, const void* g_dev, const void* phi_dev, void* out_dev, void* cuda_stream) {
+    if (!g) return GX_ERR_ARG;
+    if (!g_dev || !phi_dev || !out_dev) return fail(g, GX_ERR_ARG, "gx_linear_rhs_static: null pointer");
+    const unsigned long long need = 3ull * (unsigned long long)g->Ns * g->Nz * (unsigned long long)g->nk;
+    if (need > kStaticMomElems)
+        return fail(g, GX_ERR_UNSUPPORTED, "gx_linear_rhs_static: moments workspace of " + std::to_string(need) +
+                    " complex values (3 Ns Nz nakx naky) exceeds the static scratch of " + std::to_string(kStaticMomElems) +
+                    " (GX_STATIC_SCRATCH_ELEMS); use gx_linear_rhs");
+    if (overlap(g_dev, out_dev, (size_t)g->Ns * g->Nm * g->Nl * g->Nz * g->nk * sizeof(float2)))
+        return fail(g, GX_ERR_ARG, "gx_linear_rhs_static: out must not alias g");
+    if (misaligned(g_dev) || misaligned(phi_dev) || misaligned(out_dev))
+        return fail(g, GX_ERR_ARG, "gx_linear_rhs_static: device pointers must be 16-byte aligned");
+    if (!g->geo_set || !g->have_lin_geo) return fail(g, GX_ERR_STATE, "gx_linear_rhs_static: full geometry not set");
+    if (!g->static_mom) return fail(g, GX_ERR_STATE, "gx_linear_rhs_static: static scratch address not resolved");
+    gx::LinTables t = g->lin;            // plain struct of device pointers and scalars: a copy owns nothing
+    t.mom = g->static_mom;               // every element read is written by lin_moments_kernel earlier in this call
+    cudaError_t e = gx::lin_rhs(t, (const float2*)g_dev, (const float2*)phi_dev, (float2*)out_dev,
+                                /*accumulate=*/false, (cudaStream_t)cuda_stream);
+    if (e != cudaSuccess) return cuda_fail(g, e, "gx_linear_rhs_static");
     return GX_OK;
 }
 

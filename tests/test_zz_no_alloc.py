@@ -1,0 +1,76 @@
+"""gx_linear_rhs_static (include/gx.h): the allocation-free variant of gx_linear_rhs, whose Dougherty-moments workspace
+is a file-scope static __device__ array of the library.  Checked against the existing path (gx_linear_rhs, workspace
+owned by the handle) on two calls in a row, and against the fp64 oracle.  Collected last on purpose (test_zz_*)."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import gx_oracle as O
+from paper_2209_06731_b200 import inputs as I
+
+pytestmark = pytest.mark.gpu
+TOL = 2e-5                      # the bar of tests/test_parity_gpu.py
+
+
+@pytest.fixture(scope="module")
+def torch_cuda():
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def _state_and_phi(cfg, geo):
+    G = I.make_state(cfg, geo)
+    Phi = O.field_solve(G, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species,
+                        tau_fac=cfg.tau_fac, adiabatic=(cfg.Ns == 1)).astype(np.complex64)
+    return G, Phi
+
+
+@pytest.mark.parametrize("name", ["tiny", "cyclone", "kinetic"])
+def test_static_scratch_entry_matches_existing_path_on_two_calls_in_a_row(torch_cuda, name):
+    torch = torch_cuda
+    from paper_2209_06731_b200 import binding
+    cfg = I.named_config(name)
+    geo = I.geometry_arrays(cfg)
+    grid = binding.Grid(cfg, geo)
+    # two different states: the second call finds the first call's moments in the shared static array
+    states = [_state_and_phi(dataclasses.replace(cfg, seed=cfg.seed + 17 * i), geo) for i in range(2)]
+    dev = [(torch.from_numpy(G).cuda(), torch.from_numpy(Phi).cuda()) for G, Phi in states]
+    want = []
+    for g, phi in dev:                                         # existing path (also loads every kernel the new one launches)
+        out = torch.full_like(g, float("nan"))
+        grid.linear_rhs(g, phi, out)
+        want.append(out)
+    got = [torch.full_like(g, float("nan")) for g, _ in dev]
+    torch.cuda.synchronize()
+    free_before = torch.cuda.mem_get_info()[0]
+    for (g, phi), out in zip(dev, got):                        # two calls in a row, no synchronisation in between
+        grid.linear_rhs_static(g, phi, out)
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free_before         # the calls took no device memory
+    assert not torch.equal(want[0], want[1])                   # the two calls really had different inputs
+    for i in range(2):
+        a, b = got[i].cpu().numpy(), want[i].cpu().numpy()
+        assert np.all(np.isfinite(a))
+        assert O.relative_max_error(a, b) <= TOL, i
+    if name != "kinetic":                                      # and against the oracle (seconds for these sizes)
+        import gx_linear as OL
+        G, Phi = states[1]
+        ref = OL.linear_rhs(G, Phi, cfg.Nx, cfg.Ny, cfg.dkx, cfg.dky, cfg.shat, geo, cfg.species)
+        assert O.relative_max_error(got[1].cpu().numpy(), ref) <= TOL
+    grid.close()
+
+
+def test_static_scratch_entry_rejects_grids_beyond_its_limit(torch_cuda):
+    """hires plane: 3 * Ns * Nz * nakx * naky = 3 * 32 * 171 * 32 = 525 312 > GX_STATIC_SCRATCH_ELEMS = 524 288."""
+    torch = torch_cuda
+    from paper_2209_06731_b200 import binding as B
+    h = B.gx_grid_create(256, 96, 32, 8, 2, 1)
+    buf = torch.zeros(64, dtype=torch.complex64, device="cuda")
+    with pytest.raises(B.GxError) as e:
+        B.gx_linear_rhs_static(h, buf.data_ptr(), buf.data_ptr(), buf.data_ptr() + 256)
+    assert e.value.code == B.GX_ERR_UNSUPPORTED
+    assert "525312" in str(e.value) and "524288" in str(e.value)
+    B.gx_grid_destroy(h)
