@@ -41,17 +41,22 @@ def workload_name(cfg):
 
 # ------------------------------------------------------------------------------- clocks
 class ClockSampler:
-    """Samples SM clock and throttle reasons with NVML in a thread while the timed region runs."""
+    """Samples SM clock and throttle reasons with NVML in a thread while the timed region runs.  The thread starts
+    sampling when arm() is called -- by the timed loop right after its last launch is enqueued, while the GPU still
+    works through the queue -- so that no NVML call competes with the kernel launches for the driver."""
 
     def __init__(self, index=0, period=0.01):
         self.samples, self.reasons, self.max_mhz = [], set(), None
         self.period, self._stop, self._thr, self.ok = period, threading.Event(), None, False
+        self._armed = threading.Event()
         try:
             import pynvml
             pynvml.nvmlInit()
             self.nv = pynvml
             self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
             self.max_mhz = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            pynvml.nvmlDeviceGetClockInfo(self.h, pynvml.NVML_CLOCK_SM)           # first-use cost of the queries, discarded
+            pynvml.nvmlDeviceGetCurrentClocksEventReasons(self.h)
             self.ok = True
         except Exception:
             self.ok = False
@@ -60,7 +65,8 @@ class ClockSampler:
         nv = self.nv
         names = {"hw_slowdown": 0x8, "sw_thermal_slowdown": 0x20, "hw_thermal_slowdown": 0x40,
                  "hw_power_brake_slowdown": 0x80, "sw_power_cap": 0x4}
-        while not self._stop.is_set():
+        self._armed.wait()
+        while True:
             try:
                 self.samples.append(int(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)))
                 r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
@@ -69,16 +75,21 @@ class ClockSampler:
                         self.reasons.add(k)
             except Exception:
                 pass
-            time.sleep(self.period)
+            if self._stop.wait(self.period):
+                break
 
     def __enter__(self):
-        if self.ok:
+        if self.ok and self._thr is None:
             self._thr = threading.Thread(target=self._run, daemon=True)
             self._thr.start()
         return self
 
+    def arm(self):
+        self._armed.set()
+
     def __exit__(self, *a):
         self._stop.set()
+        self._armed.set()
         if self._thr:
             self._thr.join()
 
@@ -373,17 +384,20 @@ def run_gpu(args):
         k = i % nsets
         grid.nonlinear_rhs(gs[k], phis[k], outs[k])
 
+    sampler = ClockSampler(local_rank)      # NVML initialised and the (idle) thread started before the warm-up, not at
+    sampler.__enter__()                     # the edge of the timed region
     for i in range(args.warmup):
         step(i)
     torch.cuda.synchronize()
     D.barrier()
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clk:
+    with sampler as clk:
         torch.cuda.synchronize()
         ev0.record()
         for i in range(args.steps):
             step(i)
         ev1.record()
+        clk.arm()                           # everything is enqueued: sample the clocks while the GPU runs it
         torch.cuda.synchronize()
     D.barrier()
     sec = ev0.elapsed_time(ev1) * 1e-3
