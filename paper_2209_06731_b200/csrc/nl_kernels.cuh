@@ -567,12 +567,15 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
                 const int h = r / HB, rp = r - h * HB;
                 const int row = C::ADJ ? bt * RB + 2 * rp + h : bt * HB + rp + h * (NX / 2);
                 float2 v[R2];
+                float2 dv[R2];                                       // requested before the transform (L2 round trip under it)
+#pragma unroll
+                for (int k2 = 0; k2 < R2; ++k2) dv[k2] = __ldcg(dchi + (size_t)(k1 * R2 + k2) * NX + row);
 #pragma unroll
                 for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[(k1 * R2 + n2) * RB + r];
                 dft<R2, +1>(v);
 #pragma unroll
                 for (int k2 = 0; k2 < R2; ++k2) {
-                    const float2 d = dchi[(size_t)(k1 * R2 + k2) * NX + row];
+                    const float2 d = dv[k2];
                     S[(k1 * R2 + k2) * RB + r] = make_float2(fmaf(d.y, v[k2].x, -d.x * v[k2].y), 0.f);
                 }
             }
@@ -598,12 +601,15 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
                     const int r = rp + h * HB;
                     const int row = C::ADJ ? bt * RB + 2 * rp + h : bt * HB + rp + h * (NX / 2);
                     float2 v[R2];
+                    float2 dv[R2];                                   // requested before the transform: the L2 round trip passes under it
+#pragma unroll
+                    for (int k2 = 0; k2 < R2; ++k2) dv[k2] = __ldcg(dchi + (size_t)(k1 * R2 + k2) * NX + row);
 #pragma unroll
                     for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[(k1 * R2 + n2) * RB + r];
                     dft<R2, +1>(v);
 #pragma unroll
                     for (int k2 = 0; k2 < R2; ++k2) {
-                        const float2 d = dchi[(size_t)(k1 * R2 + k2) * NX + row];
+                        const float2 d = dv[k2];
                         const float b = fmaf(d.y, v[k2].x, -d.x * v[k2].y);   // d_y chi d_x g - d_x chi d_y g
                         if (h == 0) c[k2].x = b; else c[k2].y = b;
                     }

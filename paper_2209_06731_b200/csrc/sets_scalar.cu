@@ -29,7 +29,7 @@ using C128x64  = gx::PlaneCfg<128, 64, 16, 8, 8, 8, 64, 512, 1, true>;
 using B192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, 64, 448, 2, true>;
 using C192x64  = gx::PlaneCfg<192, 64, 16, 12, 8, 8, 64, 512, 1, true>;
 using B256x64  = gx::PlaneCfg<256, 64, 16, 16, 8, 8, 64, 256, 1, true>;
-using B256x96  = gx::PlaneCfg<256, 96, 16, 16, 8, 12, 64, 384, 1, true>;
+using B256x96  = gx::PlaneCfg<256, 96, 16, 16, 8, 12, 128, 512, 1, true>;    // RB 128: every y phase has 448-1536 items for 512 threads (RB 64 / 384 threads: 224-256 items in the two heavy phases)
 using B192x192 = gx::PlaneCfg<192, 192, 16, 12, 12, 16, 16, 384, 1, false>;
 using B64x192  = gx::PlaneCfg<64, 192, 8, 8, 12, 16, 16, 256, 2, true>;   // RB 16: 92 KB, two CTAs per SM
 const KernelSet kKernelSets[] = {
