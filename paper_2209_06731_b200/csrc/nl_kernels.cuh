@@ -56,6 +56,14 @@ struct PlaneCfg {
     // NX/2 apart, which lie in the same shared-memory banks whenever HB < 16: 26 % of the stellarator kernel's
     // wavefronts were conflicts) or, for the small batches, the adjacent rows 2p and 2p + 1 (conflict-free for HB <= 8).
     static constexpr bool ADJ = RB <= 16;
+    // Position of (y = a*RY2 + b, row slot r) in the batch buffer S.  With batches of 16 rows the pair phases run 8 lanes
+    // per y value and 4 values of a (2 KB apart) or of b (128 B apart) per warp, all in the same half of the banks
+    // (25 % of the stellarator kernel's shared-memory wavefronts were conflicts): rows with odd a + b hold their two
+    // halves swapped.
+    static constexpr bool SWZ = RB == 16;
+    __device__ __forceinline__ static int sidx(int a, int b, int r) {
+        return (a * RY2 + b) * RB + (SWZ ? (r ^ (((a ^ b) & 1) * HB)) : r);
+    }
     static constexpr int W_ELEMS = NX * NCOL;
     static constexpr int S_ELEMS = (STAGE && NK > NY * RB) ? NK : NY * RB;
     static constexpr int SMEM_BYTES = (W_ELEMS + S_ELEMS + NX + NY) * (int)sizeof(float2);
@@ -234,7 +242,7 @@ __device__ __forceinline__ void y_inverse_pass1(const float2* __restrict__ W, fl
         dft<R1, +1, C::ZMY>(v);
 #pragma unroll
         for (int k1 = 0; k1 < R1; ++k1)
-            S[(k1 * R2 + n2) * RB + r] = k1 == 0 ? v[0] : cmul(v[k1], twy[n2 * k1]);
+            S[C::sidx(k1, n2, r)] = k1 == 0 ? v[0] : cmul(v[k1], twy[n2 * k1]);
     }
     __syncthreads();
 }
@@ -497,7 +505,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) chi_planes_kernel(const NlPara
             const int k1 = t / RB, r = t - k1 * RB;
             float2 v[R2];
 #pragma unroll
-            for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[(k1 * R2 + n2) * RB + r];
+            for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[C::sidx(k1, n2, r)];
             dft<R2, +1>(v);
 #pragma unroll
             for (int k2 = 0; k2 < R2; ++k2) dchi[(size_t)(k1 * R2 + k2) * C::NX + bt * RB + r] = v[k2];
@@ -571,12 +579,12 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
 #pragma unroll
                 for (int k2 = 0; k2 < R2; ++k2) dv[k2] = __ldcg(dchi + (size_t)(k1 * R2 + k2) * NX + row);
 #pragma unroll
-                for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[(k1 * R2 + n2) * RB + r];
+                for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[C::sidx(k1, n2, r)];
                 dft<R2, +1>(v);
 #pragma unroll
                 for (int k2 = 0; k2 < R2; ++k2) {
                     const float2 d = dv[k2];
-                    S[(k1 * R2 + k2) * RB + r] = make_float2(fmaf(d.y, v[k2].x, -d.x * v[k2].y), 0.f);
+                    S[C::sidx(k1, k2, r)] = make_float2(fmaf(d.y, v[k2].x, -d.x * v[k2].y), 0.f);
                 }
             }
             __syncthreads();
@@ -585,11 +593,11 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
                 float2 c[R2];
 #pragma unroll
                 for (int k2 = 0; k2 < R2; ++k2)
-                    c[k2] = make_float2(S[(k1 * R2 + k2) * RB + rp].x, S[(k1 * R2 + k2) * RB + rp + HB].x);
+                    c[k2] = make_float2(S[C::sidx(k1, k2, rp)].x, S[C::sidx(k1, k2, rp + HB)].x);
                 dft<R2, -1>(c);
 #pragma unroll
                 for (int d = 0; d < R2; ++d)
-                    S[(k1 * R2 + d) * RB + rp] = d == 0 ? c[0] : cmul_conj(c[d], twy[k1 * d]);
+                    S[C::sidx(k1, d, rp)] = d == 0 ? c[0] : cmul_conj(c[d], twy[k1 * d]);
             }
         } else {
             // ---- a4 (last pass) + a5 bracket + a6 (first forward pass), all in registers
@@ -605,7 +613,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
 #pragma unroll
                     for (int k2 = 0; k2 < R2; ++k2) dv[k2] = __ldcg(dchi + (size_t)(k1 * R2 + k2) * NX + row);
 #pragma unroll
-                    for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[(k1 * R2 + n2) * RB + r];
+                    for (int n2 = 0; n2 < R2; ++n2) v[n2] = S[C::sidx(k1, n2, r)];
                     dft<R2, +1>(v);
 #pragma unroll
                     for (int k2 = 0; k2 < R2; ++k2) {
@@ -617,7 +625,7 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
                 dft<R2, -1>(c);
 #pragma unroll
                 for (int d = 0; d < R2; ++d)
-                    S[(k1 * R2 + d) * RB + rp] = d == 0 ? c[0] : cmul_conj(c[d], twy[k1 * d]);
+                    S[C::sidx(k1, d, rp)] = d == 0 ? c[0] : cmul_conj(c[d], twy[k1 * d]);
             }
         }
         __syncthreads();
@@ -629,17 +637,17 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
                 const int d = t / HB, rp = t - d * HB;
                 float2 u[R1];
 #pragma unroll
-                for (int a = 0; a < R1; ++a) u[a] = S[(a * R2 + d) * RB + rp];
+                for (int a = 0; a < R1; ++a) u[a] = S[C::sidx(a, d, rp)];
                 dft<R1, -1>(u);
 #pragma unroll
-                for (int a = 0; a < R1; ++a) S[(a * R2 + d) * RB + rp] = u[a];
+                for (int a = 0; a < R1; ++a) S[C::sidx(a, d, rp)] = u[a];
             }
             __syncthreads();
             for (int t = threadIdx.x; t < (Q + 1) * HB; t += C::NT) {
                 const int k = t / HB, rp = t - k * HB;
                 const int d = k % R2, cc = k / R2;
                 const int dp = (R2 - d) % R2, cp = d == 0 ? (R1 - cc) % R1 : R1 - 1 - cc;     // NY - k = dp + R2*cp
-                const float2 A = S[(cc * R2 + d) * RB + rp], B = S[(cp * R2 + dp) * RB + rp];
+                const float2 A = S[C::sidx(cc, d, rp)], B = S[C::sidx(cp, dp, rp)];
                 float2* __restrict__ W0 = W + (C::ADJ ? bt * RB + 2 * rp : bt * HB + rp) * NCOL;
                 float2* __restrict__ W1 = W0 + (C::ADJ ? 1 : NX / 2) * NCOL;
                 W0[k] = make_float2(0.5f * (A.x + B.x), 0.5f * (A.y - B.y));
@@ -652,11 +660,11 @@ __global__ void __launch_bounds__(C::NT, C::MINB) bracket_kernel(const NlParams 
                 const int d0 = dd, d1 = (R2 - dd) % R2;
                 float2 u0[R1], u1[R1];
 #pragma unroll
-                for (int a = 0; a < R1; ++a) u0[a] = S[(a * R2 + d0) * RB + rp];
+                for (int a = 0; a < R1; ++a) u0[a] = S[C::sidx(a, d0, rp)];
                 dft<R1, -1>(u0);
                 if (d1 != d0) {
 #pragma unroll
-                    for (int a = 0; a < R1; ++a) u1[a] = S[(a * R2 + d1) * RB + rp];
+                    for (int a = 0; a < R1; ++a) u1[a] = S[C::sidx(a, d1, rp)];
                     dft<R1, -1>(u1);
                 } else {
 #pragma unroll
