@@ -49,7 +49,7 @@ def test_static_scratch_entry_matches_existing_path_on_two_calls_in_a_row(torch_
     for (g, phi), out in zip(dev, got):                        # two calls in a row, no synchronisation in between
         grid.linear_rhs_static(g, phi, out)
     torch.cuda.synchronize()
-    assert torch.cuda.mem_get_info()[0] == free_before         # the calls took no device memory
+    assert torch.cuda.mem_get_info()[0] >= free_before         # the calls took no device memory
     assert not torch.equal(want[0], want[1])                   # the two calls really had different inputs
     for i in range(2):
         a, b = got[i].cpu().numpy(), want[i].cpu().numpy()
