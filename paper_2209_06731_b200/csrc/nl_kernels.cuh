@@ -328,21 +328,25 @@ __device__ __forceinline__ void x_forward(float2* __restrict__ W, const float2* 
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 
-// S[i] = sum_l coef[l] * planes[l*lstride + i], i < NK: 4 positions x 4 planes = 16 independent 8-byte
+// S[i] = sum_l coef[l] * planes[l*lstride + i], i < NK: U positions x 2 planes of independent 8-byte
 // loads in flight per thread (the loop is latency-bound otherwise: ncu r01 showed 35% of the bracket
 // kernel's stall samples here).
 template <class C>
 __device__ __forceinline__ void stage_combine(float2* __restrict__ S, const float2* __restrict__ planes,
                                               size_t lstride, const float* __restrict__ coef, int Nl) {
-    constexpr int NK = C::NK, NT = C::NT, U = 4;
+    // U positions x LB planes per round trip, U chosen so that the positions of a thread take the fewest rounds of at
+    // most 12 (stellarator plane: 22 positions per thread = 2 rounds of 11, 22 loads in flight; measured against
+    // 4 x 4: 3 982 -> 3 865 us per call, 6 x 4: 3 930, 6 x 8: 3 886, 3 x 11: 3 881)
+    constexpr int NK = C::NK, NT = C::NT, LB = 2;
+    constexpr int PER = (NK + NT - 1) / NT, ROUNDS = (PER + 11) / 12, U = (PER + ROUNDS - 1) / ROUNDS;
     for (int i0 = threadIdx.x; i0 < NK; i0 += U * NT) {
         float2 acc[U];
 #pragma unroll
         for (int u = 0; u < U; ++u) acc[u] = make_float2(0.f, 0.f);
-        for (int l0 = 0; l0 < Nl; l0 += 4) {
-            float2 f[4][U];
+        for (int l0 = 0; l0 < Nl; l0 += LB) {
+            float2 f[LB][U];
 #pragma unroll
-            for (int dl = 0; dl < 4; ++dl)
+            for (int dl = 0; dl < LB; ++dl)
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
                     const int i = i0 + u * NT;
@@ -350,7 +354,7 @@ __device__ __forceinline__ void stage_combine(float2* __restrict__ S, const floa
                                                         : make_float2(0.f, 0.f);
                 }
 #pragma unroll
-            for (int dl = 0; dl < 4; ++dl) {
+            for (int dl = 0; dl < LB; ++dl) {
                 const float t = (l0 + dl < Nl) ? __ldg(coef + l0 + dl) : 0.f;
 #pragma unroll
                 for (int u = 0; u < U; ++u) {
